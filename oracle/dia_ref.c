@@ -1,0 +1,163 @@
+/* dia_ref.c -- CPU ORACLE (test infrastructure only; see dia_ref.h).
+ *
+ * Plain FP64 loops in the paper's order and notation.  No blocking, fusion or reordering
+ * beyond what the definitions state; OpenMP (optional) splits image rows over threads and
+ * sums per-thread partials in thread-index order, so results are deterministic for a fixed
+ * thread count.
+ */
+#include "dia_ref.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int dia_ref_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+static int check_cfg(const dia_ref_config* c) {
+  if (!c) return 0;
+  if (c->m < 1 || (c->m % 2) == 0) return 0;
+  if (c->n_rows < c->m || c->n_cols < c->m) return 0;
+  if (c->loss != DIA_REF_LOSS_GAUSSIAN && c->loss != DIA_REF_LOSS_HUBER) return 0;
+  if (c->noise != DIA_REF_NOISE_MODEL && c->noise != DIA_REF_NOISE_FIXED) return 0;
+  if (c->noise == DIA_REF_NOISE_MODEL && !(c->gain > 0.0 && c->sigma0 >= 0.0)) return 0;
+  if (c->loss == DIA_REF_LOSS_HUBER && !(c->huber_c > 0.0)) return 0;
+  return 1;
+}
+
+/* Eq. 2: M_ij = sum_lm K_lm R_(i+l)(j+m) + B0, cross-correlation, no flip
+ * (reading R2).  (i, j) are image coordinates of a valid pixel. */
+static double model_pixel(const float* R, int n_cols, int m, const float* theta, int i, int j) {
+  const int h = (m - 1) / 2;
+  double M = 0.0;
+  for (int a = 0; a < m; ++a)
+    for (int b = 0; b < m; ++b)
+      M += (double)theta[a * m + b] * (double)R[(size_t)(i - h + a) * n_cols + (j - h + b)];
+  return M + (double)theta[m * m];
+}
+
+int dia_ref_model(const dia_ref_config* cfg, const float* R, const float* theta, double* M) {
+  if (!check_cfg(cfg) || !R || !theta || !M) return DIA_REF_ERR_INVALID_ARG;
+  const int m = cfg->m, h = (m - 1) / 2;
+  const int vr = cfg->n_rows - m + 1, vc = cfg->n_cols - m + 1;
+#pragma omp parallel for schedule(static)
+  for (int i = 0; i < vr; ++i)
+    for (int j = 0; j < vc; ++j)
+      M[(size_t)i * vc + j] = model_pixel(R, cfg->n_cols, m, theta, i + h, j + h);
+  return DIA_REF_OK;
+}
+
+/* One epoch of c.1.  part_* are per-call scratch of size (m*m+1). */
+static void eval_one(const dia_ref_config* cfg, const float* R, const float* I,
+                     const unsigned char* mask, const float* var, const float* theta,
+                     double* loss_out, double* grad, double* gscale) {
+  const int m = cfg->m, h = (m - 1) / 2, np = m * m + 1;
+  const int nr = cfg->n_rows, nc = cfg->n_cols;
+  int nthreads = dia_ref_num_threads();
+  double* tl = (double*)calloc((size_t)nthreads, sizeof(double));
+  double* tg = (double*)calloc((size_t)nthreads * np, sizeof(double));
+  double* ts = (double*)calloc((size_t)nthreads * np, sizeof(double));
+
+#pragma omp parallel
+  {
+#ifdef _OPENMP
+    const int tid = omp_get_thread_num();
+#else
+    const int tid = 0;
+#endif
+    double L = 0.0;
+    double* g = tg + (size_t)tid * np;
+    double* s = ts + (size_t)tid * np;
+#pragma omp for schedule(static)
+    for (int i = h; i < nr - h; ++i) {
+      for (int j = h; j < nc - h; ++j) {
+        const size_t p = (size_t)i * nc + j;
+        if (mask && mask[p] == 0) continue;                 /* reading R4 */
+        const double M = model_pixel(R, nc, m, theta, i, j);
+        double v, bp;
+        if (cfg->noise == DIA_REF_NOISE_MODEL) {
+          /* Eq. 6: sigma^2 = sigma0^2/F^2 + M/(G F); reading R1: photon
+           * term uses max(M, 0) and its derivative is 0 there. */
+          const double F = cfg->flat ? (double)cfg->flat[p] : 1.0;
+          const double a_ij = cfg->sigma0 * cfg->sigma0 / (F * F);
+          const double b_ij = 1.0 / (cfg->gain * F);
+          v = a_ij + b_ij * (M > 0.0 ? M : 0.0);
+          bp = (M > 0.0) ? b_ij : 0.0;
+        } else {
+          v = (double)var[p];
+          bp = 0.0;
+        }
+        const double r = (double)I[p] - M;
+        const double sd = sqrt(v);
+        const double z = r / sd;
+        double rho, psi;
+        if (cfg->loss == DIA_REF_LOSS_HUBER && fabs(z) > cfg->huber_c) {
+          /* Eq. 12 */
+          rho = cfg->huber_c * (fabs(z) - 0.5 * cfg->huber_c);
+          psi = (z > 0.0) ? cfg->huber_c : -cfg->huber_c;
+        } else {
+          rho = 0.5 * z * z;
+          psi = z;
+        }
+        /* Eq. 8 / Eq. 13 without theta-independent constants (reading R3); in FIXED mode
+         * sum ln sigma is a constant and is dropped. */
+        L += rho;
+        if (cfg->noise == DIA_REF_NOISE_MODEL) L += 0.5 * log(v);
+        /* D1: w = dL/dM = -psi/s - psi z b'/(2v) + b'/(2v) */
+        const double w = -psi / sd - psi * z * bp / (2.0 * v) + bp / (2.0 * v);
+        const double aw = fabs(w);
+        for (int a = 0; a < m; ++a)
+          for (int b = 0; b < m; ++b) {
+            const double x = (double)R[(size_t)(i - h + a) * nc + (j - h + b)];
+            g[a * m + b] += w * x;
+            s[a * m + b] += aw * fabs(x);
+          }
+        g[m * m] += w;
+        s[m * m] += aw;
+      }
+    }
+    tl[tid] = L;
+  }
+  double L = 0.0;
+  for (int t = 0; t < nthreads; ++t) L += tl[t];
+  *loss_out = L;
+  for (int k = 0; k < np; ++k) {
+    double gs = 0.0, ss = 0.0;
+    for (int t = 0; t < nthreads; ++t) {
+      gs += tg[(size_t)t * np + k];
+      ss += ts[(size_t)t * np + k];
+    }
+    grad[k] = gs;
+    if (gscale) gscale[k] = ss;
+  }
+  free(tl); free(tg); free(ts);
+}
+
+int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epochs,
+                           const float* I, const unsigned char* mask, const float* var,
+                           const float* theta, double* loss, double* grad, double* grad_scale) {
+  if (!check_cfg(cfg) || !R || !I || !theta || !loss || !grad || n_epochs < 1)
+    return DIA_REF_ERR_INVALID_ARG;
+  if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
+  const size_t npix = (size_t)cfg->n_rows * cfg->n_cols;
+  const int np = cfg->m * cfg->m + 1;
+  for (int e = 0; e < n_epochs; ++e)
+    eval_one(cfg, R, I + e * npix, mask ? mask + e * npix : NULL, var ? var + e * npix : NULL,
+             theta + (size_t)e * np, loss + e, grad + (size_t)e * np,
+             grad_scale ? grad_scale + (size_t)e * np : NULL);
+  return DIA_REF_OK;
+}
+
+/* Eq. 14: Q = N ln( sqrt(2 pi) erf(c/sqrt 2) + 2 exp(-c^2/2)/c ). */
+double dia_ref_huber_Q(double c, double N) {
+  const double pi = 3.14159265358979323846;
+  return N * log(sqrt(2.0 * pi) * erf(c / sqrt(2.0)) + 2.0 * exp(-0.5 * c * c) / c);
+}

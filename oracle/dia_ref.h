@@ -1,0 +1,89 @@
+/* dia_ref.h -- CPU ORACLE for the DIA objective/gradient/fit.  TEST INFRASTRUCTURE ONLY.
+ *
+ * A plain, slow, FP64 restatement of what the hot path computes, written from the paper
+ * (PAPER.md = arxiv 2104.13715, "PyTorchDIA") and the readings listed in DESIGN.md.
+ * It shares no code, header, table or helper with the CUDA library in
+ * paper_2104_13715_b200/csrc and is used only by tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs.  All pointers are HOST pointers.
+ *
+ * Layout conventions (identical in meaning to include/dia.h, restated here on purpose):
+ *   images row-major [n_rows][n_cols]; kernel K row-major [m][m], K[a][b] with
+ *   a = l + h, b = mm + h, h = (m-1)/2, (l, mm) the kernel coordinates of Eq. 2
+ *   (PAPER.md:60); theta = [K (m*m values), B0]; the valid set is
+ *   h <= i < n_rows-h, h <= j < n_cols-h intersected with mask != 0.
+ *
+ * Pin status (tests/test_oracle_*.py): model, noise, both losses, gradient, B08 solve,
+ * fixed-weight fit and planted recovery are pinned.  The free-running Adam->L-BFGS fit on
+ * NOISY data is "parity unpinned" beyond its fixed-weight / planted special cases
+ * (no external value exists).
+ */
+#ifndef DIA_REF_H
+#define DIA_REF_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { DIA_REF_OK = 0, DIA_REF_ERR_INVALID_ARG = -1, DIA_REF_ERR_ALLOC = -3, DIA_REF_ERR_NOT_PD = -5 };
+enum { DIA_REF_LOSS_GAUSSIAN = 0 /* Eq. 8 */, DIA_REF_LOSS_HUBER = 1 /* Eq. 13 */ };
+enum { DIA_REF_NOISE_MODEL = 0 /* Eq. 6 */, DIA_REF_NOISE_FIXED = 1 /* caller variance */ };
+enum { DIA_REF_FIT_CONVERGED_GRAD = 0, DIA_REF_FIT_CONVERGED_CHANGE = 1, DIA_REF_FIT_MAX_ITERS = 2,
+       DIA_REF_FIT_NONFINITE = 3 };
+
+typedef struct {
+  int n_rows, n_cols, m;      /* m odd */
+  int loss;    double huber_c;          /* c = 1.345 default */
+  int noise;   double sigma0, gain;     /* Eq. 6 parameters */
+  const float* flat;                    /* [n_rows][n_cols] or NULL => F == 1 */
+} dia_ref_config;
+
+typedef struct {                        /* PAPER.md:242-244; [reading] marks DESIGN.md readings */
+  double lr_kernel, lr_b0;              /* 1e-3; 1, 10 or 100 */
+  double adam_beta1, adam_beta2, adam_eps;          /* [reading R5] 0.9, 0.999, 1e-8 */
+  double tol_switch;                    /* 1e-6 */
+  double lbfgs_lr;                      /* 1.0 */
+  int    lbfgs_history;                 /* [reading R7] 100 */
+  int    lbfgs_backtrack;               /* [reading R7] 1 */
+  double tol_change_rel, tol_grad_abs, tol_grad_rel;   /* 1e-8, 1e-7, [reading] 0 = off */
+  int    max_adam_iters, max_lbfgs_iters;              /* [reading] 20000, 500 */
+  int    force_adam_iters, force_lbfgs_iters;          /* [reading] -1 = off (lock-step mode) */
+} dia_ref_fit_opts;
+
+typedef struct {
+  double loss, grad_inf_norm, photometric_scale;
+  int n_adam, n_lbfgs, n_evals, status;
+} dia_ref_fit_result;
+
+void dia_ref_default_fit_opts(dia_ref_fit_opts* o);
+
+/* Model image of Eq. 2 on the valid region: M [n_rows-m+1][n_cols-m+1] (FP64). */
+int dia_ref_model(const dia_ref_config* cfg, const float* R, const float* theta, double* M);
+
+/* Loss and gradient (SURVEY/DESIGN c.1).  theta float32 [n_epochs][m*m+1];
+ * loss [n_epochs]; grad [n_epochs][m*m+1].  grad_scale (nullable) receives
+ * S_p = sum_V |w_ij| |X_p(i,j)|, the cancellation-free magnitude used by the parity protocol. */
+int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epochs,
+                           const float* I, const unsigned char* mask, const float* var,
+                           const float* theta, double* loss, double* grad, double* grad_scale);
+
+/* Adam -> L-BFGS fit (DESIGN c.2), one epoch after another.  theta in/out float32. */
+int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
+                int n_epochs, const float* I, const unsigned char* mask, const float* var,
+                float* theta, dia_ref_fit_result* result);
+
+/* B08 iterated normal-equation solve (DESIGN c.3).  One epoch.
+ * var_fixed (nullable): if given, every iteration uses this variance map instead of Eq. 6.
+ * theta out FP64 [m*m+1]; H (nullable) out [(m*m+1)^2] row-major, the last normal matrix. */
+int dia_ref_b08_solve(const dia_ref_config* cfg, const float* R, const float* I,
+                      const unsigned char* mask, const float* var_fixed, int n_iters,
+                      int clip_last, double* theta, double* H);
+
+/* Normalising constant Q of Eq. 14 for N pixels. */
+double dia_ref_huber_Q(double c, double N);
+
+int dia_ref_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
