@@ -1,0 +1,122 @@
+/* dia.h -- C ABI of the B200-native DIA objective/gradient/fit engine.
+ *
+ * Hot path of PyTorchDIA (arxiv 2104.13715; citations are PAPER.md:<line>): the repeated
+ * evaluation of the objective and its analytic gradient for the B08 discrete-pixel kernel
+ * model, the on-device Adam -> L-BFGS optimiser with its convergence test, and a batched mode
+ * that fits many target epochs against one resident reference.
+ *
+ * CONVENTIONS
+ *  - Every `d_*` pointer is a DEVICE pointer owned by the caller (e.g. a torch tensor's
+ *    data_ptr()); the library never frees or reallocates caller memory.  Struct pointers
+ *    (dia_config, dia_fit_opts) are HOST pointers read during the call.
+ *  - Images are row-major [n_rows][n_cols] float32.  The kernel K is row-major [m][m] with
+ *    K[a][b], a = l + h, b = mm + h, h = (m-1)/2, (l, mm) the kernel coordinates of Eq. 2
+ *    (PAPER.md:60): M_ij = sum_ab K[a][b] R[i-h+a][j-h+b] + B0 -- a cross-correlation, no flip.
+ *    theta = [K (m*m values, row-major), B0], m*m+1 parameters per epoch.
+ *  - The valid set V is h <= i < n_rows-h, h <= j < n_cols-h, intersected with
+ *    mask != 0 when a mask is given.  Pixels of I, mask, var, flat outside V are never read.
+ *  - Every call is ASYNCHRONOUS on cfg.stream and performs no host synchronisation
+ *    (dia_create / dia_destroy may).  Outputs are valid once the caller synchronises the stream.
+ *  - Argument errors are detected on the host before any launch and return a negative code
+ *    with outputs untouched.  Numerical failure (non-finite loss) is data dependent and is
+ *    reported per epoch in dia_fit_result.status, not by return code.
+ *  - Same inputs => bit-identical outputs on repeated calls (fixed tile->block map, fixed-order
+ *    FP64 reductions, no floating-point atomics).
+ *  - There is no CPU fallback: without a CUDA device every entry point fails with DIA_ERR_CUDA.
+ */
+#ifndef DIA_H
+#define DIA_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dia_handle dia_handle;     /* opaque; owns only its own workspace */
+
+enum { DIA_OK = 0, DIA_ERR_INVALID_ARG = -1, DIA_ERR_CUDA = -2, DIA_ERR_ALLOC = -3,
+       DIA_ERR_UNSUPPORTED = -4 };
+enum { DIA_LOSS_GAUSSIAN = 0 /* Eq. 8 */, DIA_LOSS_HUBER = 1 /* Eq. 12-13 */ };
+enum { DIA_NOISE_MODEL = 0 /* Eq. 6: sigma depends on theta */,
+       DIA_NOISE_FIXED = 1 /* caller variance map */ };
+enum { DIA_FIT_CONVERGED_GRAD = 0, DIA_FIT_CONVERGED_CHANGE = 1, DIA_FIT_MAX_ITERS = 2,
+       DIA_FIT_NONFINITE = 3 };
+
+#define DIA_MAX_KERNEL_SIZE 31            /* m odd, 1 <= m <= 31 in this build */
+
+typedef struct {
+  int n_rows, n_cols, m;          /* m odd, 1 <= m <= min(n_rows, n_cols, DIA_MAX_KERNEL_SIZE) */
+  int max_epochs;                 /* batch capacity of the handle, >= 1 */
+  int loss;    float huber_c;     /* c > 0; 1.345 is the paper's default */
+  int noise;   float sigma0, gain;/* Eq. 6: read noise [ADU] >= 0, gain [e-/ADU] > 0 */
+  const float* d_flat;            /* master flat F [n_rows][n_cols] or NULL => F == 1; borrowed for handle life */
+  void* stream;                   /* cudaStream_t; NULL = legacy default stream */
+} dia_config;
+
+typedef struct {                  /* PAPER.md:242-244 unless marked [reading] */
+  float  lr_kernel;               /* Adam learning rate of the kernel pixels, 1e-3 */
+  float  lr_b0;                   /* Adam learning rate of B0: 1, 10 or 100 */
+  double adam_beta1, adam_beta2, adam_eps;   /* [reading R5] 0.9, 0.999, 1e-8 */
+  double tol_switch;              /* Adam -> L-BFGS when |dL| < tol_switch |L|, 1e-6 */
+  double lbfgs_lr;                /* 1.0 */
+  int    lbfgs_history;           /* [reading R7] 100; 1 <= history <= 128 */
+  int    lbfgs_backtrack;         /* [reading R7] 1 = Armijo back-off (<= 20 halvings) */
+  double tol_change_rel;          /* stop when |dL| <= tol_change_rel |L|, 1e-8 [R8] */
+  double tol_grad_abs;            /* stop when max|g| < tol_grad_abs, 1e-7 */
+  double tol_grad_rel;            /* [reading] stop when max|g| < tol_grad_rel * max|g at switch|; 0 = off */
+  int    max_adam_iters, max_lbfgs_iters;    /* [reading] 20000, 500 */
+  int    force_adam_iters, force_lbfgs_iters;/* [reading] -1 = off; >= 0 replaces the data-dependent
+                                                exits by fixed counts (lock-step parity mode) */
+} dia_fit_opts;
+
+typedef struct {
+  double loss, grad_inf_norm, photometric_scale;   /* final L, max|g|, P = sum K (Eq. 3) */
+  int n_adam, n_lbfgs, n_evals, status;            /* status: DIA_FIT_* */
+} dia_fit_result;
+
+/* Fills `opts` (HOST) with the defaults listed above. */
+void dia_default_fit_opts(dia_fit_opts* opts);
+
+/* Creates a handle for one reference image d_R [n_rows][n_cols] (DEVICE, borrowed for the
+ * handle's life, must stay unchanged).  Allocates the workspace for cfg->max_epochs epochs.
+ * May synchronise.  Errors: INVALID_ARG (bad sizes/enums/NULLs), UNSUPPORTED (m too large),
+ * CUDA, ALLOC. */
+int dia_create(const dia_config* cfg, const float* d_R, dia_handle** out);
+
+/* Loss and gradient of the objective (Eq. 8 or Eq. 13 without theta-independent constants,
+ * with the noise model of Eq. 6 or a fixed variance map) for n_epochs targets, each at its own
+ * theta:   M = R (x) K + B0 (Eq. 2);  r = I - M;  v = sigma0^2/F^2 + max(M,0)/(G F);
+ *          L = sum_V rho(r/sqrt v) + 1/2 ln v;   dL/dK[a][b] = sum_V w_ij R[i-h+a][j-h+b],
+ *          dL/dB0 = sum_V w_ij,  w = dL/dM.
+ * 1 <= n_epochs <= max_epochs.  Asynchronous on the handle's stream. */
+int dia_eval_loss_grad(dia_handle* h, int n_epochs,
+                       const float* d_I,            /* [n_epochs][n_rows][n_cols] */
+                       const unsigned char* d_mask, /* same shape, 1 = use; or NULL */
+                       const float* d_var,          /* variance map, same shape; required iff DIA_NOISE_FIXED, else NULL */
+                       const float* d_theta,        /* [n_epochs][m*m+1] */
+                       double* d_loss,              /* out [n_epochs] */
+                       double* d_grad);             /* out [n_epochs][m*m+1] */
+
+/* Full fit: Adam (Eq. 9) until the relative loss change drops below
+ * tol_switch, then L-BFGS (Eq. 10) until convergence, all on the device; the host enqueues one
+ * graph launch and never reads a per-iteration value.  d_theta holds the initial theta on entry
+ * and the fitted theta on exit.  d_result [n_epochs] is DEVICE memory. */
+int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs,
+            const float* d_I, const unsigned char* d_mask, const float* d_var,
+            float* d_theta, dia_fit_result* d_result);
+
+/* Frees the handle's workspace (synchronises the handle's stream first). */
+int dia_destroy(dia_handle* h);
+
+const char* dia_status_string(int code);
+/* Last error text recorded on this handle (or on the creating thread when h == NULL). */
+const char* dia_last_error(const dia_handle* h);
+
+/* Introspection used by bench.py / tests: number of kernels the last eval or fit call
+ * enqueued per iteration, and the persistent grid size. */
+int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_per_block,
+                 int* smem_bytes, int* launches_per_eval);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

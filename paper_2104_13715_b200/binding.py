@@ -1,0 +1,207 @@
+"""ctypes binding of libdia_b200.so -- argument marshalling only.
+
+The functions mirror include/dia.h one to one (dia_create, dia_eval_loss_grad, dia_fit,
+dia_destroy); `Handle` is a small convenience wrapper that allocates the outputs as torch
+CUDA tensors.  PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+from . import build as _build
+
+LOSS_GAUSSIAN, LOSS_HUBER = 0, 1
+NOISE_MODEL, NOISE_FIXED = 0, 1
+FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
+EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
+                    "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info")
+
+
+class DiaError(RuntimeError):
+    pass
+
+
+class _Config(C.Structure):
+    _fields_ = [("n_rows", C.c_int), ("n_cols", C.c_int), ("m", C.c_int), ("max_epochs", C.c_int),
+                ("loss", C.c_int), ("huber_c", C.c_float),
+                ("noise", C.c_int), ("sigma0", C.c_float), ("gain", C.c_float),
+                ("d_flat", C.c_void_p), ("stream", C.c_void_p)]
+
+
+class FitOpts(C.Structure):
+    _fields_ = [("lr_kernel", C.c_float), ("lr_b0", C.c_float),
+                ("adam_beta1", C.c_double), ("adam_beta2", C.c_double), ("adam_eps", C.c_double),
+                ("tol_switch", C.c_double), ("lbfgs_lr", C.c_double),
+                ("lbfgs_history", C.c_int), ("lbfgs_backtrack", C.c_int),
+                ("tol_change_rel", C.c_double), ("tol_grad_abs", C.c_double), ("tol_grad_rel", C.c_double),
+                ("max_adam_iters", C.c_int), ("max_lbfgs_iters", C.c_int),
+                ("force_adam_iters", C.c_int), ("force_lbfgs_iters", C.c_int)]
+
+    @staticmethod
+    def default(**kw) -> "FitOpts":
+        o = FitOpts()
+        load_library().dia_default_fit_opts(C.byref(o))
+        for k, v in kw.items():
+            if not hasattr(o, k):
+                raise AttributeError(k)
+            setattr(o, k, v)
+        return o
+
+
+class FitResult(C.Structure):
+    _fields_ = [("loss", C.c_double), ("grad_inf_norm", C.c_double), ("photometric_scale", C.c_double),
+                ("n_adam", C.c_int), ("n_lbfgs", C.c_int), ("n_evals", C.c_int), ("status", C.c_int)]
+
+
+_LIB = None
+
+
+def load_library(build_if_missing: bool = True):
+    """Loads libdia_b200.so (building it with nvcc if it is missing or stale).  Raises if it
+    cannot be loaded: there is no fallback implementation."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = _build.LIB
+    if build_if_missing and os.environ.get("DIA_NO_BUILD") != "1":
+        try:
+            path = _build.build()
+        except Exception as exc:  # stale-but-present library is still usable
+            if not os.path.exists(path):
+                raise DiaError(f"cannot build {path}: {exc}") from exc
+    if not os.path.exists(path):
+        raise DiaError(f"{path} is missing; run python -m paper_2104_13715_b200.build")
+    lib = C.CDLL(path)
+    lib.dia_status_string.restype = C.c_char_p
+    lib.dia_status_string.argtypes = [C.c_int]
+    lib.dia_last_error.restype = C.c_char_p
+    lib.dia_last_error.argtypes = [C.c_void_p]
+    lib.dia_create.argtypes = [C.POINTER(_Config), C.c_void_p, C.POINTER(C.c_void_p)]
+    lib.dia_eval_loss_grad.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.dia_fit.argtypes = [C.c_void_p, C.POINTER(FitOpts), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                            C.c_void_p, C.c_void_p]
+    lib.dia_destroy.argtypes = [C.c_void_p]
+    lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
+    _LIB = lib
+    return lib
+
+
+def _dptr(t: Optional[torch.Tensor], dtype, what: str):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise DiaError(f"{what} must be a contiguous CUDA tensor of dtype {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _check(rc: int, handle=None):
+    if rc != 0:
+        lib = load_library()
+        msg = lib.dia_last_error(handle).decode()
+        raise DiaError(f"{lib.dia_status_string(rc).decode()} ({rc}): {msg}")
+
+
+# ------------------------------------------------------------------------------------------
+# one-to-one C ABI
+# ------------------------------------------------------------------------------------------
+def dia_create(n_rows: int, n_cols: int, m: int, d_R: torch.Tensor, *, max_epochs: int = 1,
+               loss: int = LOSS_GAUSSIAN, huber_c: float = 1.345, noise: int = NOISE_MODEL,
+               sigma0: float = 0.0, gain: float = 1.0, d_flat: Optional[torch.Tensor] = None,
+               stream: Optional[torch.cuda.Stream] = None) -> int:
+    lib = load_library()
+    cfg = _Config(n_rows, n_cols, m, max_epochs, loss, huber_c, noise, sigma0, gain,
+                  None if d_flat is None else _dptr(d_flat, torch.float32, "d_flat").value,
+                  None if stream is None else stream.cuda_stream)
+    if d_R is not None and tuple(d_R.shape) != (n_rows, n_cols):
+        raise DiaError("d_R has the wrong shape")
+    out = C.c_void_p()
+    _check(lib.dia_create(C.byref(cfg), _dptr(d_R, torch.float32, "d_R"), C.byref(out)))
+    return out.value
+
+
+def dia_eval_loss_grad(handle: int, n_epochs: int, d_I, d_mask, d_var, d_theta, d_loss, d_grad) -> None:
+    lib = load_library()
+    _check(lib.dia_eval_loss_grad(handle, n_epochs, _dptr(d_I, torch.float32, "d_I"),
+                                  _dptr(d_mask, torch.uint8, "d_mask"), _dptr(d_var, torch.float32, "d_var"),
+                                  _dptr(d_theta, torch.float32, "d_theta"),
+                                  _dptr(d_loss, torch.float64, "d_loss"), _dptr(d_grad, torch.float64, "d_grad")),
+           handle)
+
+
+def dia_fit(handle: int, opts: FitOpts, n_epochs: int, d_I, d_mask, d_var, d_theta, d_result) -> None:
+    lib = load_library()
+    _check(lib.dia_fit(handle, C.byref(opts), n_epochs, _dptr(d_I, torch.float32, "d_I"),
+                       _dptr(d_mask, torch.uint8, "d_mask"), _dptr(d_var, torch.float32, "d_var"),
+                       _dptr(d_theta, torch.float32, "d_theta"), _dptr(d_result, torch.uint8, "d_result")),
+           handle)
+
+
+def dia_destroy(handle: int) -> None:
+    _check(load_library().dia_destroy(handle))
+
+
+# ------------------------------------------------------------------------------------------
+# convenience wrapper
+# ------------------------------------------------------------------------------------------
+class Handle:
+    """Owns one dia_handle and keeps the borrowed tensors (R, flat) alive."""
+
+    def __init__(self, R: torch.Tensor, m: int, *, max_epochs: int = 1, loss: int = LOSS_GAUSSIAN,
+                 huber_c: float = 1.345, noise: int = NOISE_MODEL, sigma0: float = 0.0, gain: float = 1.0,
+                 flat: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None):
+        self.R, self.flat, self.m, self.max_epochs = R, flat, m, max_epochs
+        self.n_rows, self.n_cols = R.shape
+        self.np = m * m + 1
+        self.stream = stream
+        self._h = dia_create(self.n_rows, self.n_cols, m, R, max_epochs=max_epochs, loss=loss,
+                             huber_c=huber_c, noise=noise, sigma0=sigma0, gain=gain, d_flat=flat,
+                             stream=stream)
+
+    @property
+    def raw(self) -> int:
+        return self._h
+
+    def info(self) -> dict:
+        v = [C.c_int() for _ in range(4)]
+        _check(load_library().dia_get_info(self._h, *[C.byref(x) for x in v]), self._h)
+        return dict(grid_blocks=v[0].value, threads_per_block=v[1].value, smem_bytes=v[2].value,
+                    launches_per_eval=v[3].value)
+
+    def _epochs(self, I):
+        return 1 if I.dim() == 2 else I.shape[0]
+
+    def eval_loss_grad(self, I, theta, mask=None, var=None, loss=None, grad=None):
+        E = self._epochs(I)
+        dev = I.device
+        loss = torch.empty(E, dtype=torch.float64, device=dev) if loss is None else loss
+        grad = torch.empty((E, self.np), dtype=torch.float64, device=dev) if grad is None else grad
+        dia_eval_loss_grad(self._h, E, I, mask, var, theta, loss, grad)
+        return loss, grad
+
+    def fit(self, I, theta0, opts: Optional[FitOpts] = None, mask=None, var=None):
+        """Returns (theta_hat float32 [E][np] CUDA tensor, list[FitResult]); synchronises to read results."""
+        E = self._epochs(I)
+        theta = theta0.clone().reshape(E, self.np).contiguous()
+        res = torch.zeros(E * C.sizeof(FitResult), dtype=torch.uint8, device=I.device)
+        opts = opts or FitOpts.default()
+        dia_fit(self._h, opts, E, I, mask, var, theta, res)
+        host = res.cpu().numpy().tobytes()          # synchronises
+        out = [FitResult.from_buffer_copy(host[i * C.sizeof(FitResult):(i + 1) * C.sizeof(FitResult)])
+               for i in range(E)]
+        return theta, out
+
+    def close(self):
+        if self._h:
+            dia_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

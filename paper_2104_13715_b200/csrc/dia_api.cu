@@ -1,0 +1,203 @@
+// dia_api.cu -- host side of the C ABI declared in include/dia.h.
+#include "../../include/dia.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "dia_eval.cuh"
+#include "dia_fit.cuh"
+
+struct dia_handle {
+  dia_config cfg;
+  const float* d_R;
+  cudaStream_t stream;
+  int grid, np, sms;
+  size_t smem;
+  double* d_partials;      // [max_epochs][grid][np+1]
+  dia::FitWorkspace fit;   // device optimiser state + cached graph
+  std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(dia_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_create_err = msg;
+  return code;
+}
+static int cuda_fail(dia_handle* h, cudaError_t e, const char* what) {
+  return fail(h, DIA_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+extern "C" const char* dia_status_string(int code) {
+  switch (code) {
+    case DIA_OK: return "ok";
+    case DIA_ERR_INVALID_ARG: return "invalid argument";
+    case DIA_ERR_CUDA: return "CUDA error";
+    case DIA_ERR_ALLOC: return "allocation failed";
+    case DIA_ERR_UNSUPPORTED: return "unsupported configuration";
+    default: return "unknown status";
+  }
+}
+extern "C" const char* dia_last_error(const dia_handle* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+extern "C" void dia_default_fit_opts(dia_fit_opts* o) {
+  if (!o) return;
+  o->lr_kernel = 1e-3f;  o->lr_b0 = 10.0f;
+  o->adam_beta1 = 0.9;  o->adam_beta2 = 0.999;  o->adam_eps = 1e-8;
+  o->tol_switch = 1e-6;  o->lbfgs_lr = 1.0;
+  o->lbfgs_history = 100;  o->lbfgs_backtrack = 1;
+  o->tol_change_rel = 1e-8;  o->tol_grad_abs = 1e-7;  o->tol_grad_rel = 0.0;
+  o->max_adam_iters = 20000;  o->max_lbfgs_iters = 500;
+  o->force_adam_iters = -1;  o->force_lbfgs_iters = -1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernel-size dispatch: one instantiation per odd m
+// ---------------------------------------------------------------------------------------------
+#define DIA_FOR_EACH_M(X) X(1) X(3) X(5) X(7) X(9) X(11) X(13) X(15) X(17) X(19) X(21) X(23) X(25) X(27) X(29) X(31)
+
+static size_t smem_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::Geo<MM>::SMEM;
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return 0;
+}
+static const void* kernel_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return (const void*)dia::eval_kernel<MM>;
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return nullptr;
+}
+
+namespace dia {
+const void* eval_kernel_ptr(const dia_handle* h) { return kernel_for(h->cfg.m); }
+size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
+cudaError_t launch_eval(const dia_handle* h, const EvalParams& p) {
+  void* args[] = {(void*)&p};
+  return cudaLaunchKernel(kernel_for(h->cfg.m), dim3(h->grid), dim3(kThreads), args, h->smem, h->stream);
+}
+}  // namespace dia
+
+static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
+                        const float* d_var, const float* d_theta, const int* d_done, dia::EvalParams* p) {
+  const dia_config& c = h->cfg;
+  p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
+  p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
+  p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;
+  p->tiles_x = (c.n_cols - c.m + 1 + dia::kTW - 1) / dia::kTW;
+  p->tiles_y = (c.n_rows - c.m + 1 + dia::kTH - 1) / dia::kTH;
+  p->loss_kind = c.loss;  p->noise_kind = c.noise;
+  p->huber_c = c.huber_c;  p->sigma0_sq = c.sigma0 * c.sigma0;
+  p->inv_gain = c.noise == DIA_NOISE_MODEL ? 1.0f / c.gain : 0.f;
+  p->r_vec4 = (c.n_cols % 4 == 0) && ((reinterpret_cast<uintptr_t>(h->d_R) & 15) == 0);
+}
+
+extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** out) {
+  if (!cfg || !d_R || !out) return fail(nullptr, DIA_ERR_INVALID_ARG, "null argument");
+  *out = nullptr;
+  if (cfg->m < 1 || cfg->m % 2 == 0) return fail(nullptr, DIA_ERR_INVALID_ARG, "m must be odd and >= 1");
+  if (cfg->n_rows < cfg->m || cfg->n_cols < cfg->m) return fail(nullptr, DIA_ERR_INVALID_ARG, "image smaller than kernel");
+  if (cfg->max_epochs < 1) return fail(nullptr, DIA_ERR_INVALID_ARG, "max_epochs must be >= 1");
+  if (cfg->loss != DIA_LOSS_GAUSSIAN && cfg->loss != DIA_LOSS_HUBER) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad loss");
+  if (cfg->noise != DIA_NOISE_MODEL && cfg->noise != DIA_NOISE_FIXED) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad noise mode");
+  if (cfg->loss == DIA_LOSS_HUBER && !(cfg->huber_c > 0.f)) return fail(nullptr, DIA_ERR_INVALID_ARG, "huber_c must be > 0");
+  if (cfg->noise == DIA_NOISE_MODEL && !(cfg->gain > 0.f && cfg->sigma0 >= 0.f))
+    return fail(nullptr, DIA_ERR_INVALID_ARG, "need gain > 0 and sigma0 >= 0");
+  if (cfg->m > DIA_MAX_KERNEL_SIZE) return fail(nullptr, DIA_ERR_UNSUPPORTED, "m exceeds DIA_MAX_KERNEL_SIZE");
+
+  int dev = 0, sms = 0;
+  cudaError_t ce = cudaGetDevice(&dev);
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDevice (no CUDA device: there is no CPU fallback)");
+  ce = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaDeviceGetAttribute");
+
+  dia_handle* h = new (std::nothrow) dia_handle();
+  if (!h) return fail(nullptr, DIA_ERR_ALLOC, "host allocation failed");
+  h->cfg = *cfg;  h->d_R = d_R;  h->stream = (cudaStream_t)cfg->stream;  h->sms = sms;
+  h->np = cfg->m * cfg->m + 1;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
+
+  const void* k = kernel_for(cfg->m);
+  ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
+  if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
+  int occ = 0;
+  ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, dia::kThreads, h->smem);
+  if (ce != cudaSuccess || occ < 1) { int rc = cuda_fail(nullptr, ce, "occupancy query"); delete h; return rc; }
+  const int tiles = ((cfg->n_cols - cfg->m + 1 + dia::kTW - 1) / dia::kTW) * ((cfg->n_rows - cfg->m + 1 + dia::kTH - 1) / dia::kTH);
+  h->grid = sms * occ;                       // persistent grid: every CTA resident
+  if (h->grid > tiles) h->grid = tiles;
+  ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * h->grid * (h->np + 1));
+  if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
+  int rc = dia::fit_workspace_create(&h->fit, cfg->max_epochs, h->np);
+  if (rc != DIA_OK) { cudaFree(h->d_partials); fail(nullptr, rc, "fit workspace allocation failed"); delete h; return rc; }
+  *out = h;
+  return DIA_OK;
+}
+
+extern "C" int dia_destroy(dia_handle* h) {
+  if (!h) return DIA_ERR_INVALID_ARG;
+  cudaStreamSynchronize(h->stream);
+  dia::fit_workspace_destroy(&h->fit);
+  cudaFree(h->d_partials);
+  delete h;
+  return DIA_OK;
+}
+
+static int check_eval_args(dia_handle* h, int n_epochs, const void* d_I, const void* d_var, const void* d_theta) {
+  if (!h) return DIA_ERR_INVALID_ARG;
+  if (n_epochs < 1 || n_epochs > h->cfg.max_epochs) return fail(h, DIA_ERR_INVALID_ARG, "n_epochs out of range");
+  if (!d_I || !d_theta) return fail(h, DIA_ERR_INVALID_ARG, "null image or theta");
+  if (h->cfg.noise == DIA_NOISE_FIXED && !d_var) return fail(h, DIA_ERR_INVALID_ARG, "DIA_NOISE_FIXED needs d_var");
+  if (h->cfg.noise == DIA_NOISE_MODEL && d_var) return fail(h, DIA_ERR_INVALID_ARG, "d_var must be NULL in DIA_NOISE_MODEL");
+  return DIA_OK;
+}
+
+extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
+                                  const float* d_var, const float* d_theta, double* d_loss, double* d_grad) {
+  int rc = check_eval_args(h, n_epochs, d_I, d_var, d_theta);
+  if (rc != DIA_OK) return rc;
+  if (!d_loss || !d_grad) return fail(h, DIA_ERR_INVALID_ARG, "null output");
+  dia::EvalParams p;
+  fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p);
+  cudaError_t ce = dia::launch_eval(h, p);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "eval launch");
+  const int np1 = h->np + 1;
+  dia::reduce_partials_kernel<<<dim3((np1 + 127) / 128, n_epochs), 128, 0, h->stream>>>(
+      h->d_partials, h->grid, np1, nullptr, d_loss, d_grad);
+  ce = cudaGetLastError();
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
+  return DIA_OK;
+}
+
+extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, const float* d_I,
+                       const unsigned char* d_mask, const float* d_var, float* d_theta,
+                       dia_fit_result* d_result) {
+  int rc = check_eval_args(h, n_epochs, d_I, d_var, d_theta);
+  if (rc != DIA_OK) return rc;
+  if (!opts || !d_result) return fail(h, DIA_ERR_INVALID_ARG, "null opts or result");
+  if (opts->lbfgs_history < 1 || opts->lbfgs_history > dia::kMaxHistory)
+    return fail(h, DIA_ERR_INVALID_ARG, "lbfgs_history out of range");
+  dia::EvalParams p;
+  fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p);
+  std::string err;
+  rc = dia::fit_run(&h->fit, h, p, *opts, n_epochs, d_theta, d_result, h->grid, h->stream, &err);
+  if (rc != DIA_OK) return fail(h, rc, err);
+  return DIA_OK;
+}
+
+extern "C" int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_per_block, int* smem_bytes,
+                            int* launches_per_eval) {
+  if (!h) return DIA_ERR_INVALID_ARG;
+  if (grid_blocks) *grid_blocks = h->grid;
+  if (threads_per_block) *threads_per_block = dia::kThreads;
+  if (smem_bytes) *smem_bytes = (int)h->smem;
+  if (launches_per_eval) *launches_per_eval = 2;
+  return DIA_OK;
+}

@@ -1,0 +1,429 @@
+// dia_fit.cuh -- on-device optimiser: Adam (Eq. 9) then L-BFGS (PAPER.md:132-135,
+// Eq. 10; two-loop recursion), with the switch / stop rules of PAPER.md:244, 248-255 under the
+// readings R5-R9 of DESIGN.md.  One CTA per epoch runs a small state machine after every
+// evaluation; the loop itself is a CUDA-graph WHILE node whose condition is cleared by the last
+// epoch to finish, so the host enqueues one graph launch per fit and never reads a per-iteration value.
+// All optimiser state is FP64; theta is rounded to float32 only where it enters the stencil (R9).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstring>
+#include <string>
+
+#include "../../include/dia.h"
+#include "dia_eval.cuh"
+
+struct dia_handle;
+
+namespace dia {
+
+constexpr int kMaxHistory = 128;
+constexpr int kFitThreads = 256;
+constexpr int kMaxPerThread = 4;      // ceil((31*31+1) / 256)
+
+cudaError_t launch_eval(const dia_handle* h, const EvalParams& p);
+const void* eval_kernel_ptr(const dia_handle* h);
+size_t eval_smem_bytes(const dia_handle* h);
+
+enum { PH_ADAM = 0, PH_LBFGS = 1, PH_DONE = 2 };
+
+struct FitState {
+  int phase, t, n_adam, n_lbfgs, n_evals, status;
+  int k, n_pairs, head, nbt;
+  double L, Lprev, b1t, b2t, g_switch, alpha, gtd;
+};
+
+struct FitBuffers {
+  double* theta64;   // [E][np]
+  double* g;         // [E][np]  gradient at the current iterate (L-BFGS)
+  double* m1;        // [E][np]
+  double* m2;        // [E][np]
+  double* d;         // [E][np]  search direction
+  double* S;         // [E][hist_cap][np]
+  double* Y;         // [E][hist_cap][np]
+  double* rho;       // [E][hist_cap]
+  double* yy;        // [E][hist_cap]
+  FitState* st;      // [E]
+  float* theta32;    // [E][np]  evaluation point
+  int* done;         // [E]
+  int* remaining;    // [1]
+};
+
+struct FitWorkspace {
+  FitBuffers b;
+  float* d_theta32;  // alias of b.theta32 (what the eval kernel reads)
+  int* d_done;
+  int max_epochs, np, hist_cap;
+  cudaGraph_t graph;
+  cudaGraphExec_t exec;
+  unsigned char key[256];
+  int key_len;
+};
+
+struct StepArgs {
+  FitBuffers b;
+  const double* partials;
+  int n_blocks, np, hist_cap;
+  dia_fit_opts o;
+  float* theta_out;          // caller's theta [E][np]
+  dia_fit_result* result;    // caller's results [E]
+  cudaGraphConditionalHandle cond;
+};
+
+// ---------------------------------------------------------------- block-wide FP64 reductions
+__device__ __forceinline__ double block_sum(double v, double* sh) {
+  v = warp_sum_f64(v);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll
+  for (int w = 0; w < kFitThreads / 32; ++w) s += sh[w];
+  return s;
+}
+__device__ __forceinline__ double block_max(double v, double* sh) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { double u = __shfl_xor_sync(0xffffffffu, v, o); v = (u > v || u != u) ? u : v; }
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll
+  for (int w = 0; w < kFitThreads / 32; ++w) { double u = sh[w]; s = (u > s || u != u) ? u : s; }
+  return s;
+}
+
+__global__ void fit_init_kernel(FitBuffers b, const float* __restrict__ theta_in, int np, int n_epochs) {
+  const int e = blockIdx.x;
+  for (int k = threadIdx.x; k < np; k += blockDim.x) {
+    const float v = theta_in[(size_t)e * np + k];
+    b.theta64[(size_t)e * np + k] = (double)v;
+    b.theta32[(size_t)e * np + k] = v;
+    b.m1[(size_t)e * np + k] = 0.0;
+    b.m2[(size_t)e * np + k] = 0.0;
+  }
+  if (threadIdx.x == 0) {
+    FitState s;
+    s.phase = PH_ADAM; s.t = 0; s.n_adam = 0; s.n_lbfgs = 0; s.n_evals = 0; s.status = DIA_FIT_MAX_ITERS;
+    s.k = 0; s.n_pairs = 0; s.head = 0; s.nbt = 0;
+    s.L = 0.0; s.Lprev = 0.0; s.b1t = 1.0; s.b2t = 1.0; s.g_switch = 0.0; s.alpha = 0.0; s.gtd = 0.0;
+    b.st[e] = s;
+    b.done[e] = 0;
+    if (e == 0) *b.remaining = n_epochs;
+  }
+}
+
+// One optimiser transition for epoch blockIdx.x, run after every evaluation.
+__global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a) {
+  const int e = blockIdx.x;
+  if (a.b.done[e]) return;
+  __shared__ double sh[kFitThreads / 32];
+  __shared__ double s_alpha[kMaxHistory];
+  const int np = a.np, nk = np - 1, tid = threadIdx.x;
+  const dia_fit_opts& o = a.o;
+  FitState st = a.b.st[e];                       // every thread holds a private copy; thread 0 writes back
+
+  double* theta = a.b.theta64 + (size_t)e * np;
+  double* gcur = a.b.g + (size_t)e * np;
+  double* dvec = a.b.d + (size_t)e * np;
+  double* Sm = a.b.S + (size_t)e * a.hist_cap * np;
+  double* Ym = a.b.Y + (size_t)e * a.hist_cap * np;
+  double* rho = a.b.rho + (size_t)e * a.hist_cap;
+  double* yy = a.b.yy + (size_t)e * a.hist_cap;
+  float* th32 = a.b.theta32 + (size_t)e * np;
+  const int hist = o.lbfgs_history;
+
+  // ---- second-level reduction of the evaluation's block partials, fixed order
+  double gn[kMaxPerThread];
+  double Ln = 0.0;
+  {
+    const double* src = a.partials + (size_t)e * a.n_blocks * (np + 1);
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+      const int k = tid + q * kFitThreads;
+      double s = 0.0;
+      if (k < np + 1)
+        for (int blk = 0; blk < a.n_blocks; ++blk) s += src[(size_t)blk * (np + 1) + k];
+      gn[q] = (k < np) ? s : 0.0;
+      if (k == np) sh[0] = s;                    // loss lives in slot np
+    }
+    __syncthreads();
+    Ln = sh[0];
+    __syncthreads();
+  }
+  st.n_evals += 1;
+  bool finished = false;
+  bool at_top = false;                           // enter the L-BFGS loop head with (st.L, gcur) current
+
+  if (st.phase == PH_ADAM) {
+    const int t = st.t + 1;
+    if (!isfinite(Ln)) {
+      st.status = DIA_FIT_NONFINITE; st.L = Ln; finished = true;
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) gcur[k] = gn[q]; }
+    } else {
+      bool sw;
+      if (o.force_adam_iters >= 0) sw = t > o.force_adam_iters;
+      else sw = (t >= 2 && fabs(Ln - st.Lprev) < o.tol_switch * fabs(st.Lprev)) || (t > o.max_adam_iters);
+      if (!sw) {
+        st.b1t *= o.adam_beta1; st.b2t *= o.adam_beta2;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) {
+          const int k = tid + q * kFitThreads;
+          if (k < np) {
+            double* m1 = a.b.m1 + (size_t)e * np; double* m2 = a.b.m2 + (size_t)e * np;
+            const double g = gn[q];
+            const double v1 = o.adam_beta1 * m1[k] + (1.0 - o.adam_beta1) * g;
+            const double v2 = o.adam_beta2 * m2[k] + (1.0 - o.adam_beta2) * g * g;
+            m1[k] = v1; m2[k] = v2;
+            const double mh = v1 / (1.0 - st.b1t), vh = v2 / (1.0 - st.b2t);
+            const double lr = (k < nk) ? (double)o.lr_kernel : (double)o.lr_b0;
+            const double th = theta[k] - lr * mh / (sqrt(vh) + o.adam_eps);
+            theta[k] = th;
+            th32[k] = (float)th;
+          }
+        }
+        st.n_adam += 1; st.Lprev = Ln; st.t = t; st.L = Ln;
+      } else {
+        // switch: L-BFGS starts from this iterate and reuses this evaluation (R6)
+        double gi = 0.0;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) {
+          const int k = tid + q * kFitThreads;
+          if (k < np) { gcur[k] = gn[q]; const double ag = fabs(gn[q]); gi = (ag > gi || ag != ag) ? ag : gi; }
+        }
+        st.g_switch = block_max(gi, sh);
+        st.L = Ln; st.phase = PH_LBFGS; st.k = 1; st.n_pairs = 0; st.head = 0; st.t = t;
+        at_top = true;
+      }
+    }
+  } else {  // PH_LBFGS: (Ln, gn) is the trial point theta + alpha d
+    const bool bad = !isfinite(Ln);
+    if (o.lbfgs_backtrack && (bad || Ln > st.L + 1e-4 * st.alpha * st.gtd) && st.nbt < 20) {
+      st.alpha *= 0.5; st.nbt += 1;
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) {
+        const int k = tid + q * kFitThreads;
+        if (k < np) th32[k] = (float)(theta[k] + st.alpha * dvec[k]);
+      }
+    } else if (bad) {
+      st.status = DIA_FIT_NONFINITE; finished = true;
+    } else {
+      double sty = 0.0, yty = 0.0;
+      double sv[kMaxPerThread], yv[kMaxPerThread];
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) {
+        const int k = tid + q * kFitThreads;
+        sv[q] = 0.0; yv[q] = 0.0;
+        if (k < np) { sv[q] = st.alpha * dvec[k]; yv[q] = gn[q] - gcur[k]; sty += sv[q] * yv[q]; yty += yv[q] * yv[q]; }
+      }
+      sty = block_sum(sty, sh);
+      yty = block_sum(yty, sh);
+      if (sty > 1e-10) {                                 // R7 curvature guard, FIFO eviction
+        int id;
+        if (st.n_pairs < hist) { id = (st.head + st.n_pairs) % hist; st.n_pairs += 1; }
+        else { id = st.head; st.head = (st.head + 1) % hist; }
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) {
+          const int k = tid + q * kFitThreads;
+          if (k < np) { Sm[(size_t)id * np + k] = sv[q]; Ym[(size_t)id * np + k] = yv[q]; }
+        }
+        if (tid == 0) { rho[id] = 1.0 / sty; yy[id] = yty; }
+      }
+      const double dL = fabs(Ln - st.L);
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) {
+        const int k = tid + q * kFitThreads;
+        if (k < np) { theta[k] += sv[q]; gcur[k] = gn[q]; }
+      }
+      st.L = Ln; st.n_lbfgs += 1;
+      if (o.force_lbfgs_iters < 0) {
+        if (dL <= o.tol_change_rel * fabs(st.L)) { st.status = DIA_FIT_CONVERGED_CHANGE; finished = true; }   // R8
+        else if (st.k >= o.max_lbfgs_iters) { st.status = DIA_FIT_MAX_ITERS; finished = true; }
+      }
+      if (!finished) { st.k += 1; at_top = true; }
+      __syncthreads();                                   // rho / yy / S / Y visible to the block
+    }
+  }
+
+  if (at_top && !finished) {
+    // ---- L-BFGS loop head: stop test, two-loop recursion, first trial point
+    double q4[kMaxPerThread];
+    double gi = 0.0, g1 = 0.0;
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+      const int k = tid + q * kFitThreads;
+      q4[q] = (k < np) ? gcur[k] : 0.0;
+      const double ag = fabs(q4[q]);
+      gi = (ag > gi || ag != ag) ? ag : gi;
+      g1 += ag;
+    }
+    gi = block_max(gi, sh);
+    g1 = block_sum(g1, sh);
+    bool stop = false;
+    if (o.force_lbfgs_iters >= 0) { if (st.k > o.force_lbfgs_iters) { st.status = DIA_FIT_MAX_ITERS; stop = true; } }
+    else if (gi < o.tol_grad_abs || gi < o.tol_grad_rel * st.g_switch) { st.status = DIA_FIT_CONVERGED_GRAD; stop = true; }
+    if (stop) {
+      finished = true;
+    } else {
+      double gq[kMaxPerThread];
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) gq[q] = q4[q];
+      for (int i = st.n_pairs - 1; i >= 0; --i) {
+        const int id = (st.head + i) % hist;
+        double part = 0.0;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) part += Sm[(size_t)id * np + k] * q4[q]; }
+        const double al = rho[id] * block_sum(part, sh);
+        if (tid == 0) s_alpha[i] = al;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) q4[q] -= al * Ym[(size_t)id * np + k]; }
+      }
+      __syncthreads();
+      double gamma = 1.0;
+      if (st.n_pairs > 0) { const int id = (st.head + st.n_pairs - 1) % hist; gamma = (1.0 / rho[id]) / yy[id]; }
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) q4[q] *= gamma;
+      for (int i = 0; i < st.n_pairs; ++i) {
+        const int id = (st.head + i) % hist;
+        double part = 0.0;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) part += Ym[(size_t)id * np + k] * q4[q]; }
+        const double beta = rho[id] * block_sum(part, sh);
+        const double c = s_alpha[i] - beta;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) q4[q] += c * Sm[(size_t)id * np + k]; }
+      }
+      double part = 0.0;
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) { q4[q] = -q4[q]; part += gq[q] * q4[q]; }
+      double gtd = block_sum(part, sh);
+      if (!(gtd < 0.0)) {                                 // not a descent direction: drop the history
+        st.n_pairs = 0; st.head = 0;
+        part = 0.0;
+#pragma unroll
+        for (int q = 0; q < kMaxPerThread; ++q) { q4[q] = -gq[q]; part += gq[q] * q4[q]; }
+        gtd = block_sum(part, sh);
+      }
+      double alpha = o.lbfgs_lr;
+      if (st.n_pairs == 0) alpha *= (g1 > 1.0) ? 1.0 / g1 : 1.0;     // R7 first-step scaling
+      st.alpha = alpha; st.gtd = gtd; st.nbt = 0;
+#pragma unroll
+      for (int q = 0; q < kMaxPerThread; ++q) {
+        const int k = tid + q * kFitThreads;
+        if (k < np) { dvec[k] = q4[q]; th32[k] = (float)(theta[k] + alpha * q4[q]); }
+      }
+    }
+  }
+
+  if (finished) {
+    double gi = 0.0, P = 0.0;
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+      const int k = tid + q * kFitThreads;
+      if (k < np) {
+        const double ag = fabs(gcur[k]);
+        gi = (ag > gi || ag != ag) ? ag : gi;
+        if (k < nk) P += theta[k];
+        a.theta_out[(size_t)e * np + k] = (float)theta[k];
+      }
+    }
+    gi = block_max(gi, sh);
+    P = block_sum(P, sh);                                  // Eq. 3
+    st.phase = PH_DONE;
+    if (tid == 0) {
+      dia_fit_result r;
+      r.loss = st.L; r.grad_inf_norm = gi; r.photometric_scale = P;
+      r.n_adam = st.n_adam; r.n_lbfgs = st.n_lbfgs; r.n_evals = st.n_evals; r.status = st.status;
+      a.result[e] = r;
+      a.b.done[e] = 1;
+      __threadfence();
+      if (atomicSub(a.b.remaining, 1) == 1) cudaGraphSetConditional(a.cond, 0);
+    }
+  }
+  if (tid == 0) a.b.st[e] = st;
+}
+
+// ---------------------------------------------------------------- host side
+inline int fit_workspace_create(FitWorkspace* w, int max_epochs, int np) {
+  std::memset(w, 0, sizeof(*w));
+  w->max_epochs = max_epochs; w->np = np; w->hist_cap = kMaxHistory;
+  const size_t E = (size_t)max_epochs, n = E * np;
+  auto A = [&](void** p, size_t bytes) { return cudaMalloc(p, bytes) == cudaSuccess; };
+  bool ok = A((void**)&w->b.theta64, 8 * n) && A((void**)&w->b.g, 8 * n) && A((void**)&w->b.m1, 8 * n) &&
+            A((void**)&w->b.m2, 8 * n) && A((void**)&w->b.d, 8 * n) &&
+            A((void**)&w->b.S, 8 * n * kMaxHistory) && A((void**)&w->b.Y, 8 * n * kMaxHistory) &&
+            A((void**)&w->b.rho, 8 * E * kMaxHistory) && A((void**)&w->b.yy, 8 * E * kMaxHistory) &&
+            A((void**)&w->b.st, sizeof(FitState) * E) && A((void**)&w->b.theta32, 4 * n) &&
+            A((void**)&w->b.done, 4 * E) && A((void**)&w->b.remaining, 4);
+  if (!ok) { cudaGetLastError(); return DIA_ERR_ALLOC; }
+  w->d_theta32 = w->b.theta32; w->d_done = w->b.done;
+  return DIA_OK;
+}
+
+inline void fit_workspace_destroy(FitWorkspace* w) {
+  if (w->exec) cudaGraphExecDestroy(w->exec);
+  if (w->graph) cudaGraphDestroy(w->graph);
+  void* ptrs[] = {w->b.theta64, w->b.g, w->b.m1, w->b.m2, w->b.d, w->b.S, w->b.Y, w->b.rho, w->b.yy,
+                  w->b.st, w->b.theta32, w->b.done, w->b.remaining};
+  for (void* p : ptrs) cudaFree(p);
+  std::memset(w, 0, sizeof(*w));
+}
+
+#define DIA_CU(x) do { cudaError_t _e = (x); if (_e != cudaSuccess) { *err = std::string(#x) + ": " + cudaGetErrorString(_e); return DIA_ERR_CUDA; } } while (0)
+
+// Builds (or reuses) the fit graph  init -> WHILE { eval ; step }  and launches it once.
+inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, const dia_fit_opts& o,
+                   int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, cudaStream_t stream,
+                   std::string* err) {
+  unsigned char key[256];
+  int len = 0;
+  auto put = [&](const void* src, size_t n) { std::memcpy(key + len, src, n); len += (int)n; };
+  put(&n_epochs, sizeof(int)); put(&p.I, sizeof(void*)); put(&p.mask, sizeof(void*)); put(&p.var, sizeof(void*));
+  put(&d_theta, sizeof(void*)); put(&d_result, sizeof(void*)); put(&o, sizeof(o));
+  if (!(w->exec && len == w->key_len && std::memcmp(key, w->key, len) == 0)) {
+    if (w->exec) { cudaGraphExecDestroy(w->exec); w->exec = nullptr; }
+    if (w->graph) { cudaGraphDestroy(w->graph); w->graph = nullptr; }
+    DIA_CU(cudaGraphCreate(&w->graph, 0));
+    // node 1: init
+    const float* theta_in = d_theta;
+    int np = w->np, ne = n_epochs;
+    void* init_args[] = {(void*)&w->b, (void*)&theta_in, (void*)&np, (void*)&ne};
+    cudaKernelNodeParams kp = {};
+    kp.func = (void*)fit_init_kernel; kp.gridDim = dim3(n_epochs); kp.blockDim = dim3(256);
+    kp.sharedMemBytes = 0; kp.kernelParams = init_args; kp.extra = nullptr;
+    cudaGraphNode_t n_init;
+    DIA_CU(cudaGraphAddKernelNode(&n_init, w->graph, nullptr, 0, &kp));
+    // node 2: WHILE
+    cudaGraphConditionalHandle cond;
+    DIA_CU(cudaGraphConditionalHandleCreate(&cond, w->graph, 1, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = cond; cp.conditional.type = cudaGraphCondTypeWhile; cp.conditional.size = 1;
+    cudaGraphNode_t n_while;
+    DIA_CU(cudaGraphAddNode(&n_while, w->graph, &n_init, 1, &cp));
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    // body: eval -> step
+    EvalParams pe = p;
+    void* eval_args[] = {(void*)&pe};
+    cudaKernelNodeParams ke = {};
+    ke.func = (void*)eval_kernel_ptr(h); ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
+    ke.sharedMemBytes = (unsigned)eval_smem_bytes(h); ke.kernelParams = eval_args; ke.extra = nullptr;
+    cudaGraphNode_t n_eval, n_step;
+    DIA_CU(cudaGraphAddKernelNode(&n_eval, body, nullptr, 0, &ke));
+    StepArgs sa;
+    sa.b = w->b; sa.partials = p.partials; sa.n_blocks = grid; sa.np = w->np; sa.hist_cap = w->hist_cap;
+    sa.o = o; sa.theta_out = d_theta; sa.result = d_result; sa.cond = cond;
+    void* step_args[] = {(void*)&sa};
+    cudaKernelNodeParams ks = {};
+    ks.func = (void*)fit_step_kernel; ks.gridDim = dim3(n_epochs); ks.blockDim = dim3(kFitThreads);
+    ks.sharedMemBytes = 0; ks.kernelParams = step_args; ks.extra = nullptr;
+    DIA_CU(cudaGraphAddKernelNode(&n_step, body, &n_eval, 1, &ks));
+    DIA_CU(cudaGraphInstantiate(&w->exec, w->graph, 0));
+    std::memcpy(w->key, key, len); w->key_len = len;
+  }
+  DIA_CU(cudaGraphLaunch(w->exec, stream));
+  return DIA_OK;
+}
+
+}  // namespace dia
