@@ -1,0 +1,140 @@
+"""GPU-vs-oracle parity of dia_fit (on-device Adam -> L-BFGS), through the C ABI.
+
+Fit parity protocol: same theta_init and options on both sides;
+  |dP| <= 1e-4 |P|,  |dB0| <= 1e-4 max(|B0|, 1),  max|dK| <= 1e-4 max|K_or|.
+Lock-step mode (force_*_iters) pins the optimiser arithmetic step by step; the free-running
+fits additionally exercise the device-side switch / stop tests.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dia():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2104_13715_b200 as dia
+    dia.load_library()
+    return dia
+
+
+def _dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda().contiguous()
+
+
+OPT_KEYS = ("lr_kernel", "lr_b0", "adam_beta1", "adam_beta2", "adam_eps", "tol_switch", "lbfgs_lr",
+            "lbfgs_history", "lbfgs_backtrack", "tol_change_rel", "tol_grad_abs", "tol_grad_rel",
+            "max_adam_iters", "max_lbfgs_iters", "force_adam_iters", "force_lbfgs_iters")
+
+
+def _both_opts(dia, **kw):
+    og, oo = dia.FitOpts.default(**kw), oracle.RefFitOpts.default(**kw)
+    for k in OPT_KEYS:                       # the two libraries state the same defaults independently
+        assert float(getattr(og, k)) == pytest.approx(float(getattr(oo, k)), rel=1e-7), k
+    return og, oo
+
+
+def _fit_both(dia, w, og, oo, var=None, noise_fixed=False):
+    lossg = dia.LOSS_HUBER if w.loss == "huber" else dia.LOSS_GAUSSIAN
+    losso = oracle.LOSS_HUBER if w.loss == "huber" else oracle.LOSS_GAUSSIAN
+    cfg = oracle.RefConfig(w.n, w.n, w.m, loss=losso, sigma0=w.sigma0, gain=w.gain, flat=w.flat,
+                           noise=oracle.NOISE_FIXED if noise_fixed else oracle.NOISE_MODEL)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=w.n_epochs, loss=lossg, sigma0=w.sigma0, gain=w.gain,
+                   flat=_dev(w.flat), noise=dia.NOISE_FIXED if noise_fixed else dia.NOISE_MODEL)
+    tho, ro = oracle.fit(cfg, w.R, w.I, w.theta0, oo, mask=w.mask, var=var)
+    thg, rg = h.fit(_dev(w.I), _dev(w.theta0), og, mask=_dev(w.mask), var=_dev(var))
+    h.close()
+    return tho, ro, thg.cpu().numpy(), rg
+
+
+def _assert_fit_close(tho, ro, thg, rg, tag, tol=1e-4):
+    for e in range(tho.shape[0]):
+        Ko, Kg = tho[e][:-1].astype(np.float64), thg[e][:-1].astype(np.float64)
+        dK = np.abs(Kg - Ko).max() / np.abs(Ko).max()
+        dP = abs(rg[e].photometric_scale - ro[e].photometric_scale) / abs(ro[e].photometric_scale)
+        dB = abs(float(thg[e][-1]) - float(tho[e][-1])) / max(abs(float(tho[e][-1])), 1.0)
+        dL = abs(rg[e].loss - ro[e].loss) / abs(ro[e].loss) if ro[e].loss != 0 else abs(rg[e].loss)
+        print(f"{tag} e{e}: dK={dK:.2e} dP={dP:.2e} dB0={dB:.2e} dL={dL:.2e} "
+              f"gpu(adam={rg[e].n_adam}, lbfgs={rg[e].n_lbfgs}, evals={rg[e].n_evals}, st={rg[e].status}) "
+              f"oracle(adam={ro[e].n_adam}, lbfgs={ro[e].n_lbfgs}, evals={ro[e].n_evals}, st={ro[e].status})")
+        assert dP <= tol and dB <= tol and dK <= tol, f"{tag} epoch {e}"
+        assert rg[e].photometric_scale == pytest.approx(Kg.sum(), rel=1e-6)      # Eq. 3
+
+
+@pytest.mark.parametrize("n_adam,n_lbfgs", [(1, 0), (5, 0), (40, 0), (0, 3), (30, 12)])
+def test_fit_lockstep(dia, n_adam, n_lbfgs):
+    """Fixed iteration counts: both sides take exactly the same steps, so the iterates differ only by
+    the FP32 evaluation error of the gradient.  Catches any mistake in the device Adam / two-loop
+    recursion / step-size / history bookkeeping."""
+    w = make_workload(0)
+    og, oo = _both_opts(dia, force_adam_iters=n_adam, force_lbfgs_iters=n_lbfgs)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo)
+    assert rg[0].n_adam == ro[0].n_adam == n_adam
+    assert rg[0].n_lbfgs == ro[0].n_lbfgs
+    assert rg[0].n_evals == ro[0].n_evals
+    _assert_fit_close(tho, ro, thg, rg, f"lockstep {n_adam}/{n_lbfgs}")
+
+
+def test_fit_free_running_config0(dia):
+    """BASELINE config 0 (128^2, m = 7, Gaussian likelihood, seed 0), paper settings."""
+    w = make_workload(0)
+    og, oo = _both_opts(dia)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo)
+    assert rg[0].status in (0, 1) and ro[0].status in (0, 1)
+    _assert_fit_close(tho, ro, thg, rg, "c0 free")
+    # and lands on the planted parameters within the noise (P = 1.2)
+    assert rg[0].photometric_scale == pytest.approx(1.2, abs=0.02)
+
+
+def test_fit_planted_recovery_fixed_mode(dia):
+    """Noise-free target, FIXED variance (reading R12): the minimum is theta_true with L = 0
+    (paper tests (i)-(iii), report eps_P ~ 4e-7 at FP32)."""
+    w = make_workload(0, noise=False)
+    var = np.full(w.I.shape, 25.0, np.float32)
+    og, oo = _both_opts(dia, lr_b0=1.0)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo, var=var, noise_fixed=True)
+    P_true = w.theta_true[0][:-1].sum()
+    assert abs(rg[0].photometric_scale - P_true) / P_true < 1e-4
+    assert abs(ro[0].photometric_scale - P_true) / P_true < 1e-4
+    assert np.abs(thg[0][:-1] - w.theta_true[0][:-1]).max() < 1e-4 * w.theta_true[0][:-1].max() * 10
+
+
+def test_fit_batched_epochs_match_oracle_and_singles(dia):
+    """Batched fit (subsystem 3): epochs converge after different iteration counts inside one graph
+    launch; each must equal the fit of that epoch alone."""
+    w = make_workload(4, n=160, n_epochs=3, m=9)
+    og, oo = _both_opts(dia, max_adam_iters=3000)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo)
+    _assert_fit_close(tho, ro, thg, rg, "c4-small batched")
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=1, sigma0=w.sigma0, gain=w.gain)
+    for e in range(3):
+        th1, r1 = h.fit(_dev(w.I[e:e + 1]), _dev(w.theta0[e:e + 1]), og)
+        assert np.array_equal(th1.cpu().numpy()[0], thg[e])
+        assert (r1[0].n_adam, r1[0].n_lbfgs, r1[0].n_evals) == (rg[e].n_adam, rg[e].n_lbfgs, rg[e].n_evals)
+    h.close()
+
+
+def test_fit_huber_with_cosmic_rays(dia):
+    """BASELINE config 2 shape at reduced size: robust objective, 0.1 % cosmic-ray hits, no mask."""
+    w = make_workload(2, n=200, m=9)
+    og, oo = _both_opts(dia, max_adam_iters=4000)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo)
+    _assert_fit_close(tho, ro, thg, rg, "c2-small huber")
+    assert rg[0].photometric_scale == pytest.approx(1.1, abs=0.03)
+
+
+def test_fit_nonfinite_status(dia):
+    """sigma0 = 0 and a negative model make ln v non-finite (reading R1): status NONFINITE, no hang."""
+    w = make_workload(0, n=64, m=5)
+    h = dia.Handle(_dev(w.R), 5, sigma0=0.0, gain=1.0)
+    th0 = w.theta0.copy()
+    th0[:, :-1] = -0.04
+    th, r = h.fit(_dev(w.I), _dev(th0), dia.FitOpts.default())
+    assert r[0].status == 3 and r[0].n_evals == 1
+    h.close()

@@ -1,0 +1,233 @@
+"""GPU-vs-oracle parity of dia_eval_loss_grad, through the C ABI (python -m pytest -m gpu).
+
+Protocol: on the same seeded inputs
+  loss      |L_gpu - L_or| <= 1e-5 |L_or|                                   at every point
+  gradient  e_norm = max|dg| / max|g_or| <= 1e-5                            where the gradient is far from
+                                                                            cancelling (theta_init)
+            e_S    = max_p |dg_p| / S_p <= 1e-5, S_p = sum_V |w| |X_p|      at near-stationary points
+                                                                            (theta_true and perturbations),
+                                                                            e_norm reported
+and repeated evaluations are bit-identical.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def dia():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2104_13715_b200 as dia
+    dia.load_library()
+    return dia
+
+
+def _dev(a, dtype=None):
+    if a is None:
+        return None
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda().contiguous()
+
+
+def _ref_cfg(w, **kw):
+    loss = oracle.LOSS_HUBER if w.loss == "huber" else oracle.LOSS_GAUSSIAN
+    args = dict(loss=loss, sigma0=w.sigma0, gain=w.gain, flat=w.flat)
+    args.update(kw)
+    return oracle.RefConfig(w.n, w.n, w.m, **args)
+
+
+def _handle(dia, w, max_epochs=None, **kw):
+    args = dict(max_epochs=max_epochs or w.n_epochs,
+                loss=dia.LOSS_HUBER if w.loss == "huber" else dia.LOSS_GAUSSIAN,
+                sigma0=w.sigma0, gain=w.gain, flat=_dev(w.flat))
+    args.update(kw)
+    return dia.Handle(_dev(w.R), w.m, **args)
+
+
+def _points(w):
+    """P0 = theta_init, P1 = theta_true, P2 = theta_true (1 + 1e-3 xi)."""
+    rng = np.random.default_rng(77 + w.config.index)
+    p2 = w.theta_true * (1.0 + 1e-3 * rng.standard_normal(w.theta_true.shape))
+    return [("P0", w.theta0.astype(np.float32), "norm"),
+            ("P1", w.theta_true.astype(np.float32), "S"),
+            ("P2", p2.astype(np.float32), "S")]
+
+
+def _compare(Lg, gg, Lo, go, So, kind, tag):
+    Lg, gg = Lg.cpu().numpy(), gg.cpu().numpy()
+    for e in range(Lo.shape[0]):
+        assert abs(Lg[e] - Lo[e]) <= TOL * abs(Lo[e]), f"{tag} epoch {e}: loss {Lg[e]} vs {Lo[e]}"
+        d = np.abs(gg[e] - go[e])
+        e_norm = d.max() / np.abs(go[e]).max()
+        e_S = (d / So[e]).max()
+        print(f"{tag} e{e}: dL/L={abs(Lg[e]-Lo[e])/abs(Lo[e]):.2e} e_norm={e_norm:.2e} e_S={e_S:.2e}")
+        assert e_S <= TOL, f"{tag} epoch {e}: e_S = {e_S:.3e}"
+        if kind == "norm":
+            assert e_norm <= TOL, f"{tag} epoch {e}: e_norm = {e_norm:.3e}"
+
+
+CASES = [  # (config, n, n_epochs): element-by-element sizes the oracle finishes in seconds;
+    (0, None, None),     # several 64x64 tiles plus a ragged tail in every case
+    (1, None, None),
+    (2, 600, None),
+    (3, 500, None),
+    (4, 333, 3),         # odd n: unaligned rows (scalar cp.async path)
+    (4, 520, 2),
+]
+
+
+@pytest.mark.parametrize("c,n,E", CASES)
+def test_eval_parity(dia, c, n, E):
+    w = make_workload(c, n=n, n_epochs=E)
+    h = _handle(dia, w)
+    cfg = _ref_cfg(w)
+    I, mask = _dev(w.I), _dev(w.mask)
+    for name, th, kind in _points(w):
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=w.mask, want_scale=True)
+        Lg, gg = h.eval_loss_grad(I, _dev(th), mask=mask)
+        Lg2, gg2 = h.eval_loss_grad(I, _dev(th), mask=mask)
+        torch.cuda.synchronize()
+        assert torch.equal(Lg, Lg2) and torch.equal(gg, gg2), "evaluation is not deterministic"
+        _compare(Lg, gg, Lo, go, So, kind, f"c{c} n={w.n} {name}")
+    h.close()
+
+
+@pytest.mark.parametrize("loss", ["gaussian", "huber"])
+@pytest.mark.parametrize("m", [1, 3, 5, 9, 11, 13, 17, 21, 23, 27, 29, 31])
+def test_eval_parity_all_kernel_sizes(dia, loss, m):
+    """Every instantiated kernel size, both objectives, FIXED and MODEL noise."""
+    w = make_workload(2 if loss == "huber" else 1, n=150, m=m)
+    for noise in ("model", "fixed"):
+        var = None
+        kw = {}
+        if noise == "fixed":
+            var = (w.sigma0 ** 2 + np.maximum(w.I, 0.0) / w.gain).astype(np.float32)
+            kw = dict(noise=dia.NOISE_FIXED)
+        h = _handle(dia, w, **kw)
+        cfg = _ref_cfg(w, **({"noise": oracle.NOISE_FIXED} if noise == "fixed" else {}))
+        for name, th, kind in _points(w)[:2]:
+            Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, var=var, want_scale=True)
+            Lg, gg = h.eval_loss_grad(_dev(w.I), _dev(th), var=_dev(var))
+            _compare(Lg, gg, Lo, go, So, kind, f"m={m} {loss} {noise} {name}")
+        h.close()
+
+
+def test_rectangular_image(dia):
+    w = make_workload(1, n=200, m=9)
+    R, I = w.R[:137, :], w.I[:, :137, :]
+    cfg = oracle.RefConfig(137, 200, 9, sigma0=w.sigma0, gain=w.gain)
+    h = dia.Handle(_dev(R), 9, sigma0=w.sigma0, gain=w.gain)
+    for th, kind in ((w.theta0, "norm"), (w.theta_true.astype(np.float32), "S")):
+        Lo, go, So = oracle.eval_loss_grad(cfg, R, I, th, want_scale=True)
+        Lg, gg = h.eval_loss_grad(_dev(I), _dev(th))
+        _compare(Lg, gg, Lo, go, So, kind, "rect")
+    h.close()
+
+
+def test_border_poison_and_mask(dia):
+    """Pixels of I / mask / var outside the valid set are never read (include/dia.h); a masked
+    pixel contributes nothing (reading R4)."""
+    w = make_workload(0, n=100, m=7)
+    hh = 3
+    h = _handle(dia, w)
+    th = _dev(w.theta_true.astype(np.float32))
+    L0, g0 = h.eval_loss_grad(_dev(w.I), th)
+    Ip = w.I.copy()
+    Ip[:, :hh, :] = np.nan; Ip[:, -hh:, :] = np.nan; Ip[:, :, :hh] = np.nan; Ip[:, :, -hh:] = np.nan
+    L1, g1 = h.eval_loss_grad(_dev(Ip), th)
+    assert torch.equal(L0, L1) and torch.equal(g0, g1)
+    # NaN under a masked pixel must not leak
+    rng = np.random.default_rng(5)
+    mask = (rng.random(w.I.shape) > 0.3).astype(np.uint8)
+    Ip = w.I.copy()
+    Ip[mask == 0] = np.nan
+    Lg, gg = h.eval_loss_grad(_dev(Ip), th, mask=_dev(mask))
+    Lo, go, So = oracle.eval_loss_grad(_ref_cfg(w), w.R, w.I, w.theta_true.astype(np.float32), mask=mask,
+                                       want_scale=True)
+    _compare(Lg, gg, Lo, go, So, "S", "mask")
+    # everything masked: exact zeros
+    Lz, gz = h.eval_loss_grad(_dev(w.I), th, mask=_dev(np.zeros_like(mask)))
+    assert float(Lz[0]) == 0.0 and float(gz.abs().max()) == 0.0
+    h.close()
+
+
+def test_minimum_size_image(dia):
+    """Degenerate case n == m: a single valid pixel."""
+    rng = np.random.default_rng(2)
+    m = 5
+    R = (100 + 50 * rng.random((m, m))).astype(np.float32)
+    I = (120 + 50 * rng.random((1, m, m))).astype(np.float32)
+    th = np.concatenate([np.full(m * m, 0.04), [2.0]]).astype(np.float32)
+    cfg = oracle.RefConfig(m, m, m, sigma0=3.0, gain=1.5)
+    Lo, go, So = oracle.eval_loss_grad(cfg, R, I, th, want_scale=True)
+    h = dia.Handle(_dev(R), m, sigma0=3.0, gain=1.5)
+    Lg, gg = h.eval_loss_grad(_dev(I), _dev(th))
+    _compare(Lg, gg, Lo, go, So, "norm", "n==m")
+    h.close()
+
+
+def test_batched_equals_singles(dia):
+    """Batched mode (north_star subsystem 3): one launch over E epochs == E single-epoch calls, bit for bit."""
+    w = make_workload(4, n=300, n_epochs=4, m=19)
+    h = _handle(dia, w)
+    th = _dev(w.theta0)
+    I = _dev(w.I)
+    L, g = h.eval_loss_grad(I, th)
+    for e in range(4):
+        Le, ge = h.eval_loss_grad(I[e:e + 1].contiguous(), th[e:e + 1].contiguous())
+        assert torch.equal(Le[0], L[e]) and torch.equal(ge[0], g[e])
+    h.close()
+
+
+def test_argument_errors(dia):
+    w = make_workload(0, n=64, m=5)
+    R = _dev(w.R)
+    with pytest.raises(dia.DiaError):
+        dia.Handle(R, 4)                       # even m
+    with pytest.raises(dia.DiaError):
+        dia.Handle(R, 33)                      # above DIA_MAX_KERNEL_SIZE
+    with pytest.raises(dia.DiaError):
+        dia.Handle(R, 5, gain=0.0)
+    h = dia.Handle(R, 5, sigma0=5.0)
+    with pytest.raises(dia.DiaError):          # n_epochs > max_epochs
+        h.eval_loss_grad(_dev(np.stack([w.I[0], w.I[0]])), _dev(np.stack([w.theta0[0]] * 2)))
+    with pytest.raises(dia.DiaError):          # var given in MODEL mode
+        h.eval_loss_grad(_dev(w.I), _dev(w.theta0), var=_dev(w.I))
+    with pytest.raises(dia.DiaError):          # host tensor
+        h.eval_loss_grad(torch.from_numpy(w.I), _dev(w.theta0))
+    h.close()
+
+
+def test_full_size_sampled_c4(dia):
+    """BASELINE config 4 at full size in bench.py's launch configuration (4096^2, m = 19, batched
+    epochs).  A sparse random mask (1 pixel in 256) makes the result a sum the oracle can afford
+    pixel by pixel; the complementary-mask identity L(all) = L(mask) + L(~mask) ties the unmasked
+    full-size evaluation to it."""
+    E = 2
+    w = make_workload(4, n_epochs=E)
+    rng = np.random.default_rng(99)
+    mask = (rng.random(w.I.shape) < 1.0 / 256).astype(np.uint8)
+    h = _handle(dia, w)
+    cfg = _ref_cfg(w)
+    I = _dev(w.I)
+    for name, th, kind in _points(w)[:2]:
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=mask, want_scale=True)
+        t = _dev(th)
+        Lg, gg = h.eval_loss_grad(I, t, mask=_dev(mask))
+        _compare(Lg, gg, Lo, go, So, kind, f"c4 full sampled {name}")
+        if name == "P0":                       # gradient far from cancelling: FP32 strip rounding only
+            La, ga = h.eval_loss_grad(I, t)
+            Lc, gc = h.eval_loss_grad(I, t, mask=_dev(1 - mask))
+            assert torch.allclose(La, Lg + Lc, rtol=1e-7, atol=0)
+            assert float((ga - (gg + gc)).abs().max()) <= 2e-6 * float(ga.abs().max())
+    h.close()
