@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -17,6 +18,8 @@ struct dia_handle {
   cudaStream_t stream;
   int grid, np, sms;
   size_t smem;
+  int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
+  CUtensorMap tmR;         // valid iff use_tma
   double* d_partials;      // [max_epochs][grid][np+1]
   dia::FitWorkspace fit;   // device optimiser state + cached graph
   std::string err;
@@ -68,26 +71,73 @@ static size_t smem_for(int m) {
   }
   return 0;
 }
-static const void* kernel_for(int m) {
+static void geometry_for(int m, int* rpitch, int* rh) {
   switch (m) {
-#define X(MM) case MM: return (const void*)dia::eval_kernel<MM>;
+#define X(MM) case MM: *rpitch = dia::Geo<MM>::RPITCH; *rh = dia::Geo<MM>::RH; return;
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+}
+// aux = true: mask / flat field / caller variance map present (read from global memory per pixel)
+static const void* kernel_for(int m, bool aux) {
+  switch (m) {
+#define X(MM) case MM: return aux ? (const void*)dia::eval_kernel<MM, true> : (const void*)dia::eval_kernel<MM, false>;
     DIA_FOR_EACH_M(X)
 #undef X
   }
   return nullptr;
 }
 
+// ---------------------------------------------------------------------------------------------
+// TMA tensor maps (driver entry point fetched through the runtime: no link against libcuda)
+// ---------------------------------------------------------------------------------------------
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static encode_tiled_fn get_encode() {
+  static encode_tiled_fn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (encode_tiled_fn)ptr;
+    else
+      cudaGetLastError();
+  }
+  return fn;
+}
+// float32 tensor {n_cols, n_rows[, n_img]} with box {box_w, box_h[, 1]}; out-of-bounds elements read as 0
+static bool make_tensor_map(CUtensorMap* tm, const float* base, int n_cols, int n_rows, int n_img, int box_w,
+                            int box_h) {
+  encode_tiled_fn enc = get_encode();
+  if (!enc) return false;
+  const cuuint32_t rank = n_img > 0 ? 3 : 2;
+  cuuint64_t dims[3] = {(cuuint64_t)n_cols, (cuuint64_t)n_rows, (cuuint64_t)(n_img > 0 ? n_img : 1)};
+  cuuint64_t strides[2] = {(cuuint64_t)n_cols * 4, (cuuint64_t)n_cols * 4 * (cuuint64_t)n_rows};
+  cuuint32_t box[3] = {(cuuint32_t)box_w, (cuuint32_t)box_h, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, rank, (void*)base, dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
 namespace dia {
-const void* eval_kernel_ptr(const dia_handle* h) { return kernel_for(h->cfg.m); }
+const void* eval_kernel_ptr(const dia_handle* h, bool aux) { return kernel_for(h->cfg.m, aux); }
 size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
-cudaError_t launch_eval(const dia_handle* h, const EvalParams& p) {
-  void* args[] = {(void*)&p};
-  return cudaLaunchKernel(kernel_for(h->cfg.m), dim3(h->grid), dim3(kThreads), args, h->smem, h->stream);
+cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm) {
+  void* args[] = {(void*)&p, (void*)&tm};
+  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p)), dim3(h->grid), dim3(kThreads), args, h->smem,
+                          h->stream);
 }
 }  // namespace dia
 
 static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
-                        const float* d_var, const float* d_theta, const int* d_done, dia::EvalParams* p) {
+                        const float* d_var, const float* d_theta, const int* d_done, dia::EvalParams* p,
+                        dia::TensorMaps* tm) {
   const dia_config& c = h->cfg;
   p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
   p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
@@ -97,7 +147,13 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->loss_kind = c.loss;  p->noise_kind = c.noise;
   p->huber_c = c.huber_c;  p->sigma0_sq = c.sigma0 * c.sigma0;
   p->inv_gain = c.noise == DIA_NOISE_MODEL ? 1.0f / c.gain : 0.f;
-  p->r_vec4 = (c.n_cols % 4 == 0) && ((reinterpret_cast<uintptr_t>(h->d_R) & 15) == 0);
+  p->use_tma = 0;
+  std::memset(tm, 0, sizeof(*tm));
+  if (h->use_tma && aligned16(d_I) &&
+      make_tensor_map(&tm->I, d_I, c.n_cols, c.n_rows, n_epochs, dia::kIPitch, dia::kTH)) {
+    tm->R = h->tmR;
+    p->use_tma = 1;
+  }
 }
 
 extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** out) {
@@ -124,12 +180,23 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   h->cfg = *cfg;  h->d_R = d_R;  h->stream = (cudaStream_t)cfg->stream;  h->sms = sms;
   h->np = cfg->m * cfg->m + 1;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
 
-  const void* k = kernel_for(cfg->m);
-  ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
-  if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
   int occ = 0;
-  ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, dia::kThreads, h->smem);
-  if (ce != cudaSuccess || occ < 1) { int rc = cuda_fail(nullptr, ce, "occupancy query"); delete h; return rc; }
+  for (int aux = 0; aux < 2; ++aux) {
+    const void* k = kernel_for(cfg->m, aux != 0);
+    ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
+    if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
+    int o = 0;
+    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, dia::kThreads, h->smem);
+    if (ce != cudaSuccess || o < 1) { int rc = cuda_fail(nullptr, ce, "occupancy query"); delete h; return rc; }
+    occ = (aux == 0 || o < occ) ? o : occ;   // one grid size for both variants
+  }
+  h->use_tma = 0;
+  const char* no_tma = std::getenv("DIA_DISABLE_TMA");   // test hook: force the cp.async staging path
+  if (cfg->n_cols % 4 == 0 && aligned16(d_R) && !(no_tma && no_tma[0] == '1')) {
+    int rpitch = 0, rh = 0;
+    geometry_for(cfg->m, &rpitch, &rh);
+    h->use_tma = make_tensor_map(&h->tmR, d_R, cfg->n_cols, cfg->n_rows, 0, rpitch, rh) ? 1 : 0;
+  }
   const int tiles = ((cfg->n_cols - cfg->m + 1 + dia::kTW - 1) / dia::kTW) * ((cfg->n_rows - cfg->m + 1 + dia::kTH - 1) / dia::kTH);
   h->grid = sms * occ;                       // persistent grid: every CTA resident
   if (h->grid > tiles) h->grid = tiles;
@@ -165,8 +232,9 @@ extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I,
   if (rc != DIA_OK) return rc;
   if (!d_loss || !d_grad) return fail(h, DIA_ERR_INVALID_ARG, "null output");
   dia::EvalParams p;
-  fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p);
-  cudaError_t ce = dia::launch_eval(h, p);
+  dia::TensorMaps tm;
+  fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm);
+  cudaError_t ce = dia::launch_eval(h, p, tm);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "eval launch");
   const int np1 = h->np + 1;
   dia::reduce_partials_kernel<<<dim3((np1 + 127) / 128, n_epochs), 128, 0, h->stream>>>(
@@ -185,9 +253,10 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   if (opts->lbfgs_history < 1 || opts->lbfgs_history > dia::kMaxHistory)
     return fail(h, DIA_ERR_INVALID_ARG, "lbfgs_history out of range");
   dia::EvalParams p;
-  fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p);
+  dia::TensorMaps tm;
+  fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
   std::string err;
-  rc = dia::fit_run(&h->fit, h, p, *opts, n_epochs, d_theta, d_result, h->grid, h->stream, &err);
+  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, h->grid, h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
   return DIA_OK;
 }

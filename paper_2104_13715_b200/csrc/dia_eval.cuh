@@ -1,16 +1,22 @@
 // dia_eval.cuh -- fused loss + gradient kernel for the B08 discrete-pixel kernel model (sm_100a).
 //
-// One persistent CTA loops over 64x64 tiles of the valid region.  Per tile:
-//   stage   R tile + (m-1) halo and the I tile into shared memory with cp.async (double buffered),
-//   forward each thread owns a 16-pixel row strip: M = R (x) K + B0 (Eq. 2) in FP32
-//           registers, then residual, variance (Eq. 6), loss term (Eq. 8 / Eq. 12-13,
-//           PAPER.md:115, 154-161) and the weight w = dL/dM, written back over the I tile,
-//   grad    thread (a, s) owns the m accumulators g[a][0..m-1] and correlates 16-pixel chunks of w
-//           against the staged R rows (dL/dK[a][b] = sum w_ij R[i+a][j+b]),
-//   flush   per-tile FP32 strips are summed over s in fixed order and added to FP64 accumulators.
-// Nothing n^2-sized is written to HBM.  The tile->CTA map and every reduction order are fixed, so
-// repeated evaluations are bit-identical.
+// One persistent CTA (256 threads, 2 CTAs per SM) loops over 64x64 tiles of the valid region.  Per tile:
+//   stage    one elected thread issues two TMA tensor copies (cp.async.bulk.tensor): the R tile plus its
+//            (m-1) halo, and the I tile, zero filled outside the image; completion is signalled on
+//            mbarriers, the copies of tile t+1 overlap the gradient phase of tile t.  (Images whose rows
+//            are not 16-byte aligned take a cp.async path that fills the same shared-memory layout.)
+//   forward  each thread owns a 16-pixel row strip: M = R (x) K + B0 (Eq. 2) in FP32
+//            registers, then residual, variance (Eq. 6), loss term (Eq. 8 / Eq. 12-13,
+//            PAPER.md:115, 154-161) and the weight w = dL/dM, written to the shared w tile,
+//   grad     thread (a, s) owns the m accumulators g[a][0..m-1] and correlates 16-pixel chunks of w
+//            against the staged R rows (dL/dK[a][b] = sum w_ij R[i+a][j+b]); the FP32 accumulators
+//            live in a thread-private shared-memory row between tiles,
+//   flush    once per epoch (and every kFlushTiles tiles) the FP32 strips are summed over s in fixed
+//            order in FP64 and written to this CTA's partials.
+// Two CTA-wide barriers per tile.  Nothing n^2-sized is written to HBM.  The tile->CTA map and every
+// reduction order are fixed, so repeated evaluations are bit-identical.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -20,12 +26,15 @@ constexpr int kThreads = 256;
 constexpr int kTW = 64, kTH = 64;     // output tile
 constexpr int kP = 16;                // forward strip / gradient chunk length (pixels)
 constexpr int kIPitch = 68;           // I/w tile pitch (floats); 68/4 = 17 is odd => conflict-free rows
+constexpr int kFlushTiles = 32;       // FP32 gradient strips are folded into FP64 at least this often
+constexpr int kSmemBudget = 113 * 1024;   // per CTA, two CTAs per SM
 
 __host__ __device__ constexpr int round_up(int x, int q) { return (x + q - 1) / q * q; }
 
 template <int M>
 struct Geo {
   static constexpr int H = (M - 1) / 2;
+  static constexpr int IOFF = H % 4;                         // column shift of the staged I tile
   static constexpr int NP = M * M + 1;                       // parameters per epoch
   static constexpr int RH = kTH + M - 1;                     // staged R rows
   static constexpr int RSEG = round_up(kP + M - 1, 4);       // floats a thread loads per R row
@@ -37,11 +46,25 @@ struct Geo {
   static constexpr int R_FLOATS = RH * RPITCH;
   static constexpr int I_FLOATS = kTH * kIPitch;
   static constexpr int K_FLOATS = M * KP;
-  static constexpr int RED_FLOATS = S * M * M;               // aliases the current R buffer
-  static constexpr int NOUT = (M * M + kThreads - 1) / kThreads;   // FP64 accumulators per thread
-  static constexpr size_t SMEM = sizeof(float) * (2 * R_FLOATS + 2 * I_FLOATS + K_FLOATS) + 64;
-  static_assert(RED_FLOATS <= R_FLOATS, "reduction scratch must fit in one R buffer");
+  static constexpr int ACC_FLOATS = kThreads * KP;           // thread-private FP32 gradient strips
+  static constexpr int R_BYTES = R_FLOATS * 4, I_BYTES = I_FLOATS * 4;
+  static constexpr int R_STRIDE = round_up(R_BYTES, 128);    // TMA destinations are 128-byte aligned
+  static constexpr int FIXED_BYTES = 4 * (2 * I_FLOATS + K_FLOATS + ACC_FLOATS) + 1024;
+  // two R buffers when they fit next to a second resident CTA, else one (the copy of the next R
+  // tile then waits for the gradient phase to finish)
+  static constexpr int NRBUF = (FIXED_BYTES + 2 * R_STRIDE <= kSmemBudget) ? 2 : 1;
+  // shared-memory map (byte offsets from a 128-byte aligned base)
+  static constexpr int OFF_R = 0;
+  static constexpr int OFF_I = NRBUF * R_STRIDE;
+  static constexpr int I_STRIDE = round_up(I_BYTES, 128);
+  static constexpr int OFF_W = OFF_I + I_STRIDE;
+  static constexpr int OFF_ACC = OFF_W + I_STRIDE;
+  static constexpr int OFF_K = OFF_ACC + 4 * ACC_FLOATS;
+  static constexpr int OFF_BAR = round_up(OFF_K + 4 * K_FLOATS, 16);
+  static constexpr size_t SMEM = OFF_BAR + 64 + 128 + 128;   // mbarriers, FP64 scratch, alignment slack
   static_assert(RPITCH % 8 == 4, "pitch");
+  static_assert(R_BYTES % 16 == 0 && I_BYTES % 16 == 0, "TMA sizes");
+  static_assert(RPITCH <= 256 && RH <= 256, "TMA box limits");
 };
 
 struct EvalParams {
@@ -57,53 +80,59 @@ struct EvalParams {
   int tiles_x, tiles_y;
   int loss_kind, noise_kind;
   float huber_c, sigma0_sq, inv_gain;
-  int r_vec4;                // 1: R rows are 16-byte aligned (n_cols % 4 == 0 and base aligned)
+  int use_tma;               // 1: rows are 16-byte aligned, tensor maps are valid
 };
 
-__device__ __forceinline__ void cp_async_16(void* smem, const void* gmem, int src_bytes) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
-}
-__device__ __forceinline__ void cp_async_4(void* smem, const void* gmem, int src_bytes) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+struct TensorMaps {          // passed by value as a __grid_constant__ kernel parameter
+  CUtensorMap R;             // 2-D {n_cols, n_rows}, box {RPITCH, RH}
+  CUtensorMap I;             // 3-D {n_cols, n_rows, E}, box {kIPitch, kTH, 1}
+};
 
-// Stage one tile: R rows [y0, y0+RH) x cols [x0, x0+RPITCH) and the I tile, zero filled outside.
-template <int M>
-__device__ __forceinline__ void stage_tile(const EvalParams& p, const float* __restrict__ Iep,
-                                           float* Rs, float* Is, int ty, int tx) {
-  using G = Geo<M>;
-  const int y0 = ty * kTH, x0 = tx * kTW;
-  if (p.r_vec4) {
-    constexpr int C4 = G::RPITCH / 4;
-    for (int idx = threadIdx.x; idx < G::RH * C4; idx += kThreads) {
-      const int rr = idx / C4, c4 = idx - rr * C4;
-      const int gy = y0 + rr, gx = x0 + 4 * c4;
-      const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
-      const float* src = ok ? p.R + (size_t)gy * p.n_cols + gx : p.R;
-      cp_async_16(Rs + rr * G::RPITCH + 4 * c4, src, ok ? 16 : 0);
-    }
-  } else {
-    for (int idx = threadIdx.x; idx < G::RH * G::RPITCH; idx += kThreads) {
-      const int rr = idx / G::RPITCH, cc = idx - rr * G::RPITCH;
-      const int gy = y0 + rr, gx = x0 + cc;
-      const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
-      const float* src = ok ? p.R + (size_t)gy * p.n_cols + gx : p.R;
-      cp_async_4(Rs + rr * G::RPITCH + cc, src, ok ? 4 : 0);
-    }
-  }
-  const int vr = p.n_rows - M + 1, vc = p.n_cols - M + 1;
-  for (int idx = threadIdx.x; idx < kTH * kTW; idx += kThreads) {
-    const int rr = idx / kTW, cc = idx - rr * kTW;
-    const int iy = y0 + rr, ix = x0 + cc;
-    const bool ok = (iy < vr) && (ix < vc);
-    const float* src = ok ? Iep + (size_t)(iy + G::H) * p.n_cols + (ix + G::H) : Iep;
-    cp_async_4(Is + rr * kIPitch + cc, src, ok ? 4 : 0);
-  }
+// ------------------------------------------------------------------------------------------------
+// PTX helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void cp_async_4(unsigned dst, const void* gmem, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(dst), "l"(gmem), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive(unsigned bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int x, int y, unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::
+          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* tm, int x, int y, int z, unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::
+          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 __device__ __forceinline__ double warp_sum_f64(double v) {
@@ -112,19 +141,229 @@ __device__ __forceinline__ double warp_sum_f64(double v) {
   return v;
 }
 
+// ------------------------------------------------------------------------------------------------
+// staging: executed by every thread at CTA-uniform points
+// ------------------------------------------------------------------------------------------------
+// R rows [y0, y0+RH) x cols [x0, x0+RPITCH), zero filled outside the image.
 template <int M>
-__global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p) {
+__device__ __forceinline__ void stage_R(const EvalParams& p, const TensorMaps& tm, int tile, unsigned dst, unsigned bar) {
   using G = Geo<M>;
-  extern __shared__ __align__(16) float smem[];
-  float* Rbuf[2] = {smem, smem + G::R_FLOATS};
-  float* Ibuf[2] = {smem + 2 * G::R_FLOATS, smem + 2 * G::R_FLOATS + G::I_FLOATS};
-  float* Ks = smem + 2 * G::R_FLOATS + 2 * G::I_FLOATS;
-  __shared__ double red64[2][kThreads / 32];
+  const int ty = tile / p.tiles_x, tx = tile - ty * p.tiles_x;
+  const int y0 = ty * kTH, x0 = tx * kTW;
+  if (p.use_tma) {
+    if (threadIdx.x == 0) {
+      fence_proxy_async();
+      mbar_expect_tx(bar, G::R_BYTES);
+      tma_load_2d(dst, &tm.R, x0, y0, bar);
+    }
+  } else {
+    for (int idx = threadIdx.x; idx < G::RH * G::RPITCH; idx += kThreads) {
+      const int rr = idx / G::RPITCH, cc = idx - rr * G::RPITCH;
+      const int gy = y0 + rr, gx = x0 + cc;
+      const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
+      const float* src = ok ? p.R + (size_t)gy * p.n_cols + gx : p.R;
+      cp_async_4(dst + 4u * (unsigned)idx, src, ok ? 4 : 0);
+    }
+    cp_async_mbar_arrive(bar);
+  }
+}
+
+// I rows [y0+H, y0+H+kTH) x cols [x0+H-IOFF, x0+H-IOFF+kIPitch) of epoch e, zero filled outside the image.
+// A TMA box must start on a 16-byte boundary of the row, so the tile starts IOFF = H mod 4 columns early and
+// pixel (r, c) of the tile sits at Is[r * kIPitch + c + IOFF].
+template <int M>
+__device__ __forceinline__ void stage_I(const EvalParams& p, const TensorMaps& tm, int e, int tile, unsigned dst,
+                                        unsigned bar) {
+  using G = Geo<M>;
+  const int ty = tile / p.tiles_x, tx = tile - ty * p.tiles_x;
+  const int y0 = ty * kTH + G::H, x0 = tx * kTW + G::H - G::IOFF;
+  if (p.use_tma) {
+    if (threadIdx.x == 0) {
+      fence_proxy_async();
+      mbar_expect_tx(bar, G::I_BYTES);
+      tma_load_3d(dst, &tm.I, x0, y0, e, bar);
+    }
+  } else {
+    const float* Iep = p.I + (size_t)e * p.n_rows * p.n_cols;
+    for (int idx = threadIdx.x; idx < kTH * kIPitch; idx += kThreads) {
+      const int rr = idx / kIPitch, cc = idx - rr * kIPitch;
+      const int gy = y0 + rr, gx = x0 + cc;
+      const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
+      const float* src = ok ? Iep + (size_t)gy * p.n_cols + gx : Iep;
+      cp_async_4(dst + 4u * (unsigned)(rr * kIPitch + cc), src, ok ? 4 : 0);
+    }
+    cp_async_mbar_arrive(bar);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// per-pixel residual / noise / loss / weight (D1)
+//   AUX = false: noise model of Eq. 6 with F == 1, no mask (the fast path)
+//   AUX = true : any of mask / flat field / caller variance map, read from global memory
+// ------------------------------------------------------------------------------------------------
+template <bool AUX, bool EDGE>
+__device__ __forceinline__ void pixel_terms(const EvalParams& p, int e, size_t npix, size_t gidx, bool inside,
+                                            float Mv, float Iv, float& li, float& wi) {
+  bool use = EDGE ? inside : true;
+  float v, bp;
+  if (AUX) {
+    if (use && p.mask) use = p.mask[(size_t)e * npix + gidx] != 0;
+    if (p.noise_kind == 0) {
+      float a_ij = p.sigma0_sq, b_ij = p.inv_gain;
+      if (p.flat && use) {
+        const float invF = 1.0f / p.flat[gidx];
+        a_ij *= invF * invF;
+        b_ij *= invF;
+      }
+      v = fmaf(b_ij, fmaxf(Mv, 0.f), a_ij);
+      bp = Mv > 0.f ? b_ij : 0.f;
+    } else {
+      v = use ? p.var[(size_t)e * npix + gidx] : 1.f;
+      bp = 0.f;
+    }
+  } else {
+    v = fmaf(p.inv_gain, fmaxf(Mv, 0.f), p.sigma0_sq);
+    bp = Mv > 0.f ? p.inv_gain : 0.f;
+  }
+  const float res = Iv - Mv;
+  const float inv_v = rcp_approx(v);
+  const float hb = 0.5f * bp * inv_v;
+  const float z2 = res * res * inv_v;
+  li = 0.5f * z2;
+  wi = fmaf(-res, inv_v, hb * (1.0f - z2));
+  if (p.loss_kind == 1) {                          // Huber, Eq. 12
+    const float rsd = rsqrtf(v);
+    const float z = res * rsd;
+    if (fabsf(z) > p.huber_c) {
+      const float psi = copysignf(p.huber_c, z);
+      li = p.huber_c * (fabsf(z) - 0.5f * p.huber_c);
+      wi = fmaf(-psi, rsd, hb * (1.0f - psi * z));
+    }
+  }
+  if (!AUX || p.noise_kind == 0) li = fmaf(0.5f, logf(v), li);
+  if (AUX || EDGE) {
+    if (!use) { li = 0.f; wi = 0.f; }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// forward: M for the 16-pixel strip at (f_row, f_col) of the tile.  Kernel rows are taken in pairs
+// (0, M-1), (1, M-2), ... and the centre row last; inside a row the columns go wings -> centre.
+// Each pair is one FP32 chain that is then added to the running total, so the large centre terms
+// come last ("accumulation order").
+// ------------------------------------------------------------------------------------------------
+template <int M>
+__device__ __forceinline__ void row_chain(const float* __restrict__ Ks, const float* __restrict__ Rrow, int a,
+                                          float (&rs)[kP], bool first) {
+  using G = Geo<M>;
+  float k[G::KP], r[G::RSEG];
+  const float4* k4 = reinterpret_cast<const float4*>(Ks + a * G::KP);
+#pragma unroll
+  for (int q = 0; q < G::KP / 4; ++q) {
+    const float4 v = k4[q];
+    k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
+  }
+  const float4* r4 = reinterpret_cast<const float4*>(Rrow + a * G::RPITCH);
+#pragma unroll
+  for (int q = 0; q < G::RSEG / 4; ++q) {
+    const float4 v = r4[q];
+    r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
+  }
+  if (first) {
+#pragma unroll
+    for (int q = 0; q < kP; ++q) rs[q] = k[0] * r[q];
+  } else {
+#pragma unroll
+    for (int q = 0; q < kP; ++q) rs[q] = fmaf(k[0], r[q], rs[q]);
+  }
+#pragma unroll
+  for (int ib = 1; ib < M; ++ib) {
+    const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
+#pragma unroll
+    for (int q = 0; q < kP; ++q) rs[q] = fmaf(k[b], r[q + b], rs[q]);
+  }
+}
+
+template <int M>
+__device__ __forceinline__ void forward_strip(const float* __restrict__ Ks, const float* __restrict__ Rrow, float B0,
+                                              float (&tot)[kP]) {
+  using G = Geo<M>;
+#pragma unroll
+  for (int q = 0; q < kP; ++q) tot[q] = B0;
+  float rs[kP];
+#pragma unroll 1
+  for (int ip = 0; ip < G::H; ++ip) {
+    row_chain<M>(Ks, Rrow, ip, rs, true);
+    row_chain<M>(Ks, Rrow, M - 1 - ip, rs, false);
+#pragma unroll
+    for (int q = 0; q < kP; ++q) tot[q] += rs[q];
+  }
+  row_chain<M>(Ks, Rrow, G::H, rs, true);
+#pragma unroll
+  for (int q = 0; q < kP; ++q) tot[q] += rs[q];
+}
+
+// epilogue of the forward phase for one strip: loss terms and the w strip
+template <int M, bool AUX, bool EDGE>
+__device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_t npix, int iy, int ix0, int vr, int vc,
+                                               const float (&tot)[kP], const float* __restrict__ irow,
+                                               float* __restrict__ wrow, float& lsum, float& wsum) {
+  using G = Geo<M>;
+  float iv[kP];
+  if (G::IOFF == 0) {
+#pragma unroll
+    for (int q = 0; q < kP / 4; ++q) {
+      const float4 v = reinterpret_cast<const float4*>(irow)[q];
+      iv[4 * q] = v.x; iv[4 * q + 1] = v.y; iv[4 * q + 2] = v.z; iv[4 * q + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int q = 0; q < kP; ++q) iv[q] = irow[q + G::IOFF];
+  }
+  const size_t gbase = (size_t)(iy + G::H) * p.n_cols + (ix0 + G::H);
+  lsum = 0.f; wsum = 0.f;
+#pragma unroll
+  for (int q = 0; q < kP; ++q) {
+    float li, wi;
+    pixel_terms<AUX, EDGE>(p, e, npix, gbase + q, (iy < vr) && (ix0 + q < vc), tot[q], iv[q], li, wi);
+    lsum += li;
+    wsum += wi;
+    iv[q] = wi;
+  }
+#pragma unroll
+  for (int q = 0; q < kP / 4; ++q)
+    reinterpret_cast<float4*>(wrow)[q] = make_float4(iv[4 * q], iv[4 * q + 1], iv[4 * q + 2], iv[4 * q + 3]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// the fused kernel
+// ------------------------------------------------------------------------------------------------
+template <int M, bool AUX>
+__global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, const __grid_constant__ TensorMaps tm) {
+  using G = Geo<M>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  // 128-byte aligned base (TMA destinations)
+  unsigned char* sm = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  float* const Rbase = reinterpret_cast<float*>(sm + G::OFF_R);
+  float* const Is = reinterpret_cast<float*>(sm + G::OFF_I);      // staged I tile (shifted by IOFF columns)
+  float* const Ws = reinterpret_cast<float*>(sm + G::OFF_W);      // w = dL/dM tile
+  float* const accS = reinterpret_cast<float*>(sm + G::OFF_ACC);
+  float* const Ks = reinterpret_cast<float*>(sm + G::OFF_K);
+  const unsigned bar0 = smem_u32(sm + G::OFF_BAR);            // barR[0], barR[1], barI
+  double* const red64 = reinterpret_cast<double*>(sm + G::OFF_BAR + 64);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n_tiles = p.tiles_x * p.tiles_y;
   const int vr = p.n_rows - M + 1, vc = p.n_cols - M + 1;
   const size_t npix = (size_t)p.n_rows * p.n_cols;
+
+  if (tid == 0) {
+    const unsigned cnt = p.use_tma ? 1u : (unsigned)kThreads;
+#pragma unroll
+    for (int b = 0; b < 3; ++b) mbar_init(bar0 + 8u * b, cnt);
+    fence_mbar_init();
+  }
+  __syncthreads();
 
   // forward mapping: warp covers 32 px x 16 rows; lane -> (fx, fy) = (lane & 1, lane >> 1)
   const int f_col = (warp & 1) * 32 + (lane & 1) * kP;
@@ -132,149 +371,95 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p) {
   // gradient mapping: consecutive threads own consecutive kernel rows a
   const int g_a = tid % M, g_s = tid / M;
   const bool g_active = g_s < G::S;
+  float4* const myacc = reinterpret_cast<float4*>(accS + tid * G::KP);
+
+  unsigned it = 0;                         // tiles this CTA has staged so far (mbarrier phase bookkeeping)
+  auto Rbuf = [&](unsigned i) { return Rbase + (G::NRBUF == 2 ? (i & 1u) : 0u) * (G::R_STRIDE / 4); };
+  auto barR = [&](unsigned i) { return bar0 + 8u * (G::NRBUF == 2 ? (i & 1u) : 0u); };
+  const unsigned barI = bar0 + 16u;
+  auto parR = [&](unsigned i) { return G::NRBUF == 2 ? ((i >> 1) & 1u) : (i & 1u); };
+  auto parI = [&](unsigned i) { return i & 1u; };
 
   for (int e = 0; e < p.n_epochs; ++e) {
     if (p.done && p.done[e]) continue;
-    const float* __restrict__ Iep = p.I + (size_t)e * npix;
     const float* __restrict__ th = p.theta + (size_t)e * G::NP;
-    __syncthreads();                       // previous epoch finished with Ks / buffers
+    double* out = p.partials + ((size_t)e * gridDim.x + blockIdx.x) * (G::NP + 1);
+    // the previous epoch ended with a barrier after its last shared-memory reads
     for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
       const int a = idx / G::KP, b = idx - a * G::KP;
       Ks[idx] = (b < M) ? th[a * M + b] : 0.f;
     }
     const float B0 = th[M * M];
-
-    double loss64 = 0.0, gb064 = 0.0;
-    double gacc64[G::NOUT];
 #pragma unroll
-    for (int q = 0; q < G::NOUT; ++q) gacc64[q] = 0.0;
+    for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+    double loss64 = 0.0, gb064 = 0.0;
+    bool flushed = false;
+    int since_flush = 0;
 
     int t = blockIdx.x;
-    int buf = 0;
-    if (t < n_tiles) stage_tile<M>(p, Iep, Rbuf[0], Ibuf[0], t / p.tiles_x, t % p.tiles_x);
-    cp_async_commit();
+    if (t < n_tiles) {
+      stage_R<M>(p, tm, t, smem_u32(Rbuf(it)), barR(it));
+      stage_I<M>(p, tm, e, t, smem_u32(Is), barI);
+    }
+    __syncthreads();                       // Ks visible
 
-    for (; t < n_tiles; t += gridDim.x, buf ^= 1) {
-      const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
-      cp_async_wait<0>();
-      __syncthreads();                     // tile t landed; everyone is done with the other buffers
-      {
-        const int tn = t + gridDim.x;
-        if (tn < n_tiles) stage_tile<M>(p, Iep, Rbuf[buf ^ 1], Ibuf[buf ^ 1], tn / p.tiles_x, tn % p.tiles_x);
-        cp_async_commit();
+    // fold the FP32 strips of all pixel sub-sets into this CTA's FP64 partials, fixed order
+    auto flush = [&]() {
+      __syncthreads();
+      for (int o = tid; o < M * M; o += kThreads) {
+        const int a = o / M, b = o - a * M;
+        double s = 0.0;
+#pragma unroll 1
+        for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
+        out[o] = flushed ? out[o] + s : s;
       }
-      const float* __restrict__ Rs = Rbuf[buf];
-      float* __restrict__ Ws = Ibuf[buf];
+      __syncthreads();
+#pragma unroll
+      for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+      flushed = true;
+      since_flush = 0;
+    };
+
+    for (; t < n_tiles; t += gridDim.x, ++it) {
+      const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
+      const int tn = t + gridDim.x;
+      const float* __restrict__ Rs = Rbuf(it);
+      mbar_wait(barR(it), parR(it));
+      mbar_wait(barI, parI(it));
 
       // ------------------------------------------------------------------ forward
       {
         float tot[kP];
-#pragma unroll
-        for (int q = 0; q < kP; ++q) tot[q] = B0;
-        // kernel rows outer -> inner, each row chain wings -> centre, rows combined in FP32:
-        // keeps the large centre terms last ("accumulation order")
-#pragma unroll 1
-        for (int ia = 0; ia < M; ++ia) {
-          const int a = (ia & 1) ? (M - 1 - (ia >> 1)) : (ia >> 1);
-          float k[G::KP], r[G::RSEG];
-          const float4* k4 = reinterpret_cast<const float4*>(Ks + a * G::KP);
-#pragma unroll
-          for (int q = 0; q < G::KP / 4; ++q) {
-            const float4 v = k4[q];
-            k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
-          }
-          const float4* r4 = reinterpret_cast<const float4*>(Rs + (f_row + a) * G::RPITCH + f_col);
-#pragma unroll
-          for (int q = 0; q < G::RSEG / 4; ++q) {
-            const float4 v = r4[q];
-            r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
-          }
-          float rs[kP];
-#pragma unroll
-          for (int q = 0; q < kP; ++q) rs[q] = k[0] * r[q];
-#pragma unroll
-          for (int ib = 1; ib < M; ++ib) {
-            const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
-#pragma unroll
-            for (int q = 0; q < kP; ++q) rs[q] = fmaf(k[b], r[q + b], rs[q]);
-          }
-#pragma unroll
-          for (int q = 0; q < kP; ++q) tot[q] += rs[q];
-        }
-        // ---------------------------------------------------------------- residual, noise, loss, weight
+        forward_strip<M>(Ks, Rs + f_row * G::RPITCH + f_col, B0, tot);
         const int iy = tile_y * kTH + f_row, ix0 = tile_x * kTW + f_col;
+        const float* irow = Is + f_row * kIPitch + f_col;
         float* wrow = Ws + f_row * kIPitch + f_col;
-        float iv4[kP];
-#pragma unroll
-        for (int q = 0; q < kP / 4; ++q) {
-          const float4 v = reinterpret_cast<const float4*>(wrow)[q];
-          iv4[4 * q] = v.x; iv4[4 * q + 1] = v.y; iv4[4 * q + 2] = v.z; iv4[4 * q + 3] = v.w;
-        }
-        float lsum = 0.f, wsum = 0.f;
-        const size_t gbase = (size_t)(iy + G::H) * p.n_cols + (ix0 + G::H);
-#pragma unroll
-        for (int q = 0; q < kP; ++q) {
-          bool use = (iy < vr) && (ix0 + q < vc);
-          if (use && p.mask) use = p.mask[(size_t)e * npix + gbase + q] != 0;
-          const float Mv = tot[q];
-          float v, bp;
-          if (p.noise_kind == 0) {
-            float a_ij = p.sigma0_sq, b_ij = p.inv_gain;
-            if (p.flat && use) {
-              const float invF = 1.0f / p.flat[gbase + q];
-              a_ij *= invF * invF;
-              b_ij *= invF;
-            }
-            v = fmaf(b_ij, fmaxf(Mv, 0.f), a_ij);
-            bp = Mv > 0.f ? b_ij : 0.f;
-          } else {
-            v = use ? p.var[(size_t)e * npix + gbase + q] : 1.f;
-            bp = 0.f;
-          }
-          const float res = iv4[q] - Mv;
-          const float inv_v = 1.0f / v;
-          const float hb = 0.5f * bp * inv_v;
-          float li, wi;
-          const float z2 = res * res * inv_v;
-          bool lin = false;
-          float rsd = 0.f, z = 0.f;
-          if (p.loss_kind == 1) {
-            rsd = rsqrtf(v);
-            z = res * rsd;
-            lin = fabsf(z) > p.huber_c;
-          }
-          if (!lin) {
-            li = 0.5f * z2;
-            wi = fmaf(-res, inv_v, hb * (1.0f - z2));
-          } else {
-            const float psi = copysignf(p.huber_c, z);
-            li = p.huber_c * (fabsf(z) - 0.5f * p.huber_c);
-            wi = fmaf(-psi, rsd, hb * (1.0f - psi * z));
-          }
-          if (p.noise_kind == 0) li = fmaf(0.5f, logf(v), li);
-          if (!use) { li = 0.f; wi = 0.f; }
-          lsum += li;
-          wsum += wi;
-          iv4[q] = wi;
-        }
-#pragma unroll
-        for (int q = 0; q < kP / 4; ++q)
-          reinterpret_cast<float4*>(wrow)[q] = make_float4(iv4[4 * q], iv4[4 * q + 1], iv4[4 * q + 2], iv4[4 * q + 3]);
+        float lsum, wsum;
+        const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
+        if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
+        else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
         loss64 += (double)lsum;
         gb064 += (double)wsum;
       }
-      __syncthreads();                     // w tile complete
+      __syncthreads();                     // (A) w tile complete, I tile consumed
+      if (tn < n_tiles) {
+        stage_I<M>(p, tm, e, tn, smem_u32(Is), barI);
+        if (G::NRBUF == 2) stage_R<M>(p, tm, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
+      }
 
       // ------------------------------------------------------------------ gradient
-      float acc[M];
-#pragma unroll
-      for (int b = 0; b < M; ++b) acc[b] = 0.f;
       if (g_active) {
+        float acc[G::KP];
+#pragma unroll
+        for (int q = 0; q < G::KP / 4; ++q) {
+          const float4 v = myacc[q];
+          acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
+        }
         const int rows_here = min(kTH, vr - tile_y * kTH);
         const int n_items = rows_here * (kTW / kP);
 #pragma unroll 1
-        for (int it = g_s; it < n_items; it += G::S) {
-          const int i = it / (kTW / kP), c = it - i * (kTW / kP);
+        for (int item = g_s; item < n_items; item += G::S) {
+          const int i = item / (kTW / kP), c = item - i * (kTW / kP);
           float w[kP], r[G::RSEG];
           const float4* w4 = reinterpret_cast<const float4*>(Ws + i * kIPitch + c * kP);
 #pragma unroll
@@ -293,45 +478,27 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p) {
 #pragma unroll
             for (int b = 0; b < M; ++b) acc[b] = fmaf(w[q], r[q + b], acc[b]);
         }
-      }
-      __syncthreads();                     // all reads of Rs / Ws done; Rs becomes the scratch
-      float* red = Rbuf[buf];
-      if (g_active) {
 #pragma unroll
-        for (int b = 0; b < M; ++b) red[g_s * (M * M) + g_a * M + b] = acc[b];
+        for (int q = 0; q < G::KP / 4; ++q)
+          myacc[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
       }
-      __syncthreads();
-#pragma unroll
-      for (int q = 0; q < G::NOUT; ++q) {
-        const int o = tid + q * kThreads;
-        if (o < M * M) {
-          double s = 0.0;
-#pragma unroll 1
-          for (int ss = 0; ss < G::S; ++ss) s += (double)red[ss * (M * M) + o];
-          gacc64[q] += s;
-        }
-      }
-      // the next iteration's first __syncthreads orders these reads before the buffer is re-staged
+      __syncthreads();                     // (B) everyone is done reading this w tile and R buffer
+      if (G::NRBUF == 1 && tn < n_tiles) stage_R<M>(p, tm, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
+      if (++since_flush == kFlushTiles && tn < n_tiles) flush();
     }
-    cp_async_wait<0>();
 
     // ---------------------------------------------------------------- per-epoch block partials
-    double* out = p.partials + ((size_t)e * gridDim.x + blockIdx.x) * (G::NP + 1);
-#pragma unroll
-    for (int q = 0; q < G::NOUT; ++q) {
-      const int o = tid + q * kThreads;
-      if (o < M * M) out[o] = gacc64[q];
-    }
+    flush();                               // ends with a barrier after the last reads of accS
     const double l = warp_sum_f64(loss64), g0 = warp_sum_f64(gb064);
-    __syncthreads();
-    if (lane == 0) { red64[0][warp] = l; red64[1][warp] = g0; }
+    if (lane == 0) { red64[warp] = l; red64[8 + warp] = g0; }
     __syncthreads();
     if (tid == 0) {
       double ls = 0.0, gs = 0.0;
-      for (int w = 0; w < kThreads / 32; ++w) { ls += red64[0][w]; gs += red64[1][w]; }
+      for (int w = 0; w < kThreads / 32; ++w) { ls += red64[w]; gs += red64[8 + w]; }
       out[M * M] = gs;
       out[M * M + 1] = ls;
     }
+    __syncthreads();                       // red64 / Ks / accS free for the next epoch
   }
 }
 

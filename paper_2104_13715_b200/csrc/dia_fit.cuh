@@ -21,8 +21,9 @@ constexpr int kMaxHistory = 128;
 constexpr int kFitThreads = 256;
 constexpr int kMaxPerThread = 4;      // ceil((31*31+1) / 256)
 
-cudaError_t launch_eval(const dia_handle* h, const EvalParams& p);
-const void* eval_kernel_ptr(const dia_handle* h);
+inline bool eval_is_aux(const EvalParams& p) { return p.mask || p.flat || p.var || p.noise_kind != 0; }
+cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm);
+const void* eval_kernel_ptr(const dia_handle* h, bool aux);
 size_t eval_smem_bytes(const dia_handle* h);
 
 enum { PH_ADAM = 0, PH_LBFGS = 1, PH_DONE = 2 };
@@ -373,7 +374,8 @@ inline void fit_workspace_destroy(FitWorkspace* w) {
 #define DIA_CU(x) do { cudaError_t _e = (x); if (_e != cudaSuccess) { *err = std::string(#x) + ": " + cudaGetErrorString(_e); return DIA_ERR_CUDA; } } while (0)
 
 // Builds (or reuses) the fit graph  init -> WHILE { eval ; step }  and launches it once.
-inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, const dia_fit_opts& o,
+inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, const TensorMaps& tm,
+                   const dia_fit_opts& o,
                    int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, cudaStream_t stream,
                    std::string* err) {
   unsigned char key[256];
@@ -405,9 +407,10 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     cudaGraph_t body = cp.conditional.phGraph_out[0];
     // body: eval -> step
     EvalParams pe = p;
-    void* eval_args[] = {(void*)&pe};
+    TensorMaps tme = tm;
+    void* eval_args[] = {(void*)&pe, (void*)&tme};
     cudaKernelNodeParams ke = {};
-    ke.func = (void*)eval_kernel_ptr(h); ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
+    ke.func = (void*)eval_kernel_ptr(h, eval_is_aux(p)); ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
     ke.sharedMemBytes = (unsigned)eval_smem_bytes(h); ke.kernelParams = eval_args; ke.extra = nullptr;
     cudaGraphNode_t n_eval, n_step;
     DIA_CU(cudaGraphAddKernelNode(&n_eval, body, nullptr, 0, &ke));
