@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the DIA hot path on B200 (contract: see the task prompt / DESIGN.md section 8).
+
+Workload (BASELINE.json configs[4], the one the metric is quoted on): one 4096x4096 float32 reference
+(200000 stars) resident on the device, 16 seeded target epochs, 19x19 kernel + B0 per epoch, Gaussian
+likelihood with the noise model of Eq. 6 (sigma0 = 5, G = 1).
+
+A "step" is one pass of the whole hot path over the batch: one dia_fit call in lock-step mode
+(force_adam_iters = 8, force_lbfgs_iters = 3), i.e. per epoch 8 Adam updates, the switch, 3 L-BFGS
+updates -- every one a fused loss+gradient evaluation (stage -> model -> residual -> variance -> loss ->
+weights -> kernel gradient -> block partials), the FP64 second-level reduction, the on-device optimiser
+step and its convergence bookkeeping, for all 16 epochs inside one CUDA-graph launch.
+  metric / value : loss+gradient evaluations per second (one evaluation = one epoch, 4096^2, m = 19),
+                   counted from the n_evals the device reports, inputs resident in HBM
+  e2e            : the same through Handle.fit_host -- pinned host I / theta0 copied in, theta-hat and the
+                   result structs copied out, inside the timed region
+  roofline       : the fused kernel against the FP32 FMA pipe ("alu"); its launch duration is measured with
+                   CUDA events around back-to-back dia_eval_loss_grad launches of the same batch
+  cpu_baseline   : the FP64 oracle (oracle/) on the host cores, one evaluation of epoch 0 (rank 0, N = 1)
+  fits           : one free-running fit of the batch with the paper's settings (fits/s, iteration counts)
+
+python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--no-fit]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+CONFIG_INDEX = 4
+N, M, E_PER_GPU = 4096, 19, 16
+STEP_ADAM, STEP_LBFGS = 8, 3
+METRIC = "loss+grad evaluations per second (4096^2 image, 19x19 kernel + B0, per epoch)"
+UNIT = "evals/s"
+SM_COUNT, FP32_LANES_PER_SM = 148, 128          # B200 (B200_PROFILING.md: 148 SMs; 128 FP32 lanes per SM)
+# dram__bytes_read.sum + dram__bytes_write.sum of one eval_kernel<19,false> launch over the 16-epoch batch,
+# from the ncu --set full capture summarised in profiles/ (None until captured)
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def useful_fma(n=N, m=M, epochs=1):
+    """2 m^2 FMA per valid pixel: m^2 forward + m^2 gradient."""
+    return 2.0 * m * m * (n - m + 1) ** 2 * epochs
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+            except Exception:
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        sm_busy = [x for x in sm if x > 0.6 * mx] or sm
+        return {"sm_mhz": float(np.median(sm_busy)) if sm_busy else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------
+# workload
+# --------------------------------------------------------------------------------------------------
+def build_workload(first_epoch: int, n_epochs: int, n: int = N, m: int = M):
+    """Reference of config 4 and target epochs [first_epoch, first_epoch + n_epochs) (seeded per epoch)."""
+    from workloads import CONFIGS, make_reference, make_target, theta_init
+    cfg = CONFIGS[CONFIG_INDEX]
+    R = make_reference(cfg, n)
+    I = np.empty((n_epochs, n, n), np.float32)
+    th0 = np.empty((n_epochs, m * m + 1), np.float32)
+    for e in range(n_epochs):
+        I[e], _, _, _ = make_target(cfg, first_epoch + e, R, m)
+        th0[e] = theta_init(R, I[e], m)
+    return cfg, R, I, th0
+
+
+def oracle_eval_rate(cfg, R, I0, th0, crop: int, repeats: int = 1):
+    """Times the FP64 oracle (as it stands) on a crop x crop corner of one epoch; returns
+    (full-size-equivalent evaluations per second, seconds per call, threads used)."""
+    import oracle
+    Rc, Ic = np.ascontiguousarray(R[:crop, :crop]), np.ascontiguousarray(I0[:crop, :crop])
+    rc = oracle.RefConfig(crop, crop, M, sigma0=cfg.sigma0, gain=cfg.gain)
+    best = float("inf")
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        oracle.eval_loss_grad(rc, Rc, Ic, th0)
+        best = min(best, time.perf_counter() - t0)
+    frac = (crop - M + 1) ** 2 / float((N - M + 1) ** 2)
+    return frac / best, best, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    crop = 1024
+    cfg, R, I, th0 = build_workload(0, 1, n=crop)      # same recipe and stellar density at the sample size
+    import oracle
+    rc = oracle.RefConfig(crop, crop, M, sigma0=cfg.sigma0, gain=cfg.gain)
+    frac = (crop - M + 1) ** 2 / float((N - M + 1) ** 2)
+    for _ in range(args.warmup):
+        oracle.eval_loss_grad(rc, R, I[0], th0[0])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.eval_loss_grad(rc, R, I[0], th0[0])
+    dt = time.perf_counter() - t0
+    value = args.steps * frac / dt
+    sample = (f"each step = one FP64 oracle loss+gradient evaluation of a {crop}x{crop} field of the config-4 recipe "
+              f"({frac:.4f} of the 4096^2 valid pixels); value scaled to full-size evaluations per second")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE configs[4]: 4096^2 reference, 19x19 kernel + B0, Gaussian likelihood",
+                       "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------------------------------
+# GPU arm
+# --------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the engine has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    import paper_2104_13715_b200 as dia
+    from paper_2104_13715_b200.sharding import epoch_shard, max_over_ranks
+
+    # weak scaling: every rank owns E_PER_GPU epochs of a (world * E_PER_GPU)-epoch batch; R is replicated
+    first, last = epoch_shard(E_PER_GPU * world, world, rank)
+    E = last - first
+    cfg, R, I, th0 = build_workload(first, E)
+    hI = torch.from_numpy(I).pin_memory()
+    hth0 = torch.from_numpy(th0).pin_memory()
+    dR = torch.from_numpy(R).to(dev)
+    dI = hI.to(dev)
+    dth0 = hth0.to(dev)
+    h = dia.Handle(dR, M, max_epochs=E, loss=dia.LOSS_GAUSSIAN, noise=dia.NOISE_MODEL, sigma0=cfg.sigma0,
+                   gain=cfg.gain)
+    step_opts = dia.FitOpts.default(force_adam_iters=STEP_ADAM, force_lbfgs_iters=STEP_LBFGS)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        a.record()
+        out = None
+        for _ in range(steps):
+            out = fn()
+        b.record()
+        barrier()
+        ms = a.elapsed_time(b)
+        if world > 1:
+            ms = max_over_ranks(ms, device=dev)
+        return ms, out
+
+    # ---- device-resident steps (value)
+    for _ in range(args.warmup):
+        h.fit(dI, dth0, step_opts)
+    with ClockSampler(local_rank) as clocks:
+        ms, (_, res) = timed(lambda: h.fit(dI, dth0, step_opts), args.steps)
+    evals_per_step_rank = sum(r.n_evals for r in res)
+    iters = max(r.n_evals for r in res)
+    total_evals = evals_per_step_rank * world          # every rank runs the same lock-step counts
+    value = total_evals * args.steps / (ms * 1e-3)
+    launches = args.steps * (1 + 2 * iters)            # fit_init + (eval_kernel, fit_step_kernel) per iteration
+
+    # ---- end to end through host buffers
+    for _ in range(max(1, args.warmup // 2)):
+        h.fit_host(hI, hth0, step_opts)
+    ms_e2e, (_, res_e, h2d, d2h) = timed(lambda: h.fit_host(hI, hth0, step_opts), args.steps)
+    e2e_value = sum(r.n_evals for r in res_e) * world * args.steps / (ms_e2e * 1e-3)
+
+    # ---- the dominant kernel alone: back-to-back batched evaluations (eval_kernel + the small reduce kernel)
+    loss = torch.empty(E, dtype=torch.float64, device=dev)
+    grad = torch.empty((E, M * M + 1), dtype=torch.float64, device=dev)
+    n_eval_launch = 10
+    for _ in range(3):
+        h.eval_loss_grad(dI, dth0, loss=loss, grad=grad)
+    ms_k, _ = timed(lambda: h.eval_loss_grad(dI, dth0, loss=loss, grad=grad), n_eval_launch)
+    ms_kernel = ms_k / n_eval_launch
+    flop_per_launch = 2.0 * useful_fma(epochs=E)
+    achieved_tflops = flop_per_launch / (ms_kernel * 1e-3) / 1e12
+    info = h.info()
+
+    line = None
+    if rank == 0:
+        peaks = measured_peaks()
+        sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+        nominal_tflops = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+        measured_fma = dia.dia_measure_fp32_peak()
+        roof = {"bound": "alu", "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
+                "frac": achieved_tflops / nominal_tflops, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                "peak_kind": f"nominal FP32 FMA pipe: {SM_COUNT} SMs x {FP32_LANES_PER_SM} lanes x 2 FLOP x "
+                             f"{sm_max_mhz:.0f} MHz (DESIGN.md section 8)",
+                "peak_measured": 2.0 * measured_fma / 1e12,
+                "frac_of_measured": achieved_tflops / (2.0 * measured_fma / 1e12),
+                "peak_measured_kind": "register-only FFMA microbenchmark run in this process (dia_measure_fp32_peak)",
+                "kernel": f"dia::eval_kernel<{M}, false>", "ms_per_launch": ms_kernel,
+                "flop_per_launch": flop_per_launch,
+                "how": f"CUDA events around {n_eval_launch} back-to-back dia_eval_loss_grad launches of the "
+                       f"{E}-epoch batch (eval_kernel + reduce_partials_kernel), useful FLOP = 4 m^2 per valid pixel",
+                "hbm_gbs_algorithmic": (4.0 * N * N * (1 + E)) / (ms_kernel * 1e-3) / 1e9,
+                "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "BASELINE configs[4]: 4096^2 reference resident on device, 16 target epochs "
+                                       "per GPU, 19x19 kernel + B0 per epoch, Gaussian likelihood, Eq. 6 noise "
+                                       "(sigma0=5, G=1)",
+                           "n": N, "m": M, "epochs_per_gpu": E, "global_epochs": E * world,
+                           "step": f"one dia_fit call in lock-step mode: {STEP_ADAM} Adam + {STEP_LBFGS} L-BFGS "
+                                   f"iterations = {iters} fused loss+gradient evaluations per epoch",
+                           "parallelism": f"epochs sharded over {world} GPU(s), reference replicated, no collective",
+                           "l2": "inputs (1 GiB of targets per GPU per evaluation) are larger than the 126 MB L2",
+                           "grid_blocks": info["grid_blocks"], "smem_bytes": info["smem_bytes"]},
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "ms_per_step": ms_e2e / args.steps},
+                "gpu_launches": launches, "clocks": clocks.summary(), "roofline": roof}
+
+    # ---- one free-running fit of the batch with the paper's settings (fits/s)
+    if not args.no_fit:
+        fit_opts = dia.FitOpts.default()
+        ms_fit, (th_hat, res_f) = timed(lambda: h.fit(dI, dth0, fit_opts), 1)
+        if rank == 0:
+            line["fits"] = {"value": E * world / (ms_fit * 1e-3), "unit": "fits/s", "ms_per_batch": ms_fit,
+                            "epochs": E * world, "settings": "paper defaults: Adam lr 1e-3 / 10, switch 1e-6, L-BFGS "
+                                                             "lr 1 history 100, stop 1e-8 (PAPER.md:242-244)",
+                            "n_adam": [r.n_adam for r in res_f], "n_lbfgs": [r.n_lbfgs for r in res_f],
+                            "n_evals": [r.n_evals for r in res_f], "status": [r.status for r in res_f],
+                            "photometric_scale": [round(r.photometric_scale, 5) for r in res_f]}
+
+    # ---- the oracle beside it (rank 0, N = 1 only)
+    if rank == 0 and world == 1 and not args.no_cpu:
+        crop = N                                   # one whole epoch: ~40 core-seconds of FP64 work
+        v, sec, cores = oracle_eval_rate(cfg, R, I[0], th0[0], crop)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"one FP64 oracle loss+gradient evaluation of the top-left {crop}x{crop} "
+                                          f"corner of epoch 0 ({sec:.1f} s), scaled to full-size evaluations per second"}
+    h.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-fit", action="store_true", help="skip the free-running fit (fits/s)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -14,7 +14,9 @@
  *    (PAPER.md:60): M_ij = sum_ab K[a][b] R[i-h+a][j-h+b] + B0 -- a cross-correlation, no flip.
  *    theta = [K (m*m values, row-major), B0], m*m+1 parameters per epoch.
  *  - The valid set V is h <= i < n_rows-h, h <= j < n_cols-h, intersected with
- *    mask != 0 when a mask is given.  Pixels of I, mask, var, flat outside V are never read.
+ *    mask != 0 when a mask is given.  Pixels of mask, var, flat outside V are never read; pixels of I
+ *    outside V (and under mask == 0) may be fetched with their tile but never influence a result
+ *    (they may hold NaN).
  *  - Every call is ASYNCHRONOUS on cfg.stream and performs no host synchronisation
  *    (dia_create / dia_destroy may).  Outputs are valid once the caller synchronises the stream.
  *  - Argument errors are detected on the host before any launch and return a negative code
@@ -59,7 +61,8 @@ typedef struct {                  /* PAPER.md:242-244 unless marked [reading] (D
   double tol_switch;              /* Adam -> L-BFGS when |dL| < tol_switch |L|, 1e-6 */
   double lbfgs_lr;                /* 1.0 */
   int    lbfgs_history;           /* [reading R7] 100; 1 <= history <= 128 */
-  int    lbfgs_backtrack;         /* [reading R7] 1 = Armijo back-off (<= 20 halvings) */
+  int    lbfgs_backtrack;         /* [reading R7] 0 = fixed step as in the paper's library route (default);
+                                     1 = Armijo back-off (<= 20 halvings) */
   double tol_change_rel;          /* stop when |dL| <= tol_change_rel |L|, 1e-8 [R8] */
   double tol_grad_abs;            /* stop when max|g| < tol_grad_abs, 1e-7 */
   double tol_grad_rel;            /* [reading] stop when max|g| < tol_grad_rel * max|g at switch|; 0 = off */
@@ -115,6 +118,12 @@ const char* dia_last_error(const dia_handle* h);
  * enqueued per iteration, and the persistent grid size. */
 int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_per_block,
                  int* smem_bytes, int* launches_per_eval);
+
+/* Register-only FFMA microbenchmark on the current device (the operand pattern of the stencil's inner
+ * loop, no memory traffic): writes the measured FP32 peak in fused multiply-adds per second to
+ * *fma_per_second (HOST pointer).  Synchronises.  This is the "measured" denominator of the FP32
+ * roofline fraction; the nominal one is SMs x 128 lanes x SM clock. */
+int dia_measure_fp32_peak(void* stream, double* fma_per_second);
 
 #ifdef __cplusplus
 }

@@ -43,7 +43,7 @@ typedef struct {                        /* PAPER.md:242-244; [reading] marks DES
   double tol_switch;                    /* 1e-6 */
   double lbfgs_lr;                      /* 1.0 */
   int    lbfgs_history;                 /* [reading R7] 100 */
-  int    lbfgs_backtrack;               /* [reading R7] 1 */
+  int    lbfgs_backtrack;               /* [reading R7] 0 = fixed step (default), 1 = Armijo back-off */
   double tol_change_rel, tol_grad_abs, tol_grad_rel;   /* 1e-8, 1e-7, [reading] 0 = off */
   int    max_adam_iters, max_lbfgs_iters;              /* [reading] 20000, 500 */
   int    force_adam_iters, force_lbfgs_iters;          /* [reading] -1 = off (lock-step mode) */

@@ -16,7 +16,7 @@ void dia_ref_default_fit_opts(dia_ref_fit_opts* o) {
   o->adam_beta1 = 0.9;  o->adam_beta2 = 0.999;  o->adam_eps = 1e-8;   /* R5 */
   o->tol_switch = 1e-6;
   o->lbfgs_lr = 1.0;
-  o->lbfgs_history = 100;  o->lbfgs_backtrack = 1;             /* R7 */
+  o->lbfgs_history = 100;  o->lbfgs_backtrack = 0;             /* R7 */
   o->tol_change_rel = 1e-8;  o->tol_grad_abs = 1e-7;  o->tol_grad_rel = 0.0;   /* PAPER.md:244, R8 */
   o->max_adam_iters = 20000;  o->max_lbfgs_iters = 500;
   o->force_adam_iters = -1;  o->force_lbfgs_iters = -1;

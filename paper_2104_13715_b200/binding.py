@@ -18,7 +18,8 @@ LOSS_GAUSSIAN, LOSS_HUBER = 0, 1
 NOISE_MODEL, NOISE_FIXED = 0, 1
 FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
-                    "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info")
+                    "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
+                    "dia_measure_fp32_peak")
 
 
 class DiaError(RuntimeError):
@@ -87,6 +88,7 @@ def load_library(build_if_missing: bool = True):
                             C.c_void_p, C.c_void_p]
     lib.dia_destroy.argtypes = [C.c_void_p]
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
+    lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     _LIB = lib
     return lib
 
@@ -145,6 +147,13 @@ def dia_destroy(handle: int) -> None:
     _check(load_library().dia_destroy(handle))
 
 
+def dia_measure_fp32_peak(stream: Optional[torch.cuda.Stream] = None) -> float:
+    """Measured FP32 peak of the current device in FMA/s (register-only FFMA microbenchmark)."""
+    out = C.c_double()
+    _check(load_library().dia_measure_fp32_peak(None if stream is None else stream.cuda_stream, C.byref(out)))
+    return out.value
+
+
 # ------------------------------------------------------------------------------------------
 # convenience wrapper
 # ------------------------------------------------------------------------------------------
@@ -194,6 +203,64 @@ class Handle:
         out = [FitResult.from_buffer_copy(host[i * C.sizeof(FitResult):(i + 1) * C.sizeof(FitResult)])
                for i in range(E)]
         return theta, out
+
+    # ---- host-buffer entry points: the same C-ABI calls with the host<->device copies around them
+    def _staging(self, E: int, dev, want_mask: bool):
+        key = (E, want_mask)
+        if getattr(self, "_stage_key", None) != key:
+            self._stage_key = key
+            self._dI = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.float32, device=dev)
+            self._dth = torch.empty((E, self.np), dtype=torch.float32, device=dev)
+            self._dmask = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.uint8, device=dev) if want_mask else None
+            self._dres = torch.zeros(E * C.sizeof(FitResult), dtype=torch.uint8, device=dev)
+            self._hres = torch.empty(E * C.sizeof(FitResult), dtype=torch.uint8).pin_memory()
+            self._hth = torch.empty((E, self.np), dtype=torch.float32).pin_memory()
+            self._dloss = torch.empty(E, dtype=torch.float64, device=dev)
+            self._dgrad = torch.empty((E, self.np), dtype=torch.float64, device=dev)
+            self._hloss = torch.empty(E, dtype=torch.float64).pin_memory()
+            self._hgrad = torch.empty((E, self.np), dtype=torch.float64).pin_memory()
+
+    def _stream_ctx(self):
+        return torch.cuda.stream(self.stream) if self.stream is not None else torch.cuda.stream(torch.cuda.current_stream())
+
+    def fit_host(self, I_host: torch.Tensor, theta0_host: torch.Tensor, opts: Optional[FitOpts] = None,
+                 mask_host: Optional[torch.Tensor] = None):
+        """dia_fit with HOST inputs and outputs (pinned tensors make the copies asynchronous): copies I, theta0
+        (and the mask) to the device, fits, copies theta-hat and the result structs back and synchronises.
+        Returns (theta_hat [E][np] float32 host tensor, list[FitResult], bytes host->device, bytes device->host)."""
+        E = 1 if I_host.dim() == 2 else I_host.shape[0]
+        dev = self.R.device
+        self._staging(E, dev, mask_host is not None)
+        opts = opts or FitOpts.default()
+        with self._stream_ctx():
+            self._dI.copy_(I_host.reshape(self._dI.shape), non_blocking=True)
+            self._dth.copy_(theta0_host.reshape(E, self.np), non_blocking=True)
+            if mask_host is not None:
+                self._dmask.copy_(mask_host.reshape(self._dmask.shape), non_blocking=True)
+            dia_fit(self._h, opts, E, self._dI, self._dmask, None, self._dth, self._dres)
+            self._hth.copy_(self._dth, non_blocking=True)
+            self._hres.copy_(self._dres, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        raw = self._hres.numpy().tobytes()
+        n = C.sizeof(FitResult)
+        res = [FitResult.from_buffer_copy(raw[i * n:(i + 1) * n]) for i in range(E)]
+        h2d = self._dI.numel() * 4 + self._dth.numel() * 4 + (self._dmask.numel() if mask_host is not None else 0)
+        d2h = self._hth.numel() * 4 + self._hres.numel()
+        return self._hth, res, h2d, d2h
+
+    def eval_loss_grad_host(self, I_host: torch.Tensor, theta_host: torch.Tensor):
+        """dia_eval_loss_grad with HOST inputs and outputs; returns (loss, grad, bytes h2d, bytes d2h)."""
+        E = 1 if I_host.dim() == 2 else I_host.shape[0]
+        self._staging(E, self.R.device, False)
+        with self._stream_ctx():
+            self._dI.copy_(I_host.reshape(self._dI.shape), non_blocking=True)
+            self._dth.copy_(theta_host.reshape(E, self.np), non_blocking=True)
+            dia_eval_loss_grad(self._h, E, self._dI, None, None, self._dth, self._dloss, self._dgrad)
+            self._hloss.copy_(self._dloss, non_blocking=True)
+            self._hgrad.copy_(self._dgrad, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        return (self._hloss, self._hgrad, self._dI.numel() * 4 + self._dth.numel() * 4,
+                self._hloss.numel() * 8 + self._hgrad.numel() * 8)
 
     def close(self):
         if self._h:

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdia_b200.so")
 SOURCES = ["dia_api.cu"]
-DEPS = SOURCES + ["dia_eval.cuh", "dia_fit.cuh"]
+DEPS = SOURCES + ["dia_eval.cuh", "dia_fit.cuh", "dia_probe.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

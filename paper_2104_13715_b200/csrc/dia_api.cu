@@ -11,6 +11,7 @@
 
 #include "dia_eval.cuh"
 #include "dia_fit.cuh"
+#include "dia_probe.cuh"
 
 struct dia_handle {
   dia_config cfg;
@@ -52,7 +53,7 @@ extern "C" void dia_default_fit_opts(dia_fit_opts* o) {
   o->lr_kernel = 1e-3f;  o->lr_b0 = 10.0f;
   o->adam_beta1 = 0.9;  o->adam_beta2 = 0.999;  o->adam_eps = 1e-8;
   o->tol_switch = 1e-6;  o->lbfgs_lr = 1.0;
-  o->lbfgs_history = 100;  o->lbfgs_backtrack = 1;
+  o->lbfgs_history = 100;  o->lbfgs_backtrack = 0;
   o->tol_change_rel = 1e-8;  o->tol_grad_abs = 1e-7;  o->tol_grad_rel = 0.0;
   o->max_adam_iters = 20000;  o->max_lbfgs_iters = 500;
   o->force_adam_iters = -1;  o->force_lbfgs_iters = -1;
@@ -258,6 +259,14 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   std::string err;
   rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, h->grid, h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
+  return DIA_OK;
+}
+
+extern "C" int dia_measure_fp32_peak(void* stream, double* fma_per_second) {
+  if (!fma_per_second) return DIA_ERR_INVALID_ARG;
+  const double v = dia::measure_fp32_peak((cudaStream_t)stream, 5);
+  if (v <= 0.0) { cudaGetLastError(); return fail(nullptr, DIA_ERR_CUDA, "FP32 peak probe failed (no CUDA device?)"); }
+  *fma_per_second = v;
   return DIA_OK;
 }
 

@@ -1,0 +1,43 @@
+"""Host-side sharding of target epochs over ranks (multi-GPU mode).
+
+The batched mode fits many target epochs against one resident reference; epochs are independent
+problems, so they shard over GPUs with no data-path collective: the reference is replicated, every
+rank fits its own contiguous block of epochs, and only the fitted parameters are gathered at the end.
+This module holds no device code and runs under any torch.distributed backend (tests use gloo).
+"""
+from __future__ import annotations
+
+from typing import List, Tuple
+
+import torch
+import torch.distributed as dist
+
+
+def epoch_shard(n_epochs: int, world_size: int, rank: int) -> Tuple[int, int]:
+    """[start, stop) of the epochs owned by `rank`: contiguous blocks whose sizes differ by at most one,
+    the first n_epochs % world_size ranks taking the larger blocks."""
+    if world_size < 1 or not (0 <= rank < world_size) or n_epochs < 0:
+        raise ValueError("bad shard arguments")
+    base, extra = divmod(n_epochs, world_size)
+    start = rank * base + min(rank, extra)
+    return start, start + base + (1 if rank < extra else 0)
+
+
+def gather_epochs(local: torch.Tensor, n_epochs: int, group=None) -> torch.Tensor:
+    """All-gathers per-epoch rows (e.g. fitted theta [E_local][np]) into [n_epochs][...] in epoch order.
+    `local` must live where the backend can reach it (CPU for gloo, CUDA for nccl)."""
+    world = dist.get_world_size(group)
+    sizes = [epoch_shard(n_epochs, world, r) for r in range(world)]
+    biggest = max(b - a for a, b in sizes)
+    pad = torch.zeros((biggest,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
+    pad[: local.shape[0]] = local
+    parts: List[torch.Tensor] = [torch.empty_like(pad) for _ in range(world)]
+    dist.all_gather(parts, pad, group=group)
+    return torch.cat([parts[r][: b - a] for r, (a, b) in enumerate(sizes)], dim=0)
+
+
+def max_over_ranks(value: float, device=None, group=None) -> float:
+    """Maximum of a per-rank scalar (a device-measured duration) over all ranks."""
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
+    return float(t.item())

@@ -1,9 +1,14 @@
 """GPU-vs-oracle parity of dia_fit (on-device Adam -> L-BFGS), through the C ABI.
 
-Fit parity protocol: same theta_init and options on both sides;
-  |dP| <= 1e-4 |P|,  |dB0| <= 1e-4 max(|B0|, 1),  max|dK| <= 1e-4 max|K_or|.
-Lock-step mode (force_*_iters) pins the optimiser arithmetic step by step; the free-running
-fits additionally exercise the device-side switch / stop tests.
+Fit parity protocol: same theta_init and options on both sides.
+  strict     |dP| <= 1e-4 |P|,  |dB0| <= 1e-4 max(|B0|, 1),  max|dK| <= 1e-4 max|K_or|
+             required (a) in lock-step mode (force_*_iters: both sides take exactly the same steps, which
+             pins the device Adam / L-BFGS arithmetic) and (b) for free-running fits driven to convergence.
+  model      |dL| <= 1e-5 |L|,  |dP| <= 1e-4 |P|,  ||M_gpu - M_or||_2 <= 1e-4 ||M_or||_2
+             required for free-running fits under the paper's stop rule (relative loss change 1e-8,
+             PAPER.md:244), which ends while the flat directions of K are still undetermined at the 1e-2
+             level (cond(H) 1e6..1e13): there the stopped K depends on every rounding and is reported, not
+             asserted ("parity unpinned").
 """
 import numpy as np
 import pytest
@@ -53,43 +58,75 @@ def _fit_both(dia, w, og, oo, var=None, noise_fixed=False):
     return tho, ro, thg.cpu().numpy(), rg
 
 
+def _diffs(tho, ro, thg, rg, e):
+    Ko, Kg = tho[e][:-1].astype(np.float64), thg[e][:-1].astype(np.float64)
+    dK = np.abs(Kg - Ko).max() / np.abs(Ko).max()
+    dP = abs(rg[e].photometric_scale - ro[e].photometric_scale) / abs(ro[e].photometric_scale)
+    dB = abs(float(thg[e][-1]) - float(tho[e][-1])) / max(abs(float(tho[e][-1])), 1.0)
+    dL = abs(rg[e].loss - ro[e].loss) / abs(ro[e].loss) if ro[e].loss != 0 else abs(rg[e].loss)
+    return dK, dP, dB, dL
+
+
+def _report(tag, e, d, ro, rg):
+    print(f"{tag} e{e}: dK={d[0]:.2e} dP={d[1]:.2e} dB0={d[2]:.2e} dL={d[3]:.2e} "
+          f"gpu(adam={rg[e].n_adam}, lbfgs={rg[e].n_lbfgs}, evals={rg[e].n_evals}, st={rg[e].status}) "
+          f"oracle(adam={ro[e].n_adam}, lbfgs={ro[e].n_lbfgs}, evals={ro[e].n_evals}, st={ro[e].status})")
+
+
 def _assert_fit_close(tho, ro, thg, rg, tag, tol=1e-4):
+    """strict criterion"""
     for e in range(tho.shape[0]):
-        Ko, Kg = tho[e][:-1].astype(np.float64), thg[e][:-1].astype(np.float64)
-        dK = np.abs(Kg - Ko).max() / np.abs(Ko).max()
-        dP = abs(rg[e].photometric_scale - ro[e].photometric_scale) / abs(ro[e].photometric_scale)
-        dB = abs(float(thg[e][-1]) - float(tho[e][-1])) / max(abs(float(tho[e][-1])), 1.0)
-        dL = abs(rg[e].loss - ro[e].loss) / abs(ro[e].loss) if ro[e].loss != 0 else abs(rg[e].loss)
-        print(f"{tag} e{e}: dK={dK:.2e} dP={dP:.2e} dB0={dB:.2e} dL={dL:.2e} "
-              f"gpu(adam={rg[e].n_adam}, lbfgs={rg[e].n_lbfgs}, evals={rg[e].n_evals}, st={rg[e].status}) "
-              f"oracle(adam={ro[e].n_adam}, lbfgs={ro[e].n_lbfgs}, evals={ro[e].n_evals}, st={ro[e].status})")
-        assert dP <= tol and dB <= tol and dK <= tol, f"{tag} epoch {e}"
-        assert rg[e].photometric_scale == pytest.approx(Kg.sum(), rel=1e-6)      # Eq. 3
+        d = _diffs(tho, ro, thg, rg, e)
+        _report(tag, e, d, ro, rg)
+        assert d[1] <= tol and d[2] <= tol and d[0] <= tol, f"{tag} epoch {e}"
+        assert rg[e].photometric_scale == pytest.approx(thg[e][:-1].astype(np.float64).sum(), rel=1e-6)  # Eq. 3
 
 
-@pytest.mark.parametrize("n_adam,n_lbfgs", [(1, 0), (5, 0), (40, 0), (0, 3), (30, 12)])
-def test_fit_lockstep(dia, n_adam, n_lbfgs):
+def _assert_fit_model_close(w, tho, ro, thg, rg, tag):
+    """model criterion: the two fits describe the same model image and photometric scale"""
+    cfg = oracle.RefConfig(w.n, w.n, w.m)
+    for e in range(tho.shape[0]):
+        d = _diffs(tho, ro, thg, rg, e)
+        _report(tag, e, d, ro, rg)
+        Mo, Mg = oracle.model(cfg, w.R, tho[e]), oracle.model(cfg, w.R, thg[e])
+        dM = np.linalg.norm(Mg - Mo) / np.linalg.norm(Mo)
+        print(f"{tag} e{e}: ||dM||/||M|| = {dM:.2e}")
+        assert d[3] <= 1e-5 and d[1] <= 1e-4 and dM <= 1e-4, f"{tag} epoch {e}"
+        assert rg[e].status in (0, 1) and ro[e].status in (0, 1)
+
+
+@pytest.mark.parametrize("n_adam,n_lbfgs,backtrack", [(1, 0, 0), (5, 0, 0), (40, 0, 0), (0, 3, 0), (0, 3, 1),
+                                                       (30, 12, 0), (30, 12, 1)])
+def test_fit_lockstep(dia, n_adam, n_lbfgs, backtrack):
     """Fixed iteration counts: both sides take exactly the same steps, so the iterates differ only by
     the FP32 evaluation error of the gradient.  Catches any mistake in the device Adam / two-loop
     recursion / step-size / history bookkeeping."""
     w = make_workload(0)
-    og, oo = _both_opts(dia, force_adam_iters=n_adam, force_lbfgs_iters=n_lbfgs)
+    og, oo = _both_opts(dia, force_adam_iters=n_adam, force_lbfgs_iters=n_lbfgs, lbfgs_backtrack=backtrack)
     tho, ro, thg, rg = _fit_both(dia, w, og, oo)
     assert rg[0].n_adam == ro[0].n_adam == n_adam
     assert rg[0].n_lbfgs == ro[0].n_lbfgs
     assert rg[0].n_evals == ro[0].n_evals
-    _assert_fit_close(tho, ro, thg, rg, f"lockstep {n_adam}/{n_lbfgs}")
+    _assert_fit_close(tho, ro, thg, rg, f"lockstep {n_adam}/{n_lbfgs}/bt{backtrack}")
 
 
-def test_fit_free_running_config0(dia):
+def test_fit_free_running_config0_paper_stop_rule(dia):
     """BASELINE config 0 (128^2, m = 7, Gaussian likelihood, seed 0), paper settings."""
     w = make_workload(0)
     og, oo = _both_opts(dia)
     tho, ro, thg, rg = _fit_both(dia, w, og, oo)
-    assert rg[0].status in (0, 1) and ro[0].status in (0, 1)
-    _assert_fit_close(tho, ro, thg, rg, "c0 free")
+    _assert_fit_model_close(w, tho, ro, thg, rg, "c0 free")
     # and lands on the planted parameters within the noise (P = 1.2, PAPER.md:65)
     assert rg[0].photometric_scale == pytest.approx(1.2, abs=0.02)
+
+
+def test_fit_free_running_config0_converged(dia):
+    """Same fit driven to convergence (loss-change rule tightened to 1e-13): the objective is convex
+    (PAPER.md:135), so both optimisers must reach the same minimiser -- strict criterion."""
+    w = make_workload(0)
+    og, oo = _both_opts(dia, tol_change_rel=1e-13, max_lbfgs_iters=3000)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo)
+    _assert_fit_close(tho, ro, thg, rg, "c0 converged")
 
 
 def test_fit_planted_recovery_fixed_mode(dia):
@@ -100,18 +137,21 @@ def test_fit_planted_recovery_fixed_mode(dia):
     og, oo = _both_opts(dia, lr_b0=1.0)
     tho, ro, thg, rg = _fit_both(dia, w, og, oo, var=var, noise_fixed=True)
     P_true = w.theta_true[0][:-1].sum()
+    print(f"planted: gpu eps_P={abs(rg[0].photometric_scale - P_true) / P_true:.2e} "
+          f"oracle eps_P={abs(ro[0].photometric_scale - P_true) / P_true:.2e} "
+          f"gpu max|dK|={np.abs(thg[0][:-1] - w.theta_true[0][:-1]).max():.2e}")
     assert abs(rg[0].photometric_scale - P_true) / P_true < 1e-4
     assert abs(ro[0].photometric_scale - P_true) / P_true < 1e-4
-    assert np.abs(thg[0][:-1] - w.theta_true[0][:-1]).max() < 1e-4 * w.theta_true[0][:-1].max() * 10
+    assert np.abs(thg[0][:-1] - w.theta_true[0][:-1]).max() < 1e-3 * w.theta_true[0][:-1].max()
 
 
 def test_fit_batched_epochs_match_oracle_and_singles(dia):
     """Batched fit (subsystem 3): epochs converge after different iteration counts inside one graph
-    launch; each must equal the fit of that epoch alone."""
+    launch; each must equal, bit for bit, the fit of that epoch alone."""
     w = make_workload(4, n=160, n_epochs=3, m=9)
     og, oo = _both_opts(dia, max_adam_iters=3000)
     tho, ro, thg, rg = _fit_both(dia, w, og, oo)
-    _assert_fit_close(tho, ro, thg, rg, "c4-small batched")
+    _assert_fit_model_close(w, tho, ro, thg, rg, "c4-small batched")
     h = dia.Handle(_dev(w.R), w.m, max_epochs=1, sigma0=w.sigma0, gain=w.gain)
     for e in range(3):
         th1, r1 = h.fit(_dev(w.I[e:e + 1]), _dev(w.theta0[e:e + 1]), og)
@@ -125,8 +165,28 @@ def test_fit_huber_with_cosmic_rays(dia):
     w = make_workload(2, n=200, m=9)
     og, oo = _both_opts(dia, max_adam_iters=4000)
     tho, ro, thg, rg = _fit_both(dia, w, og, oo)
-    _assert_fit_close(tho, ro, thg, rg, "c2-small huber")
+    _assert_fit_model_close(w, tho, ro, thg, rg, "c2-small huber")
     assert rg[0].photometric_scale == pytest.approx(1.1, abs=0.03)
+
+
+def test_fit_mask_and_flat(dia):
+    """BASELINE config 3 shape at reduced size: per-pixel flat field and 2 % masked pixels."""
+    w = make_workload(3, n=200, m=9)
+    og, oo = _both_opts(dia, max_adam_iters=4000)
+    tho, ro, thg, rg = _fit_both(dia, w, og, oo)
+    _assert_fit_model_close(w, tho, ro, thg, rg, "c3-small")
+
+
+def test_fit_is_deterministic_and_reusable(dia):
+    """Two fits through the same handle (the cached graph is relaunched) give identical bits."""
+    w = make_workload(0, n=96, m=5)
+    h = dia.Handle(_dev(w.R), w.m, sigma0=w.sigma0, gain=w.gain)
+    og = dia.FitOpts.default()
+    I, th0 = _dev(w.I), _dev(w.theta0)
+    th1, r1 = h.fit(I, th0, og)
+    th2, r2 = h.fit(I, th0, og)
+    assert torch.equal(th1, th2) and r1[0].loss == r2[0].loss and r1[0].n_evals == r2[0].n_evals
+    h.close()
 
 
 def test_fit_nonfinite_status(dia):
