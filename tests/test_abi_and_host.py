@@ -102,7 +102,7 @@ def test_status_strings_and_host_side_argument_errors():
         assert rc == -2 and out.value is None                                   # DIA_ERR_CUDA, no fallback
         cfg.m = 4
         assert lib.dia_create(C.byref(cfg), C.cast(buf, C.c_void_p), C.byref(out)) == -1
-        cfg.m = 33
+        cfg.m, cfg.n_rows, cfg.n_cols = 33, 64, 64
         assert lib.dia_create(C.byref(cfg), C.cast(buf, C.c_void_p), C.byref(out)) == -4
         peak = C.c_double()
         assert lib.dia_measure_fp32_peak(None, C.byref(peak)) == -2
@@ -137,7 +137,8 @@ _WORKER = textwrap.dedent("""
     t = max_over_ranks(10.0 + rank)
     assert t == 10.0 + world - 1
     dist.destroy_process_group()
-    print("rank", rank, "ok")
+    sys.stdout.write("rank%d-ok\n" % rank)
+    sys.stdout.flush()
 """)
 
 
@@ -153,7 +154,7 @@ def test_epoch_sharding_two_ranks_gloo(tmp_path):
            "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)]
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=240)
     assert out.returncode == 0, out.stdout + out.stderr
-    assert "rank 0 ok" in out.stdout and "rank 1 ok" in out.stdout
+    assert "rank0-ok" in out.stdout and "rank1-ok" in out.stdout, out.stdout
 
 
 def test_bench_accounting():
