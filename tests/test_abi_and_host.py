@@ -137,7 +137,7 @@ _WORKER = textwrap.dedent("""
     t = max_over_ranks(10.0 + rank)
     assert t == 10.0 + world - 1
     dist.destroy_process_group()
-    sys.stdout.write("rank%d-ok\n" % rank)
+    print("rank%d-ok" % rank, flush=True)
     sys.stdout.flush()
 """)
 
