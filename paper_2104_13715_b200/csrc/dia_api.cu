@@ -21,7 +21,7 @@ struct dia_handle {
   size_t smem;
   int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
   CUtensorMap tmR;         // valid iff use_tma
-  double* d_partials;      // [max_epochs][grid][np+1]
+  double* d_partials;      // [max_epochs][np+1][grid]
   dia::FitWorkspace fit;   // device optimiser state + cached graph
   std::string err;
 };
@@ -62,7 +62,9 @@ extern "C" void dia_default_fit_opts(dia_fit_opts* o) {
 // ---------------------------------------------------------------------------------------------
 // kernel-size dispatch: one instantiation per odd m
 // ---------------------------------------------------------------------------------------------
+#ifndef DIA_FOR_EACH_M
 #define DIA_FOR_EACH_M(X) X(1) X(3) X(5) X(7) X(9) X(11) X(13) X(15) X(17) X(19) X(21) X(23) X(25) X(27) X(29) X(31)
+#endif
 
 static size_t smem_for(int m) {
   switch (m) {
@@ -238,7 +240,7 @@ extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I,
   cudaError_t ce = dia::launch_eval(h, p, tm);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "eval launch");
   const int np1 = h->np + 1;
-  dia::reduce_partials_kernel<<<dim3((np1 + 127) / 128, n_epochs), 128, 0, h->stream>>>(
+  dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, h->stream>>>(
       h->d_partials, h->grid, np1, nullptr, d_loss, d_grad);
   ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
@@ -257,7 +259,8 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   dia::TensorMaps tm;
   fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
   std::string err;
-  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, h->grid, h->stream, &err);
+    const int unroll = 4;      // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
+  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, h->grid, unroll, h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
   return DIA_OK;
 }

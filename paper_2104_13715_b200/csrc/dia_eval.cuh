@@ -75,7 +75,7 @@ struct EvalParams {
   const float* flat;         // [n_rows][n_cols] or null
   const float* theta;        // [E][NP] float32
   const int* done;           // [E] or null: epochs with done != 0 are skipped
-  double* partials;          // [E][gridDim.x][NP+1]: g_K (M*M), g_B0, loss
+  double* partials;          // [E][NP+1][gridDim.x]: rows g_K (M*M), g_B0, loss; one column per CTA
   int n_rows, n_cols, n_epochs;
   int tiles_x, tiles_y;
   int loss_kind, noise_kind;
@@ -383,7 +383,8 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   for (int e = 0; e < p.n_epochs; ++e) {
     if (p.done && p.done[e]) continue;
     const float* __restrict__ th = p.theta + (size_t)e * G::NP;
-    double* out = p.partials + ((size_t)e * gridDim.x + blockIdx.x) * (G::NP + 1);
+    double* out = p.partials + (size_t)e * (G::NP + 1) * gridDim.x + blockIdx.x;   // element o at out[o * gridDim.x]
+    const size_t ostride = gridDim.x;
     // the previous epoch ended with a barrier after its last shared-memory reads
     for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
       const int a = idx / G::KP, b = idx - a * G::KP;
@@ -411,7 +412,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
         double s = 0.0;
 #pragma unroll 1
         for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
-        out[o] = flushed ? out[o] + s : s;
+        out[o * ostride] = flushed ? out[o * ostride] + s : s;
       }
       __syncthreads();
 #pragma unroll
@@ -495,26 +496,35 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
     if (tid == 0) {
       double ls = 0.0, gs = 0.0;
       for (int w = 0; w < kThreads / 32; ++w) { ls += red64[w]; gs += red64[8 + w]; }
-      out[M * M] = gs;
-      out[M * M + 1] = ls;
+      out[(size_t)(M * M) * ostride] = gs;
+      out[(size_t)(M * M + 1) * ostride] = ls;
     }
     __syncthreads();                       // red64 / Ks / accS free for the next epoch
   }
 }
 
-// Second level: sum the block partials in block order (fixed order => deterministic).
+// Fixed-order sum of one row of block partials by one warp: lane l adds columns l, l+32, ... in order,
+// then the 32 lane sums are combined by a fixed butterfly -- deterministic for a given n_blocks.
+__device__ __forceinline__ double warp_row_sum(const double* __restrict__ row, int n_blocks, int lane) {
+  double s = 0.0;
+  for (int b = lane; b < n_blocks; b += 32) s += row[b];
+  return warp_sum_f64(s);
+}
+
+// Second level: one warp per output sums the block partials (fixed order => deterministic).
 __global__ void reduce_partials_kernel(const double* __restrict__ partials, int n_blocks, int np1,
                                        const int* __restrict__ done, double* __restrict__ loss,
                                        double* __restrict__ grad) {
   const int e = blockIdx.y;
   if (done && done[e]) return;
-  const int o = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  const int o = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (o >= np1) return;
-  const double* src = partials + (size_t)e * n_blocks * np1 + o;
-  double s = 0.0;
-  for (int b = 0; b < n_blocks; ++b) s += src[(size_t)b * np1];
-  if (o == np1 - 1) loss[e] = s;
-  else grad[(size_t)e * (np1 - 1) + o] = s;
+  const double s = warp_row_sum(partials + ((size_t)e * np1 + o) * n_blocks, n_blocks, lane);
+  if (lane == 0) {
+    if (o == np1 - 1) loss[e] = s;
+    else grad[(size_t)e * (np1 - 1) + o] = s;
+  }
 }
 
 }  // namespace dia

@@ -72,25 +72,34 @@ struct StepArgs {
 };
 
 // ---------------------------------------------------------------- block-wide FP64 reductions
-__device__ __forceinline__ double block_sum(double v, double* sh) {
+// One barrier per reduction: two scratch rows are used alternately (`par` toggles on every call, and every
+// call is made by the whole block), so a row is rewritten only after a later barrier that all of its
+// readers have passed.
+struct BlockRed {
+  double (*sh)[kFitThreads / 32];
+  int par;
+};
+__device__ __forceinline__ double block_sum(double v, BlockRed& br) {
   v = warp_sum_f64(v);
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  double* row = br.sh[br.par];
+  br.par ^= 1;
+  if ((threadIdx.x & 31) == 0) row[threadIdx.x >> 5] = v;
   __syncthreads();
   double s = 0.0;
 #pragma unroll
-  for (int w = 0; w < kFitThreads / 32; ++w) s += sh[w];
+  for (int w = 0; w < kFitThreads / 32; ++w) s += row[w];
   return s;
 }
-__device__ __forceinline__ double block_max(double v, double* sh) {
+__device__ __forceinline__ double block_max(double v, BlockRed& br) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) { double u = __shfl_xor_sync(0xffffffffu, v, o); v = (u > v || u != u) ? u : v; }
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  double* row = br.sh[br.par];
+  br.par ^= 1;
+  if ((threadIdx.x & 31) == 0) row[threadIdx.x >> 5] = v;
   __syncthreads();
   double s = 0.0;
 #pragma unroll
-  for (int w = 0; w < kFitThreads / 32; ++w) { double u = sh[w]; s = (u > s || u != u) ? u : s; }
+  for (int w = 0; w < kFitThreads / 32; ++w) { double u = row[w]; s = (u > s || u != u) ? u : s; }
   return s;
 }
 
@@ -118,7 +127,8 @@ __global__ void fit_init_kernel(FitBuffers b, const float* __restrict__ theta_in
 __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a) {
   const int e = blockIdx.x;
   if (a.b.done[e]) return;
-  __shared__ double sh[kFitThreads / 32];
+  __shared__ double sh_rows[2][kFitThreads / 32];
+  BlockRed sh{sh_rows, 0};
   __shared__ double s_alpha[kMaxHistory];
   const int np = a.np, nk = np - 1, tid = threadIdx.x;
   const dia_fit_opts& o = a.o;
@@ -134,22 +144,34 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
   float* th32 = a.b.theta32 + (size_t)e * np;
   const int hist = o.lbfgs_history;
 
-  // ---- second-level reduction of the evaluation's block partials, fixed order
+  // ---- second-level reduction of the evaluation's block partials: one warp per output, fixed order
+  __shared__ double gsum[kFitThreads * kMaxPerThread];
   double gn[kMaxPerThread];
   double Ln = 0.0;
   {
-    const double* src = a.partials + (size_t)e * a.n_blocks * (np + 1);
+    const double* src = a.partials + (size_t)e * (np + 1) * a.n_blocks;
+    const int lane = tid & 31, wid = tid >> 5;
+    // four rows per warp at a time, so that enough loads are in flight to hide the L2 latency
+    for (int k = wid * 4; k < np + 1; k += (kFitThreads / 32) * 4) {
+      double s4[4] = {0.0, 0.0, 0.0, 0.0};
+      for (int b = lane; b < a.n_blocks; b += 32) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (k + j < np + 1) s4[j] += src[(size_t)(k + j) * a.n_blocks + b];
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const double s = warp_sum_f64(s4[j]);
+        if (lane == 0 && k + j < np + 1) gsum[k + j] = s;
+      }
+    }
+    __syncthreads();
 #pragma unroll
     for (int q = 0; q < kMaxPerThread; ++q) {
       const int k = tid + q * kFitThreads;
-      double s = 0.0;
-      if (k < np + 1)
-        for (int blk = 0; blk < a.n_blocks; ++blk) s += src[(size_t)blk * (np + 1) + k];
-      gn[q] = (k < np) ? s : 0.0;
-      if (k == np) sh[0] = s;                    // loss lives in slot np
+      gn[q] = (k < np) ? gsum[k] : 0.0;
     }
-    __syncthreads();
-    Ln = sh[0];
+    Ln = gsum[np];                               // loss lives in row np
     __syncthreads();
   }
   st.n_evals += 1;
@@ -270,6 +292,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
       double gq[kMaxPerThread];
 #pragma unroll
       for (int q = 0; q < kMaxPerThread; ++q) gq[q] = q4[q];
+      // two-loop recursion (N&W Alg. 7.4)
       for (int i = st.n_pairs - 1; i >= 0; --i) {
         const int id = (st.head + i) % hist;
         double part = 0.0;
@@ -376,13 +399,13 @@ inline void fit_workspace_destroy(FitWorkspace* w) {
 // Builds (or reuses) the fit graph  init -> WHILE { eval ; step }  and launches it once.
 inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, const TensorMaps& tm,
                    const dia_fit_opts& o,
-                   int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, cudaStream_t stream,
-                   std::string* err) {
+                   int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, int unroll,
+                   cudaStream_t stream, std::string* err) {
   unsigned char key[256];
   int len = 0;
   auto put = [&](const void* src, size_t n) { std::memcpy(key + len, src, n); len += (int)n; };
   put(&n_epochs, sizeof(int)); put(&p.I, sizeof(void*)); put(&p.mask, sizeof(void*)); put(&p.var, sizeof(void*));
-  put(&d_theta, sizeof(void*)); put(&d_result, sizeof(void*)); put(&o, sizeof(o));
+  put(&d_theta, sizeof(void*)); put(&d_result, sizeof(void*)); put(&o, sizeof(o)); put(&unroll, sizeof(int));
   if (!(w->exec && len == w->key_len && std::memcmp(key, w->key, len) == 0)) {
     if (w->exec) { cudaGraphExecDestroy(w->exec); w->exec = nullptr; }
     if (w->graph) { cudaGraphDestroy(w->graph); w->graph = nullptr; }
@@ -412,8 +435,6 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     cudaKernelNodeParams ke = {};
     ke.func = (void*)eval_kernel_ptr(h, eval_is_aux(p)); ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
     ke.sharedMemBytes = (unsigned)eval_smem_bytes(h); ke.kernelParams = eval_args; ke.extra = nullptr;
-    cudaGraphNode_t n_eval, n_step;
-    DIA_CU(cudaGraphAddKernelNode(&n_eval, body, nullptr, 0, &ke));
     StepArgs sa;
     sa.b = w->b; sa.partials = p.partials; sa.n_blocks = grid; sa.np = w->np; sa.hist_cap = w->hist_cap;
     sa.o = o; sa.theta_out = d_theta; sa.result = d_result; sa.cond = cond;
@@ -421,7 +442,16 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     cudaKernelNodeParams ks = {};
     ks.func = (void*)fit_step_kernel; ks.gridDim = dim3(n_epochs); ks.blockDim = dim3(kFitThreads);
     ks.sharedMemBytes = 0; ks.kernelParams = step_args; ks.extra = nullptr;
-    DIA_CU(cudaGraphAddKernelNode(&n_step, body, &n_eval, 1, &ks));
+    // The body holds `unroll` (eval ; step) pairs: re-evaluating the WHILE condition costs several
+    // microseconds, which matters when an evaluation takes ~10 us (small images).  Pairs that run after
+    // every epoch has stopped find done[e] set and return at once.
+    cudaGraphNode_t prev = nullptr;
+    for (int u = 0; u < unroll; ++u) {
+      cudaGraphNode_t n_eval, n_step;
+      DIA_CU(cudaGraphAddKernelNode(&n_eval, body, prev ? &prev : nullptr, prev ? 1 : 0, &ke));
+      DIA_CU(cudaGraphAddKernelNode(&n_step, body, &n_eval, 1, &ks));
+      prev = n_step;
+    }
     DIA_CU(cudaGraphInstantiate(&w->exec, w->graph, 0));
     std::memcpy(w->key, key, len); w->key_len = len;
   }
