@@ -203,6 +203,10 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   const int tiles = ((cfg->n_cols - cfg->m + 1 + dia::kTW - 1) / dia::kTW) * ((cfg->n_rows - cfg->m + 1 + dia::kTH - 1) / dia::kTH);
   h->grid = sms * occ;                       // persistent grid: every CTA resident
   if (h->grid > tiles) h->grid = tiles;
+  if (const char* lim = std::getenv("DIA_GRID_LIMIT")) {   // test hook: few CTAs => many tiles per CTA
+    const int g = std::atoi(lim);
+    if (g >= 1 && g < h->grid) h->grid = g;
+  }
   ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * h->grid * (h->np + 1));
   if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
   int rc = dia::fit_workspace_create(&h->fit, cfg->max_epochs, h->np);

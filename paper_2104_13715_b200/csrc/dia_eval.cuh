@@ -119,15 +119,29 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
 
-__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int x, int y, unsigned bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::
-          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(bar) : "memory");
+// L2 eviction policies: the reference is re-read for every epoch of a batch (keep it: evict_last), a target
+// tile is read once per evaluation (evict_first), so that a 64 MiB reference stays resident in the 126 MB L2.
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol));
+  return pol;
 }
-__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* tm, int x, int y, int z, unsigned bar) {
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int x, int y, unsigned bar,
+                                            unsigned long long pol) {
   asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::
-          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n" ::
+          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* tm, int x, int y, int z, unsigned bar,
+                                            unsigned long long pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;\n" ::
+          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(bar), "l"(pol) : "memory");
 }
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
@@ -154,7 +168,7 @@ __device__ __forceinline__ void stage_R(const EvalParams& p, const TensorMaps& t
     if (threadIdx.x == 0) {
       fence_proxy_async();
       mbar_expect_tx(bar, G::R_BYTES);
-      tma_load_2d(dst, &tm.R, x0, y0, bar);
+      tma_load_2d(dst, &tm.R, x0, y0, bar, l2_policy_evict_last());
     }
   } else {
     for (int idx = threadIdx.x; idx < G::RH * G::RPITCH; idx += kThreads) {
@@ -181,7 +195,7 @@ __device__ __forceinline__ void stage_I(const EvalParams& p, const TensorMaps& t
     if (threadIdx.x == 0) {
       fence_proxy_async();
       mbar_expect_tx(bar, G::I_BYTES);
-      tma_load_3d(dst, &tm.I, x0, y0, e, bar);
+      tma_load_3d(dst, &tm.I, x0, y0, e, bar, l2_policy_evict_first());
     }
   } else {
     const float* Iep = p.I + (size_t)e * p.n_rows * p.n_cols;

@@ -122,6 +122,30 @@ def test_eval_parity_all_kernel_sizes(dia, loss, m):
         h.close()
 
 
+@pytest.mark.parametrize("grid_limit,disable_tma", [(1, "0"), (3, "0"), (1, "1"), (296, "1")])
+def test_many_tiles_per_cta_and_staging_paths(dia, monkeypatch, grid_limit, disable_tma):
+    """Test hooks DIA_GRID_LIMIT / DIA_DISABLE_TMA: a grid of 1 or 3 CTAs makes every CTA walk through many
+    tiles (double-buffer wrap-around, mbarrier phase flips, the periodic FP64 flush every 32 tiles), and the
+    cp.async staging path is forced on an image whose rows are 16-byte aligned.  Results must still match the
+    oracle, and the two staging paths must agree bit for bit."""
+    monkeypatch.setenv("DIA_GRID_LIMIT", str(grid_limit))
+    monkeypatch.setenv("DIA_DISABLE_TMA", disable_tma)
+    w = make_workload(4, n=600, n_epochs=2, m=19)          # 10 x 10 tiles per epoch
+    h = _handle(dia, w)
+    assert h.info()["grid_blocks"] == min(grid_limit, 100)
+    cfg = _ref_cfg(w)
+    th = w.theta_true.astype(np.float32)
+    Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, want_scale=True)
+    Lg, gg = h.eval_loss_grad(_dev(w.I), _dev(th))
+    _compare(Lg, gg, Lo, go, So, "S", f"grid={grid_limit} tma_off={disable_tma}")
+    h.close()
+    monkeypatch.setenv("DIA_DISABLE_TMA", "1" if disable_tma == "0" else "0")
+    h2 = _handle(dia, w)
+    L2, g2 = h2.eval_loss_grad(_dev(w.I), _dev(th))
+    assert torch.equal(Lg, L2) and torch.equal(gg, g2)
+    h2.close()
+
+
 def test_rectangular_image(dia):
     w = make_workload(1, n=200, m=9)
     R, I = w.R[:137, :], w.I[:, :137, :]
