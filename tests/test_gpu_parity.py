@@ -146,6 +146,32 @@ def test_many_tiles_per_cta_and_staging_paths(dia, monkeypatch, grid_limit, disa
     h2.close()
 
 
+def test_emccd_noise_model_eq7(dia):
+    """EMCCD noise model, Eq. 7: sigma^2 = E M / (G_total F) with E = 2, G_total = 25.8/300
+    e-/ADU -- the affine form of Eq. 6 with no read-noise term, i.e. sigma0 = 0 and gain = G_total / E."""
+    E_excess, G_total = 2.0, 25.8 / 300.0
+    w = make_workload(1, n=200, m=9)
+    rng = np.random.default_rng(3)
+    flat = rng.uniform(0.95, 1.05, w.R.shape).astype(np.float32)
+    gain = G_total / E_excess
+    cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=0.0, gain=gain, flat=flat)
+    th = w.theta_true.astype(np.float32)
+    Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, want_scale=True)
+    # the oracle's value is Eq. 7 written out: check one pixel by hand
+    M = oracle.model(oracle.RefConfig(w.n, w.n, w.m), w.R, th[0])
+    i, j, hh = 57, 91, 4
+    v = E_excess * M[i - hh, j - hh] / (G_total * float(flat[i, j]))
+    mask = np.zeros(w.I.shape, np.uint8); mask[0, i, j] = 1
+    L1, _ = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=mask)
+    r = float(w.I[0, i, j]) - M[i - hh, j - hh]
+    assert L1[0] == pytest.approx(0.5 * r * r / v + 0.5 * np.log(v), rel=1e-9)
+    for disable in ("0", "1"):
+        h = dia.Handle(_dev(w.R), w.m, sigma0=0.0, gain=gain, flat=_dev(flat))
+        Lg, gg = h.eval_loss_grad(_dev(w.I), _dev(th))
+        _compare(Lg, gg, Lo, go, So, "S", "emccd")
+        h.close()
+
+
 def test_rectangular_image(dia):
     w = make_workload(1, n=200, m=9)
     R, I = w.R[:137, :], w.I[:, :137, :]
