@@ -52,6 +52,10 @@ typedef struct {
   int noise;   float sigma0, gain;/* Eq. 6: read noise [ADU] >= 0, gain [e-/ADU] > 0 */
   const float* d_flat;            /* master flat F [n_rows][n_cols] or NULL => F == 1; borrowed for handle life */
   void* stream;                   /* cudaStream_t; NULL = legacy default stream */
+  int n_refs;                     /* 0 or 1: one reference shared by all epochs (d_R is [n_rows][n_cols]);
+                                     == max_epochs: one reference per epoch (d_R is [max_epochs][n_rows][n_cols]) --
+                                     many independent small image pairs fitted in one launch sequence, the
+                                     shape of the paper's stamp workloads */
 } dia_config;
 
 typedef struct {                  /* PAPER.md:242-244 unless marked [reading] */
@@ -80,7 +84,8 @@ typedef struct {
 void dia_default_fit_opts(dia_fit_opts* opts);
 
 /* Creates a handle for one reference image d_R [n_rows][n_cols] (DEVICE, borrowed for the
- * handle's life, must stay unchanged).  Allocates the workspace for cfg->max_epochs epochs.
+ * handle's life, must stay unchanged; [max_epochs][n_rows][n_cols] when cfg->n_refs == max_epochs).
+ * Allocates the workspace for cfg->max_epochs epochs.
  * May synchronise.  Errors: INVALID_ARG (bad sizes/enums/NULLs), UNSUPPORTED (m too large),
  * CUDA, ALLOC. */
 int dia_create(const dia_config* cfg, const float* d_R, dia_handle** out);

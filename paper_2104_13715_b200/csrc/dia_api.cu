@@ -17,11 +17,12 @@ struct dia_handle {
   dia_config cfg;
   const float* d_R;
   cudaStream_t stream;
-  int grid, np, sms;
+  int grid, np, sms;       // grid: resident CTAs (SMs x occupancy), capped by max_epochs x tiles
+  int tiles, n_refs;
   size_t smem;
   int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
   CUtensorMap tmR;         // valid iff use_tma
-  double* d_partials;      // [max_epochs][np+1][grid]
+  double* d_partials;      // [max_epochs][np+1][min(tiles, grid)]
   dia::FitWorkspace fit;   // device optimiser state + cached graph
   std::string err;
 };
@@ -131,10 +132,18 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 namespace dia {
 const void* eval_kernel_ptr(const dia_handle* h, bool aux) { return kernel_for(h->cfg.m, aux); }
 size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
+int eval_grid(const dia_handle* h, int n_epochs) {
+  const long long items = (long long)n_epochs * h->tiles;
+  return items < h->grid ? (int)items : h->grid;
+}
+int eval_part_cols(const dia_handle* h, int n_epochs) {
+  const int g = eval_grid(h, n_epochs);
+  return h->tiles < g ? h->tiles : g;
+}
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm) {
   void* args[] = {(void*)&p, (void*)&tm};
-  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p)), dim3(h->grid), dim3(kThreads), args, h->smem,
-                          h->stream);
+  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p)), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
+                          h->smem, h->stream);
 }
 }  // namespace dia
 
@@ -144,7 +153,7 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   const dia_config& c = h->cfg;
   p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
   p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
-  p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;
+  p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;  p->n_refs = h->n_refs;
   p->tiles_x = (c.n_cols - c.m + 1 + dia::kTW - 1) / dia::kTW;
   p->tiles_y = (c.n_rows - c.m + 1 + dia::kTH - 1) / dia::kTH;
   p->loss_kind = c.loss;  p->noise_kind = c.noise;
@@ -165,6 +174,8 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (cfg->m < 1 || cfg->m % 2 == 0) return fail(nullptr, DIA_ERR_INVALID_ARG, "m must be odd and >= 1");
   if (cfg->n_rows < cfg->m || cfg->n_cols < cfg->m) return fail(nullptr, DIA_ERR_INVALID_ARG, "image smaller than kernel");
   if (cfg->max_epochs < 1) return fail(nullptr, DIA_ERR_INVALID_ARG, "max_epochs must be >= 1");
+  if (cfg->n_refs > 1 && cfg->n_refs != cfg->max_epochs)
+    return fail(nullptr, DIA_ERR_INVALID_ARG, "n_refs must be 0, 1 or max_epochs");
   if (cfg->loss != DIA_LOSS_GAUSSIAN && cfg->loss != DIA_LOSS_HUBER) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad loss");
   if (cfg->noise != DIA_NOISE_MODEL && cfg->noise != DIA_NOISE_FIXED) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad noise mode");
   if (cfg->loss == DIA_LOSS_HUBER && !(cfg->huber_c > 0.f)) return fail(nullptr, DIA_ERR_INVALID_ARG, "huber_c must be > 0");
@@ -180,6 +191,7 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
 
   dia_handle* h = new (std::nothrow) dia_handle();
   if (!h) return fail(nullptr, DIA_ERR_ALLOC, "host allocation failed");
+  h->n_refs = cfg->n_refs > 1 ? cfg->n_refs : 1;
   h->cfg = *cfg;  h->d_R = d_R;  h->stream = (cudaStream_t)cfg->stream;  h->sms = sms;
   h->np = cfg->m * cfg->m + 1;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
 
@@ -198,16 +210,17 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (cfg->n_cols % 4 == 0 && aligned16(d_R) && !(no_tma && no_tma[0] == '1')) {
     int rpitch = 0, rh = 0;
     geometry_for(cfg->m, &rpitch, &rh);
-    h->use_tma = make_tensor_map(&h->tmR, d_R, cfg->n_cols, cfg->n_rows, 0, rpitch, rh) ? 1 : 0;
+    h->use_tma = make_tensor_map(&h->tmR, d_R, cfg->n_cols, cfg->n_rows, h->n_refs, rpitch, rh) ? 1 : 0;
   }
   const int tiles = ((cfg->n_cols - cfg->m + 1 + dia::kTW - 1) / dia::kTW) * ((cfg->n_rows - cfg->m + 1 + dia::kTH - 1) / dia::kTH);
+  h->tiles = tiles;
   h->grid = sms * occ;                       // persistent grid: every CTA resident
-  if (h->grid > tiles) h->grid = tiles;
+  if ((long long)h->grid > (long long)tiles * cfg->max_epochs) h->grid = tiles * cfg->max_epochs;
   if (const char* lim = std::getenv("DIA_GRID_LIMIT")) {   // test hook: few CTAs => many tiles per CTA
     const int g = std::atoi(lim);
     if (g >= 1 && g < h->grid) h->grid = g;
   }
-  ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * h->grid * (h->np + 1));
+  ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * (tiles < h->grid ? tiles : h->grid) * (h->np + 1));
   if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
   int rc = dia::fit_workspace_create(&h->fit, cfg->max_epochs, h->np);
   if (rc != DIA_OK) { cudaFree(h->d_partials); fail(nullptr, rc, "fit workspace allocation failed"); delete h; return rc; }
@@ -245,7 +258,7 @@ extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I,
   if (ce != cudaSuccess) return cuda_fail(h, ce, "eval launch");
   const int np1 = h->np + 1;
   dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, h->stream>>>(
-      h->d_partials, h->grid, np1, nullptr, d_loss, d_grad);
+      h->d_partials, dia::eval_part_cols(h, n_epochs), np1, nullptr, d_loss, d_grad);
   ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
   return DIA_OK;
@@ -264,7 +277,7 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
   std::string err;
     const int unroll = 4;      // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
-  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, h->grid, unroll, h->stream, &err);
+  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid(h, n_epochs), dia::eval_part_cols(h, n_epochs), unroll, h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
   return DIA_OK;
 }

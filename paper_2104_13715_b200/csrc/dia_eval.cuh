@@ -68,15 +68,17 @@ struct Geo {
 };
 
 struct EvalParams {
-  const float* R;            // [n_rows][n_cols]
+  const float* R;            // [n_refs][n_rows][n_cols]
   const float* I;            // [E][n_rows][n_cols]
   const unsigned char* mask; // [E][n_rows][n_cols] or null
   const float* var;          // [E][n_rows][n_cols] or null (FIXED noise)
   const float* flat;         // [n_rows][n_cols] or null
   const float* theta;        // [E][NP] float32
   const int* done;           // [E] or null: epochs with done != 0 are skipped
-  double* partials;          // [E][NP+1][gridDim.x]: rows g_K (M*M), g_B0, loss; one column per CTA
+  double* partials;          // [E][NP+1][ncols], ncols = min(tiles, gridDim.x): rows g_K (M*M), g_B0, loss;
+                             // one column per CTA that owns tiles of the epoch
   int n_rows, n_cols, n_epochs;
+  int n_refs;                // 1: one reference shared by all epochs; else one reference per epoch
   int tiles_x, tiles_y;
   int loss_kind, noise_kind;
   float huber_c, sigma0_sq, inv_gain;
@@ -84,7 +86,7 @@ struct EvalParams {
 };
 
 struct TensorMaps {          // passed by value as a __grid_constant__ kernel parameter
-  CUtensorMap R;             // 2-D {n_cols, n_rows}, box {RPITCH, RH}
+  CUtensorMap R;             // 3-D {n_cols, n_rows, n_refs}, box {RPITCH, RH, 1}
   CUtensorMap I;             // 3-D {n_cols, n_rows, E}, box {kIPitch, kTH, 1}
 };
 
@@ -160,22 +162,25 @@ __device__ __forceinline__ double warp_sum_f64(double v) {
 // ------------------------------------------------------------------------------------------------
 // R rows [y0, y0+RH) x cols [x0, x0+RPITCH), zero filled outside the image.
 template <int M>
-__device__ __forceinline__ void stage_R(const EvalParams& p, const TensorMaps& tm, int tile, unsigned dst, unsigned bar) {
+__device__ __forceinline__ void stage_R(const EvalParams& p, const TensorMaps& tm, int e, int tile, unsigned dst,
+                                        unsigned bar) {
   using G = Geo<M>;
+  const int ref = p.n_refs > 1 ? e : 0;    // one reference per epoch, or one shared by all epochs
   const int ty = tile / p.tiles_x, tx = tile - ty * p.tiles_x;
   const int y0 = ty * kTH, x0 = tx * kTW;
   if (p.use_tma) {
     if (threadIdx.x == 0) {
       fence_proxy_async();
       mbar_expect_tx(bar, G::R_BYTES);
-      tma_load_2d(dst, &tm.R, x0, y0, bar, l2_policy_evict_last());
+      tma_load_3d(dst, &tm.R, x0, y0, ref, bar, l2_policy_evict_last());
     }
   } else {
+    const float* Rref = p.R + (size_t)ref * p.n_rows * p.n_cols;
     for (int idx = threadIdx.x; idx < G::RH * G::RPITCH; idx += kThreads) {
       const int rr = idx / G::RPITCH, cc = idx - rr * G::RPITCH;
       const int gy = y0 + rr, gx = x0 + cc;
       const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
-      const float* src = ok ? p.R + (size_t)gy * p.n_cols + gx : p.R;
+      const float* src = ok ? Rref + (size_t)gy * p.n_cols + gx : Rref;
       cp_async_4(dst + 4u * (unsigned)idx, src, ok ? 4 : 0);
     }
     cp_async_mbar_arrive(bar);
@@ -394,115 +399,41 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   auto parR = [&](unsigned i) { return G::NRBUF == 2 ? ((i >> 1) & 1u) : (i & 1u); };
   auto parI = [&](unsigned i) { return i & 1u; };
 
-  for (int e = 0; e < p.n_epochs; ++e) {
-    if (p.done && p.done[e]) continue;
-    const float* __restrict__ th = p.theta + (size_t)e * G::NP;
-    double* out = p.partials + (size_t)e * (G::NP + 1) * gridDim.x + blockIdx.x;   // element o at out[o * gridDim.x]
-    const size_t ostride = gridDim.x;
-    // the previous epoch ended with a barrier after its last shared-memory reads
-    for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
-      const int a = idx / G::KP, b = idx - a * G::KP;
-      Ks[idx] = (b < M) ? th[a * M + b] : 0.f;
+  // Work items are (epoch, tile) pairs in epoch-major order, item g = e * n_tiles + t; this CTA takes items
+  // blockIdx.x, blockIdx.x + gridDim.x, ...  (so a batch of many small images fills the grid as well as one
+  // large image does), skipping epochs whose `done` flag is set.
+  const int total = p.n_epochs * n_tiles;
+  const int grid = (int)gridDim.x;
+  const int ncols = min(n_tiles, grid);    // CTAs (columns of partials) that contribute to one epoch
+  auto advance = [&](int g) {
+    while (g < total && p.done && p.done[g / n_tiles]) g += grid;
+    return g;
+  };
+
+  float B0 = 0.f;
+  double loss64 = 0.0, gb064 = 0.0;
+  bool flushed = false;
+  int since_flush = 0, cur_e = -1;
+  double* out = nullptr;                   // element o of this CTA's partial column at out[o * ncols]
+
+  // fold the FP32 strips of all pixel sub-sets into this CTA's FP64 partials, fixed order
+  auto flush = [&]() {
+    __syncthreads();
+    for (int o = tid; o < M * M; o += kThreads) {
+      const int a = o / M, b = o - a * M;
+      double s = 0.0;
+#pragma unroll 1
+      for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
+      out[(size_t)o * ncols] = flushed ? out[(size_t)o * ncols] + s : s;
     }
-    const float B0 = th[M * M];
+    __syncthreads();
 #pragma unroll
     for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-    double loss64 = 0.0, gb064 = 0.0;
-    bool flushed = false;
-    int since_flush = 0;
-
-    int t = blockIdx.x;
-    if (t < n_tiles) {
-      stage_R<M>(p, tm, t, smem_u32(Rbuf(it)), barR(it));
-      stage_I<M>(p, tm, e, t, smem_u32(Is), barI);
-    }
-    __syncthreads();                       // Ks visible
-
-    // fold the FP32 strips of all pixel sub-sets into this CTA's FP64 partials, fixed order
-    auto flush = [&]() {
-      __syncthreads();
-      for (int o = tid; o < M * M; o += kThreads) {
-        const int a = o / M, b = o - a * M;
-        double s = 0.0;
-#pragma unroll 1
-        for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
-        out[o * ostride] = flushed ? out[o * ostride] + s : s;
-      }
-      __syncthreads();
-#pragma unroll
-      for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-      flushed = true;
-      since_flush = 0;
-    };
-
-    for (; t < n_tiles; t += gridDim.x, ++it) {
-      const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
-      const int tn = t + gridDim.x;
-      const float* __restrict__ Rs = Rbuf(it);
-      mbar_wait(barR(it), parR(it));
-      mbar_wait(barI, parI(it));
-
-      // ------------------------------------------------------------------ forward
-      {
-        float tot[kP];
-        forward_strip<M>(Ks, Rs + f_row * G::RPITCH + f_col, B0, tot);
-        const int iy = tile_y * kTH + f_row, ix0 = tile_x * kTW + f_col;
-        const float* irow = Is + f_row * kIPitch + f_col;
-        float* wrow = Ws + f_row * kIPitch + f_col;
-        float lsum, wsum;
-        const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
-        if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
-        else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
-        loss64 += (double)lsum;
-        gb064 += (double)wsum;
-      }
-      __syncthreads();                     // (A) w tile complete, I tile consumed
-      if (tn < n_tiles) {
-        stage_I<M>(p, tm, e, tn, smem_u32(Is), barI);
-        if (G::NRBUF == 2) stage_R<M>(p, tm, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
-      }
-
-      // ------------------------------------------------------------------ gradient
-      if (g_active) {
-        float acc[G::KP];
-#pragma unroll
-        for (int q = 0; q < G::KP / 4; ++q) {
-          const float4 v = myacc[q];
-          acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
-        }
-        const int rows_here = min(kTH, vr - tile_y * kTH);
-        const int n_items = rows_here * (kTW / kP);
-#pragma unroll 1
-        for (int item = g_s; item < n_items; item += G::S) {
-          const int i = item / (kTW / kP), c = item - i * (kTW / kP);
-          float w[kP], r[G::RSEG];
-          const float4* w4 = reinterpret_cast<const float4*>(Ws + i * kIPitch + c * kP);
-#pragma unroll
-          for (int q = 0; q < kP / 4; ++q) {
-            const float4 v = w4[q];
-            w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
-          }
-          const float4* r4 = reinterpret_cast<const float4*>(Rs + (i + g_a) * G::RPITCH + c * kP);
-#pragma unroll
-          for (int q = 0; q < G::RSEG / 4; ++q) {
-            const float4 v = r4[q];
-            r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
-          }
-#pragma unroll
-          for (int q = 0; q < kP; ++q)
-#pragma unroll
-            for (int b = 0; b < M; ++b) acc[b] = fmaf(w[q], r[q + b], acc[b]);
-        }
-#pragma unroll
-        for (int q = 0; q < G::KP / 4; ++q)
-          myacc[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
-      }
-      __syncthreads();                     // (B) everyone is done reading this w tile and R buffer
-      if (G::NRBUF == 1 && tn < n_tiles) stage_R<M>(p, tm, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
-      if (++since_flush == kFlushTiles && tn < n_tiles) flush();
-    }
-
-    // ---------------------------------------------------------------- per-epoch block partials
+    flushed = true;
+    since_flush = 0;
+  };
+  // per-epoch block partials: gradient strips, then g_B0 and the loss
+  auto finish_epoch = [&]() {
     flush();                               // ends with a barrier after the last reads of accS
     const double l = warp_sum_f64(loss64), g0 = warp_sum_f64(gb064);
     if (lane == 0) { red64[warp] = l; red64[8 + warp] = g0; }
@@ -510,11 +441,106 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
     if (tid == 0) {
       double ls = 0.0, gs = 0.0;
       for (int w = 0; w < kThreads / 32; ++w) { ls += red64[w]; gs += red64[8 + w]; }
-      out[(size_t)(M * M) * ostride] = gs;
-      out[(size_t)(M * M + 1) * ostride] = ls;
+      out[(size_t)(M * M) * ncols] = gs;
+      out[(size_t)(M * M + 1) * ncols] = ls;
     }
     __syncthreads();                       // red64 / Ks / accS free for the next epoch
+  };
+
+  int g = advance((int)blockIdx.x);
+  if (g < total) {
+    const int e0 = g / n_tiles, t0 = g - e0 * n_tiles;
+    stage_R<M>(p, tm, e0, t0, smem_u32(Rbuf(it)), barR(it));
+    stage_I<M>(p, tm, e0, t0, smem_u32(Is), barI);
   }
+  while (g < total) {
+    const int e = g / n_tiles, t = g - e * n_tiles;
+    const int gn = advance(g + grid);
+    const int en = gn / n_tiles, tn = gn - en * n_tiles;
+    if (e != cur_e) {                      // first tile of an epoch for this CTA
+      if (cur_e >= 0) finish_epoch();
+      cur_e = e;
+      const float* __restrict__ th = p.theta + (size_t)e * G::NP;
+      for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
+        const int a = idx / G::KP, b = idx - a * G::KP;
+        Ks[idx] = (b < M) ? th[a * M + b] : 0.f;
+      }
+      B0 = th[M * M];
+#pragma unroll
+      for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+      loss64 = 0.0; gb064 = 0.0; flushed = false; since_flush = 0;
+      // column of this CTA in epoch e: the local index (mod grid) of the tiles it owns there
+      int col = ((int)blockIdx.x - (int)(((long long)e * n_tiles) % grid) + grid) % grid;
+      out = p.partials + ((size_t)e * (G::NP + 1)) * ncols + col;
+      __syncthreads();                     // Ks visible
+    }
+    const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
+    const float* __restrict__ Rs = Rbuf(it);
+    mbar_wait(barR(it), parR(it));
+    mbar_wait(barI, parI(it));
+
+    // ------------------------------------------------------------------ forward
+    {
+      float tot[kP];
+      forward_strip<M>(Ks, Rs + f_row * G::RPITCH + f_col, B0, tot);
+      const int iy = tile_y * kTH + f_row, ix0 = tile_x * kTW + f_col;
+      const float* irow = Is + f_row * kIPitch + f_col;
+      float* wrow = Ws + f_row * kIPitch + f_col;
+      float lsum, wsum;
+      const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
+      if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
+      else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
+      loss64 += (double)lsum;
+      gb064 += (double)wsum;
+    }
+    __syncthreads();                       // (A) w tile complete, I tile consumed
+    if (gn < total) {
+      stage_I<M>(p, tm, en, tn, smem_u32(Is), barI);
+      if (G::NRBUF == 2) stage_R<M>(p, tm, en, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
+    }
+
+    // ------------------------------------------------------------------ gradient
+    if (g_active) {
+      float acc[G::KP];
+#pragma unroll
+      for (int q = 0; q < G::KP / 4; ++q) {
+        const float4 v = myacc[q];
+        acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
+      }
+      const int rows_here = min(kTH, vr - tile_y * kTH);
+      const int n_items = rows_here * (kTW / kP);
+#pragma unroll 1
+      for (int item = g_s; item < n_items; item += G::S) {
+        const int i = item / (kTW / kP), c = item - i * (kTW / kP);
+        float w[kP], r[G::RSEG];
+        const float4* w4 = reinterpret_cast<const float4*>(Ws + i * kIPitch + c * kP);
+#pragma unroll
+        for (int q = 0; q < kP / 4; ++q) {
+          const float4 v = w4[q];
+          w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
+        }
+        const float4* r4 = reinterpret_cast<const float4*>(Rs + (i + g_a) * G::RPITCH + c * kP);
+#pragma unroll
+        for (int q = 0; q < G::RSEG / 4; ++q) {
+          const float4 v = r4[q];
+          r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
+        }
+#pragma unroll
+        for (int q = 0; q < kP; ++q)
+#pragma unroll
+          for (int b = 0; b < M; ++b) acc[b] = fmaf(w[q], r[q + b], acc[b]);
+      }
+#pragma unroll
+      for (int q = 0; q < G::KP / 4; ++q)
+        myacc[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+    }
+    __syncthreads();                       // (B) everyone is done reading this w tile and R buffer
+    if (G::NRBUF == 1 && gn < total) stage_R<M>(p, tm, en, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
+    if (++since_flush == kFlushTiles && gn < total && en == e) flush();
+    g = gn;
+    ++it;
+  }
+  if (cur_e >= 0) finish_epoch();
 }
 
 // Fixed-order sum of one row of block partials by one warp: lane l adds columns l, l+32, ... in order,

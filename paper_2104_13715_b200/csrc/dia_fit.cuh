@@ -399,7 +399,7 @@ inline void fit_workspace_destroy(FitWorkspace* w) {
 // Builds (or reuses) the fit graph  init -> WHILE { eval ; step }  and launches it once.
 inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, const TensorMaps& tm,
                    const dia_fit_opts& o,
-                   int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, int unroll,
+                   int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, int part_cols, int unroll,
                    cudaStream_t stream, std::string* err) {
   unsigned char key[256];
   int len = 0;
@@ -436,7 +436,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     ke.func = (void*)eval_kernel_ptr(h, eval_is_aux(p)); ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
     ke.sharedMemBytes = (unsigned)eval_smem_bytes(h); ke.kernelParams = eval_args; ke.extra = nullptr;
     StepArgs sa;
-    sa.b = w->b; sa.partials = p.partials; sa.n_blocks = grid; sa.np = w->np; sa.hist_cap = w->hist_cap;
+    sa.b = w->b; sa.partials = p.partials; sa.n_blocks = part_cols; sa.np = w->np; sa.hist_cap = w->hist_cap;
     sa.o = o; sa.theta_out = d_theta; sa.result = d_result; sa.cond = cond;
     void* step_args[] = {(void*)&sa};
     cudaKernelNodeParams ks = {};

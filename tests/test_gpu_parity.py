@@ -132,7 +132,7 @@ def test_many_tiles_per_cta_and_staging_paths(dia, monkeypatch, grid_limit, disa
     monkeypatch.setenv("DIA_DISABLE_TMA", disable_tma)
     w = make_workload(4, n=600, n_epochs=2, m=19)          # 10 x 10 tiles per epoch
     h = _handle(dia, w)
-    assert h.info()["grid_blocks"] == min(grid_limit, 100)
+    assert h.info()["grid_blocks"] == min(grid_limit, 2 * 100)     # 2 epochs x 100 tiles of work items
     cfg = _ref_cfg(w)
     th = w.theta_true.astype(np.float32)
     Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, want_scale=True)
@@ -144,6 +144,42 @@ def test_many_tiles_per_cta_and_staging_paths(dia, monkeypatch, grid_limit, disa
     L2, g2 = h2.eval_loss_grad(_dev(w.I), _dev(th))
     assert torch.equal(Lg, L2) and torch.equal(gg, g2)
     h2.close()
+
+
+def _stamp_batch(n_stamps, n=142, m=19):
+    """Independent small image pairs in the shape of the paper's stamp workloads (142^2, 19x19 kernel,
+    PAPER.md:363-365): every stamp has its own reference (a different crop of a config-2 field) and target."""
+    big = make_workload(2, n=512, m=m)
+    from workloads import make_target, theta_init, CONFIGS
+    Rs, Is, th0, tht = [], [], [], []
+    for k in range(n_stamps):
+        y, x = 37 * (k % 9), 41 * (k // 9 % 9)
+        R = np.ascontiguousarray(big.R[y:y + n, x:x + n])
+        I, th, _, _ = make_target(CONFIGS[0], 100 + k, R, m)       # Gaussian kernel, no outliers, own seed
+        Rs.append(R); Is.append(I); tht.append(th.astype(np.float32)); th0.append(theta_init(R, I, m))
+    return np.stack(Rs), np.stack(Is), np.stack(th0), np.stack(tht)
+
+
+def test_many_small_pairs_one_reference_each(dia):
+    """Batched mode with one reference per epoch (dia_config.n_refs == max_epochs): 12 independent 142^2
+    stamps evaluated in one launch; every stamp must match the oracle run on that stamp alone, and the
+    batch must equal the stamps evaluated one at a time, bit for bit."""
+    S, n, m = 12, 142, 19
+    R, I, th0, tht = _stamp_batch(S, n, m)
+    h = dia.Handle(_dev(R), m, max_epochs=S, sigma0=5.0, gain=1.0)
+    cfg = oracle.RefConfig(n, n, m, sigma0=5.0, gain=1.0)
+    for th, kind in ((th0, "norm"), (tht, "S")):
+        Lg, gg = h.eval_loss_grad(_dev(I), _dev(th))
+        Lo = np.empty(S); go = np.empty((S, m * m + 1)); So = np.empty((S, m * m + 1))
+        for k in range(S):
+            l, g_, s_ = oracle.eval_loss_grad(cfg, R[k], I[k], th[k], want_scale=True)
+            Lo[k], go[k], So[k] = l[0], g_[0], s_[0]
+        _compare(Lg, gg, Lo, go, So, kind, "stamps")
+    h1 = dia.Handle(_dev(R[5]), m, max_epochs=1, sigma0=5.0, gain=1.0)
+    L1, g1 = h1.eval_loss_grad(_dev(I[5:6]), _dev(tht[5:6]))
+    assert torch.equal(L1[0], Lg[5]) and torch.equal(g1[0], gg[5])
+    h1.close()
+    h.close()
 
 
 def test_emccd_noise_model_eq7(dia):
