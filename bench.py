@@ -139,6 +139,51 @@ def oracle_eval_rate(cfg, R, I0, th0, crop: int, repeats: int = 1):
     return frac / best, best, oracle.num_threads()
 
 
+def stamp_batch_rate(dia, dev, n_stamps=296, n=142, m=19):
+    """Throughput of the one-reference-per-epoch mode on synthetic stamps of the paper's stamp shape
+    (142^2 images, 19x19 kernel): batched evaluations and a lock-step fit."""
+    import torch
+    from workloads import CONFIGS, make_reference, make_target, theta_init
+    cfg = CONFIGS[2]
+    big = make_reference(cfg, 1024)                        # crowded field; stamps are crops of it
+    rng = np.random.default_rng(7)
+    R = np.empty((n_stamps, n, n), np.float32); I = np.empty_like(R); th0 = np.empty((n_stamps, m * m + 1), np.float32)
+    for k in range(n_stamps):
+        y, x = rng.integers(0, 1024 - n, 2)
+        R[k] = big[y:y + n, x:x + n]
+        I[k], _, _, _ = make_target(CONFIGS[0], 1000 + k, R[k], m)
+        th0[k] = theta_init(R[k], I[k], m)
+    dR, dI, dth = (torch.from_numpy(a).to(dev) for a in (R, I, th0))
+    h = dia.Handle(dR, m, max_epochs=n_stamps, sigma0=CONFIGS[0].sigma0, gain=CONFIGS[0].gain)
+    loss = torch.empty(n_stamps, dtype=torch.float64, device=dev)
+    grad = torch.empty((n_stamps, m * m + 1), dtype=torch.float64, device=dev)
+    for _ in range(3):
+        h.eval_loss_grad(dI, dth, loss=loss, grad=grad)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(20):
+        h.eval_loss_grad(dI, dth, loss=loss, grad=grad)
+    b.record()
+    torch.cuda.synchronize()
+    ms_eval = a.elapsed_time(b) / 20
+    opts = dia.FitOpts.default(force_adam_iters=100, force_lbfgs_iters=20)
+    h.fit(dI, dth, opts)
+    torch.cuda.synchronize()
+    a.record()
+    _, res = h.fit(dI, dth, opts)
+    b.record()
+    torch.cuda.synchronize()
+    ms_fit = a.elapsed_time(b)
+    h.close()
+    fma = useful_fma(n, m, n_stamps)
+    return {"n_stamps": n_stamps, "n": n, "m": m, "evals_per_s": n_stamps / (ms_eval * 1e-3),
+            "ms_per_batched_eval": ms_eval, "tflops_useful": 2.0 * fma / (ms_eval * 1e-3) / 1e12,
+            "lockstep_fit": {"iterations": res[0].n_evals, "ms": ms_fit,
+                             "stamp_iterations_per_s": n_stamps * res[0].n_evals / (ms_fit * 1e-3)},
+            "note": "one reference per epoch (dia_config.n_refs == max_epochs), one launch sequence for the batch"}
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on the host cores, rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
@@ -300,6 +345,10 @@ def run_gpu(args):
                             "n_evals": [r.n_evals for r in res_f], "status": [r.status for r in res_f],
                             "photometric_scale": [round(r.photometric_scale, 5) for r in res_f]}
 
+    # ---- many small image pairs, one reference each (the paper's stamp workloads)
+    if rank == 0 and not args.no_stamps:
+        line["stamps"] = stamp_batch_rate(dia, dev)
+
     # ---- the oracle beside it (rank 0, N = 1 only)
     if rank == 0 and world == 1 and not args.no_cpu:
         crop = N                                   # one whole epoch: ~40 core-seconds of FP64 work
@@ -323,6 +372,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-fit", action="store_true", help="skip the free-running fit (fits/s)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
+    ap.add_argument("--no-stamps", action="store_true", help="skip the many-small-pairs leg")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
