@@ -56,6 +56,9 @@ typedef struct {
                                      == max_epochs: one reference per epoch (d_R is [max_epochs][n_rows][n_cols]) --
                                      many independent small image pairs fitted in one launch sequence, the
                                      shape of the paper's stamp workloads */
+  float lambda_reg;               /* Eq. 20: adds lambda N_data theta' L' L theta to the objective, L the
+                                     graph Laplacian of the kernel pixels (Eq. 21; 4 edge neighbours, B0 not penalised,
+                                     N_data = valid-region pixels); 0 = off (the paper's own experiments) */
 } dia_config;
 
 typedef struct {                  /* PAPER.md:242-244 unless marked [reading] */

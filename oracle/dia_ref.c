@@ -141,6 +141,38 @@ static void eval_one(const dia_ref_config* cfg, const float* R, const float* I,
   free(tl); free(tg); free(ts);
 }
 
+/* Eq. 20-21: penalty lambda N_data theta' L' L theta with L the graph Laplacian of the
+ * kernel pixels (L_uu = number of adjacent kernel pixels, L_uv = -1 for adjacent u, v; the B0 row and
+ * column are zero).  Readings (R14): "adjacent" = the 4 edge neighbours inside the m x m grid;
+ * N_data = number of valid-region pixels (n_rows-m+1)(n_cols-m+1).  L is symmetric, so the penalty is
+ * lambda N |L theta|^2 and its gradient 2 lambda N L (L theta).  Adds to *loss and grad[0..m*m). */
+static void laplacian_apply(int m, const double* x, double* y) {
+  for (int a = 0; a < m; ++a)
+    for (int b = 0; b < m; ++b) {
+      int nadj = 0;
+      double s = 0.0;
+      if (a > 0)     { nadj++; s += x[(a - 1) * m + b]; }
+      if (a < m - 1) { nadj++; s += x[(a + 1) * m + b]; }
+      if (b > 0)     { nadj++; s += x[a * m + b - 1]; }
+      if (b < m - 1) { nadj++; s += x[a * m + b + 1]; }
+      y[a * m + b] = nadj * x[a * m + b] - s;
+    }
+}
+static void add_penalty(const dia_ref_config* cfg, const float* theta, double* loss, double* grad) {
+  const int m = cfg->m, nk = m * m;
+  const double N = (double)(cfg->n_rows - m + 1) * (double)(cfg->n_cols - m + 1);
+  double* x = (double*)malloc(sizeof(double) * 3 * nk);
+  double* u = x + nk; double* v = u + nk;
+  for (int k = 0; k < nk; ++k) x[k] = (double)theta[k];
+  laplacian_apply(m, x, u);
+  laplacian_apply(m, u, v);
+  double pen = 0.0;
+  for (int k = 0; k < nk; ++k) pen += u[k] * u[k];
+  *loss += cfg->lambda_reg * N * pen;
+  for (int k = 0; k < nk; ++k) grad[k] += 2.0 * cfg->lambda_reg * N * v[k];
+  free(x);
+}
+
 int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epochs,
                            const float* I, const unsigned char* mask, const float* var,
                            const float* theta, double* loss, double* grad, double* grad_scale) {
@@ -149,10 +181,12 @@ int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epoc
   if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
   const size_t npix = (size_t)cfg->n_rows * cfg->n_cols;
   const int np = cfg->m * cfg->m + 1;
-  for (int e = 0; e < n_epochs; ++e)
+  for (int e = 0; e < n_epochs; ++e) {
     eval_one(cfg, R, I + e * npix, mask ? mask + e * npix : NULL, var ? var + e * npix : NULL,
              theta + (size_t)e * np, loss + e, grad + (size_t)e * np,
              grad_scale ? grad_scale + (size_t)e * np : NULL);
+    if (cfg->lambda_reg > 0.0) add_penalty(cfg, theta + (size_t)e * np, loss + e, grad + (size_t)e * np);
+  }
   return DIA_REF_OK;
 }
 

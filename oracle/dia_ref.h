@@ -35,6 +35,7 @@ typedef struct {
   int loss;    double huber_c;          /* c = 1.345 default */
   int noise;   double sigma0, gain;     /* Eq. 6 parameters */
   const float* flat;                    /* [n_rows][n_cols] or NULL => F == 1 */
+  double lambda_reg;                    /* Eq. 20: lambda of the Laplacian penalty, 0 = off */
 } dia_ref_config;
 
 typedef struct {                        /* PAPER.md:242-244; [reading] marks DESIGN.md readings */

@@ -18,7 +18,7 @@ class _Config(C.Structure):
     _fields_ = [("n_rows", C.c_int), ("n_cols", C.c_int), ("m", C.c_int),
                 ("loss", C.c_int), ("huber_c", C.c_double),
                 ("noise", C.c_int), ("sigma0", C.c_double), ("gain", C.c_double),
-                ("flat", C.c_void_p)]
+                ("flat", C.c_void_p), ("lambda_reg", C.c_double)]
 
 
 class RefFitOpts(C.Structure):
@@ -70,6 +70,7 @@ class RefConfig:
     sigma0: float = 5.0
     gain: float = 1.0
     flat: Optional[np.ndarray] = None
+    lambda_reg: float = 0.0
 
     def _c(self):
         keep = None
@@ -79,7 +80,7 @@ class RefConfig:
             assert keep.shape == (self.n_rows, self.n_cols)
             ptr = keep.ctypes.data
         c = _Config(self.n_rows, self.n_cols, self.m, self.loss, self.huber_c,
-                    self.noise, self.sigma0, self.gain, ptr)
+                    self.noise, self.sigma0, self.gain, ptr, self.lambda_reg)
         return c, keep
 
 

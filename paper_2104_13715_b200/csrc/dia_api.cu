@@ -147,6 +147,12 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
 }
 }  // namespace dia
 
+// lambda * N_data of Eq. 20 (N_data = valid-region pixels)
+static double lambda_n(const dia_handle* h) {
+  const dia_config& c = h->cfg;
+  return (double)c.lambda_reg * (double)(c.n_rows - c.m + 1) * (double)(c.n_cols - c.m + 1);
+}
+
 static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
                         const float* d_var, const float* d_theta, const int* d_done, dia::EvalParams* p,
                         dia::TensorMaps* tm) {
@@ -174,6 +180,7 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (cfg->m < 1 || cfg->m % 2 == 0) return fail(nullptr, DIA_ERR_INVALID_ARG, "m must be odd and >= 1");
   if (cfg->n_rows < cfg->m || cfg->n_cols < cfg->m) return fail(nullptr, DIA_ERR_INVALID_ARG, "image smaller than kernel");
   if (cfg->max_epochs < 1) return fail(nullptr, DIA_ERR_INVALID_ARG, "max_epochs must be >= 1");
+  if (!(cfg->lambda_reg >= 0.f)) return fail(nullptr, DIA_ERR_INVALID_ARG, "lambda_reg must be >= 0");
   if (cfg->n_refs > 1 && cfg->n_refs != cfg->max_epochs)
     return fail(nullptr, DIA_ERR_INVALID_ARG, "n_refs must be 0, 1 or max_epochs");
   if (cfg->loss != DIA_LOSS_GAUSSIAN && cfg->loss != DIA_LOSS_HUBER) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad loss");
@@ -259,6 +266,8 @@ extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I,
   const int np1 = h->np + 1;
   dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, h->stream>>>(
       h->d_partials, dia::eval_part_cols(h, n_epochs), np1, nullptr, d_loss, d_grad);
+  if (h->cfg.lambda_reg > 0.f)
+    dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, h->stream>>>(d_theta, h->cfg.m, lambda_n(h), d_loss, d_grad);
   ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
   return DIA_OK;
@@ -277,7 +286,7 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
   std::string err;
     const int unroll = 4;      // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
-  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid(h, n_epochs), dia::eval_part_cols(h, n_epochs), unroll, h->stream, &err);
+  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid(h, n_epochs), dia::eval_part_cols(h, n_epochs), unroll, h->cfg.m, lambda_n(h), h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
   return DIA_OK;
 }

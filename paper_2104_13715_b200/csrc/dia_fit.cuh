@@ -69,6 +69,8 @@ struct StepArgs {
   float* theta_out;          // caller's theta [E][np]
   dia_fit_result* result;    // caller's results [E]
   cudaGraphConditionalHandle cond;
+  int m;                     // kernel size
+  double lamN;               // lambda * N_data of Eq. 20, 0 = no penalty
 };
 
 // ---------------------------------------------------------------- block-wide FP64 reductions
@@ -101,6 +103,35 @@ __device__ __forceinline__ double block_max(double v, BlockRed& br) {
 #pragma unroll
   for (int w = 0; w < kFitThreads / 32; ++w) { double u = row[w]; s = (u > s || u != u) ? u : s; }
   return s;
+}
+
+// (L x)_k for the graph Laplacian of the m x m kernel grid (Eq. 21; 4 edge neighbours)
+__device__ __forceinline__ double laplacian_row(const double* __restrict__ x, int m, int k) {
+  const int a = k / m, b = k - a * m;
+  int nadj = 0;
+  double s = 0.0;
+  if (a > 0)     { ++nadj; s += x[k - m]; }
+  if (a < m - 1) { ++nadj; s += x[k + m]; }
+  if (b > 0)     { ++nadj; s += x[k - 1]; }
+  if (b < m - 1) { ++nadj; s += x[k + 1]; }
+  return nadj * x[k] - s;
+}
+
+// Eq. 20: adds lamN |L theta|^2 to loss[e] and 2 lamN L (L theta) to grad[e][0..m*m) for the
+// stand-alone evaluation path (one CTA per epoch, launched after reduce_partials_kernel).
+__global__ void __launch_bounds__(kFitThreads) penalty_kernel(const float* __restrict__ theta, int m, double lamN,
+                                                              double* __restrict__ loss, double* __restrict__ grad) {
+  __shared__ double xs[kFitThreads * kMaxPerThread], us[kFitThreads * kMaxPerThread];
+  __shared__ double sh_rows[2][kFitThreads / 32];
+  BlockRed br{sh_rows, 0};
+  const int e = blockIdx.x, nk = m * m, np = nk + 1, tid = threadIdx.x;
+  for (int k = tid; k < nk; k += kFitThreads) xs[k] = (double)theta[(size_t)e * np + k];
+  __syncthreads();
+  double pen = 0.0;
+  for (int k = tid; k < nk; k += kFitThreads) { const double u = laplacian_row(xs, m, k); us[k] = u; pen += u * u; }
+  pen = block_sum(pen, br);                    // the barrier inside also publishes us[]
+  for (int k = tid; k < nk; k += kFitThreads) grad[(size_t)e * np + k] += 2.0 * lamN * laplacian_row(us, m, k);
+  if (tid == 0) loss[e] += lamN * pen;
 }
 
 __global__ void fit_init_kernel(FitBuffers b, const float* __restrict__ theta_in, int np, int n_epochs) {
@@ -173,6 +204,20 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     }
     Ln = gsum[np];                               // loss lives in row np
     __syncthreads();
+  }
+  if (a.lamN > 0.0) {                            // Eq. 20 penalty at the evaluation point (uniform branch)
+    __shared__ double xs[kFitThreads * kMaxPerThread], us[kFitThreads * kMaxPerThread];
+    for (int k = tid; k < nk; k += kFitThreads) xs[k] = (double)th32[k];
+    __syncthreads();
+    double pen = 0.0;
+    for (int k = tid; k < nk; k += kFitThreads) { const double u = laplacian_row(xs, a.m, k); us[k] = u; pen += u * u; }
+    pen = block_sum(pen, sh);
+#pragma unroll
+    for (int q = 0; q < kMaxPerThread; ++q) {
+      const int k = tid + q * kFitThreads;
+      if (k < nk) gn[q] += 2.0 * a.lamN * laplacian_row(us, a.m, k);
+    }
+    Ln += a.lamN * pen;
   }
   st.n_evals += 1;
   bool finished = false;
@@ -400,12 +445,13 @@ inline void fit_workspace_destroy(FitWorkspace* w) {
 inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, const TensorMaps& tm,
                    const dia_fit_opts& o,
                    int n_epochs, float* d_theta, dia_fit_result* d_result, int grid, int part_cols, int unroll,
+                   int m, double lamN,
                    cudaStream_t stream, std::string* err) {
   unsigned char key[256];
   int len = 0;
   auto put = [&](const void* src, size_t n) { std::memcpy(key + len, src, n); len += (int)n; };
   put(&n_epochs, sizeof(int)); put(&p.I, sizeof(void*)); put(&p.mask, sizeof(void*)); put(&p.var, sizeof(void*));
-  put(&d_theta, sizeof(void*)); put(&d_result, sizeof(void*)); put(&o, sizeof(o)); put(&unroll, sizeof(int));
+  put(&d_theta, sizeof(void*)); put(&d_result, sizeof(void*)); put(&o, sizeof(o)); put(&unroll, sizeof(int)); put(&lamN, sizeof(double));
   if (!(w->exec && len == w->key_len && std::memcmp(key, w->key, len) == 0)) {
     if (w->exec) { cudaGraphExecDestroy(w->exec); w->exec = nullptr; }
     if (w->graph) { cudaGraphDestroy(w->graph); w->graph = nullptr; }
@@ -438,6 +484,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     StepArgs sa;
     sa.b = w->b; sa.partials = p.partials; sa.n_blocks = part_cols; sa.np = w->np; sa.hist_cap = w->hist_cap;
     sa.o = o; sa.theta_out = d_theta; sa.result = d_result; sa.cond = cond;
+    sa.m = m; sa.lamN = lamN;
     void* step_args[] = {(void*)&sa};
     cudaKernelNodeParams ks = {};
     ks.func = (void*)fit_step_kernel; ks.gridDim = dim3(n_epochs); ks.blockDim = dim3(kFitThreads);

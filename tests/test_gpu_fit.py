@@ -190,6 +190,32 @@ def test_fit_many_small_pairs(dia):
     h.close()
 
 
+def test_fit_with_laplacian_regularisation(dia):
+    """Eq. 20 inside dia_fit.  The penalty lifts the flat directions of K, so even the free-running
+    fit under the paper's stop rule is now well determined; lock-step first (strict), then free-running."""
+    w = make_workload(0)
+    lam = 10.0
+    cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
+    h = dia.Handle(_dev(w.R), w.m, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
+    og, oo = _both_opts(dia, force_adam_iters=30, force_lbfgs_iters=10)
+    tho, ro = oracle.fit(cfg, w.R, w.I, w.theta0, oo)
+    thg, rg = h.fit(_dev(w.I), _dev(w.theta0), og)
+    _assert_fit_close(tho, ro, thg.cpu().numpy(), rg, "lambda lockstep")
+    og, oo = _both_opts(dia)
+    tho, ro = oracle.fit(cfg, w.R, w.I, w.theta0, oo)
+    thg, rg = h.fit(_dev(w.I), _dev(w.theta0), og)
+    thg = thg.cpu().numpy()
+    d = _diffs(tho, ro, thg, rg, 0)
+    _report("lambda free", 0, d, ro, rg)
+    assert d[3] <= 1e-5 and d[0] <= 1e-4 and d[1] <= 1e-4 and d[2] <= 1e-4      # strict, free-running
+    # the penalised loss is larger than the plain one at the same theta, and the fitted kernel is smoother
+    cfg0 = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+    L_pen, _ = oracle.eval_loss_grad(cfg, w.R, w.I, thg[0])
+    L_0, _ = oracle.eval_loss_grad(cfg0, w.R, w.I, thg[0])
+    assert L_pen[0] > L_0[0] and rg[0].loss == pytest.approx(L_pen[0], rel=1e-6)
+    h.close()
+
+
 def test_fit_huber_with_cosmic_rays(dia):
     """BASELINE config 2 shape at reduced size: robust objective, 0.1 % cosmic-ray hits, no mask."""
     w = make_workload(2, n=200, m=9)

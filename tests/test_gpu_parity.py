@@ -182,6 +182,22 @@ def test_many_small_pairs_one_reference_each(dia):
     h.close()
 
 
+@pytest.mark.parametrize("c,n,m,lam", [(0, None, None, 1.0), (4, 300, 19, 0.1), (2, 200, 9, 100.0)])
+def test_laplacian_regularisation_eq20(dia, c, n, m, lam):
+    """Eq. 20-21: L0 + lambda N_data theta' L' L theta, evaluated on the device."""
+    w = make_workload(c, n=n, m=m, n_epochs=2 if c == 4 else None)
+    h = _handle(dia, w, lambda_reg=lam)
+    cfg = _ref_cfg(w, lambda_reg=lam)
+    cfg0 = _ref_cfg(w)
+    for name, th, kind in _points(w)[:2]:
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=w.mask, want_scale=True)
+        L0, _ = oracle.eval_loss_grad(cfg0, w.R, w.I, th, mask=w.mask)
+        assert np.all(Lo > L0) if name == "P1" else np.all(Lo >= L0)   # flat theta_init has zero Laplacian
+        Lg, gg = h.eval_loss_grad(_dev(w.I), _dev(th), mask=_dev(w.mask))
+        _compare(Lg, gg, Lo, go, So, kind, f"lambda={lam} c{c} {name}")
+    h.close()
+
+
 def test_emccd_noise_model_eq7(dia):
     """EMCCD noise model, Eq. 7: sigma^2 = E M / (G_total F) with E = 2, G_total = 25.8/300
     e-/ADU -- the affine form of Eq. 6 with no read-noise term, i.e. sigma0 = 0 and gain = G_total / E."""

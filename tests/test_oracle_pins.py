@@ -222,3 +222,43 @@ def test_huber_Q_constant(golden):
     assert oracle.huber_Q(c, 1.0) == pytest.approx(math.log(integral), rel=1e-10)
     assert oracle.huber_Q(c, 7.0) == pytest.approx(7.0 * math.log(integral), rel=1e-10)
     assert oracle.huber_Q(50.0, 10.0) == pytest.approx(5.0 * math.log(2 * math.pi), rel=1e-12)
+
+
+# ---------------------------------------------------------------- Laplacian regularisation, Eq. 20-21
+def _laplacian_matrix(m):
+    """Eq. 21 written out: (N_K+1) x (N_K+1), L_uu = number of adjacent kernel pixels,
+    L_uv = -1 for adjacent kernel pixels (4 edge neighbours, reading R14), zero row / column for B0."""
+    nk = m * m
+    L = np.zeros((nk + 1, nk + 1))
+    for a in range(m):
+        for b in range(m):
+            u = a * m + b
+            for da, db in ((-1, 0), (1, 0), (0, -1), (0, 1)):
+                aa, bb = a + da, b + db
+                if 0 <= aa < m and 0 <= bb < m:
+                    L[u, u] += 1
+                    L[u, aa * m + bb] = -1
+    return L
+
+
+def test_laplacian_penalty_matches_eq20_matrix_form():
+    """Eq. 20: L = L0 + lambda N_data theta' L' L theta.  The oracle applies the stencil; the
+    expected value is the explicit matrix product.  Catches a wrong neighbour count at the kernel border, a
+    penalty on B0, a missing factor 2 in the gradient and a wrong N_data."""
+    n, m, lam = 13, 5, 0.7
+    R, I, th = _rand_problem(n, m, seed=4)
+    c0 = _cfg(n, m, sigma0=5.0)
+    c1 = _cfg(n, m, sigma0=5.0, lambda_reg=lam)
+    L0, g0 = oracle.eval_loss_grad(c0, R, I, th)
+    L1, g1 = oracle.eval_loss_grad(c1, R, I, th)
+    Lm = _laplacian_matrix(m)
+    assert np.array_equal(Lm, Lm.T) and np.linalg.eigvalsh(Lm).min() > -1e-12        # symmetric, PSD (PAPER.md:216)
+    t = th.astype(np.float64)
+    N = n_valid(n, m)
+    pen = lam * N * t @ Lm.T @ Lm @ t
+    assert L1[0] - L0[0] == pytest.approx(pen, rel=1e-10)
+    assert np.allclose(g1[0] - g0[0], 2 * lam * N * (Lm.T @ Lm @ t), rtol=1e-9, atol=1e-12 * np.abs(g1).max())
+    assert g1[0][-1] == g0[0][-1]                                                     # B0 is not penalised
+    # a flat kernel has zero Laplacian everywhere, border included
+    flat = np.concatenate([np.full(m * m, 0.125), [1.0]]).astype(np.float32)
+    assert oracle.eval_loss_grad(c1, R, I, flat)[0][0] == oracle.eval_loss_grad(c0, R, I, flat)[0][0]
