@@ -44,6 +44,7 @@ enum { DIA_FIT_CONVERGED_GRAD = 0, DIA_FIT_CONVERGED_CHANGE = 1, DIA_FIT_MAX_ITE
        DIA_FIT_NONFINITE = 3 };
 
 #define DIA_MAX_KERNEL_SIZE 31            /* m odd, 1 <= m <= 31 in this build */
+#define DIA_MAX_BG_DEGREE 3               /* polynomial background degree d <= 3 in this build */
 
 typedef struct {
   int n_rows, n_cols, m;          /* m odd, 1 <= m <= min(n_rows, n_cols, DIA_MAX_KERNEL_SIZE) */
@@ -59,6 +60,11 @@ typedef struct {
   float lambda_reg;               /* Eq. 20: adds lambda N_data theta' L' L theta to the objective, L the
                                      graph Laplacian of the kernel pixels (Eq. 21; 4 edge neighbours, B0 not penalised,
                                      N_data = valid-region pixels); 0 = off (the paper's own experiments) */
+  int bg_degree;                  /* Eq. 18-19: degree d of the polynomial background
+                                     B(x,y) = sum_{m=0..d} sum_{n=0..d-m} b_mn eta^m xi^n, eta = (x - x_c)/N_x,
+                                     xi = (y - y_c)/N_y, x = column, y = row, centre ((N-1)/2); 0 = scalar B0.
+                                     theta then holds (d+1)(d+2)/2 coefficients after K, b_00 first (m outer, n inner),
+                                     all stepped with lr_b0; every [m*m+1] below reads [m*m + (d+1)(d+2)/2] */
 } dia_config;
 
 typedef struct {                  /* PAPER.md:242-244 unless marked [reading] */

@@ -30,18 +30,43 @@ static int check_cfg(const dia_ref_config* c) {
   if (c->noise != DIA_REF_NOISE_MODEL && c->noise != DIA_REF_NOISE_FIXED) return 0;
   if (c->noise == DIA_REF_NOISE_MODEL && !(c->gain > 0.0 && c->sigma0 >= 0.0)) return 0;
   if (c->loss == DIA_REF_LOSS_HUBER && !(c->huber_c > 0.0)) return 0;
+  if (c->bg_degree < 0 || c->bg_degree > 4) return 0;
   return 1;
+}
+
+int dia_ref_num_params(const dia_ref_config* cfg) {
+  const int d = cfg->bg_degree > 0 ? cfg->bg_degree : 0;
+  return cfg->m * cfg->m + (d + 1) * (d + 2) / 2;
+}
+
+/* Eq. 18-19: B(x, y) = sum_{m=0..d} sum_{n=0..d-m} b_mn eta^m xi^n with the normalised
+ * coordinates eta = (x - x_c)/N_x, xi = (y - y_c)/N_y.  Readings (R18): x = column index j, y = row
+ * index i, centre (x_c, y_c) = ((n_cols-1)/2, (n_rows-1)/2).  basis (nullable) receives eta^m xi^n in the
+ * coefficient order, which is also dB/db_mn. */
+static double background(const dia_ref_config* cfg, const float* b, int i, int j, double* basis) {
+  const int d = cfg->bg_degree > 0 ? cfg->bg_degree : 0;
+  const double eta = ((double)j - 0.5 * (cfg->n_cols - 1)) / (double)cfg->n_cols;
+  const double xi = ((double)i - 0.5 * (cfg->n_rows - 1)) / (double)cfg->n_rows;
+  double B = 0.0;
+  int t = 0;
+  for (int mm = 0; mm <= d; ++mm)
+    for (int nn = 0; nn <= d - mm; ++nn, ++t) {
+      const double f = pow(eta, mm) * pow(xi, nn);
+      if (basis) basis[t] = f;
+      B += (double)b[t] * f;
+    }
+  return B;
 }
 
 /* Eq. 2: M_ij = sum_lm K_lm R_(i+l)(j+m) + B0, cross-correlation, no flip
  * (reading R2).  (i, j) are image coordinates of a valid pixel. */
-static double model_pixel(const float* R, int n_cols, int m, const float* theta, int i, int j) {
+static double model_pixel(const dia_ref_config* cfg, const float* R, int n_cols, int m, const float* theta, int i, int j) {
   const int h = (m - 1) / 2;
   double M = 0.0;
   for (int a = 0; a < m; ++a)
     for (int b = 0; b < m; ++b)
       M += (double)theta[a * m + b] * (double)R[(size_t)(i - h + a) * n_cols + (j - h + b)];
-  return M + (double)theta[m * m];
+  return M + background(cfg, theta + m * m, i, j, NULL);     /* B0, or Eq. 18 */
 }
 
 int dia_ref_model(const dia_ref_config* cfg, const float* R, const float* theta, double* M) {
@@ -51,7 +76,7 @@ int dia_ref_model(const dia_ref_config* cfg, const float* R, const float* theta,
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < vr; ++i)
     for (int j = 0; j < vc; ++j)
-      M[(size_t)i * vc + j] = model_pixel(R, cfg->n_cols, m, theta, i + h, j + h);
+      M[(size_t)i * vc + j] = model_pixel(cfg, R, cfg->n_cols, m, theta, i + h, j + h);
   return DIA_REF_OK;
 }
 
@@ -59,7 +84,7 @@ int dia_ref_model(const dia_ref_config* cfg, const float* R, const float* theta,
 static void eval_one(const dia_ref_config* cfg, const float* R, const float* I,
                      const unsigned char* mask, const float* var, const float* theta,
                      double* loss_out, double* grad, double* gscale) {
-  const int m = cfg->m, h = (m - 1) / 2, np = m * m + 1;
+  const int m = cfg->m, h = (m - 1) / 2, np = dia_ref_num_params(cfg), nbg = np - m * m;
   const int nr = cfg->n_rows, nc = cfg->n_cols;
   int nthreads = dia_ref_num_threads();
   double* tl = (double*)calloc((size_t)nthreads, sizeof(double));
@@ -81,7 +106,7 @@ static void eval_one(const dia_ref_config* cfg, const float* R, const float* I,
       for (int j = h; j < nc - h; ++j) {
         const size_t p = (size_t)i * nc + j;
         if (mask && mask[p] == 0) continue;                 /* reading R4 */
-        const double M = model_pixel(R, nc, m, theta, i, j);
+        const double M = model_pixel(cfg, R, nc, m, theta, i, j);
         double v, bp;
         if (cfg->noise == DIA_REF_NOISE_MODEL) {
           /* Eq. 6: sigma^2 = sigma0^2/F^2 + M/(G F); reading R1: photon
@@ -120,8 +145,12 @@ static void eval_one(const dia_ref_config* cfg, const float* R, const float* I,
             g[a * m + b] += w * x;
             s[a * m + b] += aw * fabs(x);
           }
-        g[m * m] += w;
-        s[m * m] += aw;
+        double basis[16];
+        background(cfg, theta + m * m, i, j, basis);          /* dM/db_mn = eta^m xi^n (1 for B0) */
+        for (int t = 0; t < nbg; ++t) {
+          g[m * m + t] += w * basis[t];
+          s[m * m + t] += aw * fabs(basis[t]);
+        }
       }
     }
     tl[tid] = L;
@@ -180,7 +209,7 @@ int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epoc
     return DIA_REF_ERR_INVALID_ARG;
   if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
   const size_t npix = (size_t)cfg->n_rows * cfg->n_cols;
-  const int np = cfg->m * cfg->m + 1;
+  const int np = dia_ref_num_params(cfg);
   for (int e = 0; e < n_epochs; ++e) {
     eval_one(cfg, R, I + e * npix, mask ? mask + e * npix : NULL, var ? var + e * npix : NULL,
              theta + (size_t)e * np, loss + e, grad + (size_t)e * np,

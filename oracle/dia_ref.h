@@ -36,6 +36,8 @@ typedef struct {
   int noise;   double sigma0, gain;     /* Eq. 6 parameters */
   const float* flat;                    /* [n_rows][n_cols] or NULL => F == 1 */
   double lambda_reg;                    /* Eq. 20: lambda of the Laplacian penalty, 0 = off */
+  int bg_degree;                        /* Eq. 18: degree d of the polynomial background, 0 = scalar B0.
+                                           theta = [K (m*m), b_mn for m = 0..d, n = 0..d-m]; (d+1)(d+2)/2 coefficients */
 } dia_ref_config;
 
 typedef struct {                        /* PAPER.md:242-244; [reading] marks DESIGN.md readings */
@@ -56,6 +58,9 @@ typedef struct {
 } dia_ref_fit_result;
 
 void dia_ref_default_fit_opts(dia_ref_fit_opts* o);
+
+/* Number of parameters per epoch: m*m + (d+1)(d+2)/2. */
+int dia_ref_num_params(const dia_ref_config* cfg);
 
 /* Model image of Eq. 2 on the valid region: M [n_rows-m+1][n_cols-m+1] (FP64). */
 int dia_ref_model(const dia_ref_config* cfg, const float* R, const float* theta, double* M);

@@ -18,7 +18,7 @@ class _Config(C.Structure):
     _fields_ = [("n_rows", C.c_int), ("n_cols", C.c_int), ("m", C.c_int),
                 ("loss", C.c_int), ("huber_c", C.c_double),
                 ("noise", C.c_int), ("sigma0", C.c_double), ("gain", C.c_double),
-                ("flat", C.c_void_p), ("lambda_reg", C.c_double)]
+                ("flat", C.c_void_p), ("lambda_reg", C.c_double), ("bg_degree", C.c_int)]
 
 
 class RefFitOpts(C.Structure):
@@ -71,6 +71,12 @@ class RefConfig:
     gain: float = 1.0
     flat: Optional[np.ndarray] = None
     lambda_reg: float = 0.0
+    bg_degree: int = 0
+
+    @property
+    def n_params(self) -> int:
+        d = self.bg_degree
+        return self.m * self.m + (d + 1) * (d + 2) // 2
 
     def _c(self):
         keep = None
@@ -80,7 +86,7 @@ class RefConfig:
             assert keep.shape == (self.n_rows, self.n_cols)
             ptr = keep.ctypes.data
         c = _Config(self.n_rows, self.n_cols, self.m, self.loss, self.huber_c,
-                    self.noise, self.sigma0, self.gain, ptr, self.lambda_reg)
+                    self.noise, self.sigma0, self.gain, ptr, self.lambda_reg, self.bg_degree)
         return c, keep
 
 
@@ -103,7 +109,7 @@ def _epochs(cfg: RefConfig, I, mask, var, theta):
         I = I[None]
     E = I.shape[0]
     assert I.shape[1:] == (cfg.n_rows, cfg.n_cols)
-    theta = _f32(theta).reshape(E, cfg.m * cfg.m + 1)
+    theta = _f32(theta).reshape(E, cfg.n_params)
     mask = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8).reshape(I.shape)
     var = None if var is None else _f32(var).reshape(I.shape)
     return E, I, mask, var, theta
@@ -123,7 +129,7 @@ def eval_loss_grad(cfg: RefConfig, R, I, theta, mask=None, var=None, want_scale=
     c, keep = cfg._c()
     R = _f32(R)
     E, I, mask, var, theta = _epochs(cfg, I, mask, var, theta)
-    npar = cfg.m * cfg.m + 1
+    npar = cfg.n_params
     loss = np.empty(E, dtype=np.float64)
     grad = np.empty((E, npar), dtype=np.float64)
     scale = np.empty((E, npar), dtype=np.float64) if want_scale else None

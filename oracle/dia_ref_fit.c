@@ -49,7 +49,7 @@ static double dot(const double* a, const double* b, int n) {
 }
 
 static int fit_one(objective* ob, const dia_ref_fit_opts* o, float* theta_io, dia_ref_fit_result* res) {
-  const int np = ob->np, nk = np - 1;
+  const int np = ob->np, nk = ob->cfg->m * ob->cfg->m;
   const int hist = o->lbfgs_history > 0 ? o->lbfgs_history : 1;
   double* th = (double*)malloc(sizeof(double) * np);
   double* g = (double*)malloc(sizeof(double) * np);
@@ -187,7 +187,7 @@ int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opt
   if (cfg->m < 1 || cfg->m % 2 == 0) return DIA_REF_ERR_INVALID_ARG;
   if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
   const size_t npix = (size_t)cfg->n_rows * cfg->n_cols;
-  const int np = cfg->m * cfg->m + 1;
+  const int np = dia_ref_num_params(cfg);
   float* th32 = (float*)malloc(sizeof(float) * np);
   if (!th32) return DIA_REF_ERR_ALLOC;
   int rc = DIA_REF_OK;

@@ -30,7 +30,7 @@ class _Config(C.Structure):
     _fields_ = [("n_rows", C.c_int), ("n_cols", C.c_int), ("m", C.c_int), ("max_epochs", C.c_int),
                 ("loss", C.c_int), ("huber_c", C.c_float),
                 ("noise", C.c_int), ("sigma0", C.c_float), ("gain", C.c_float),
-                ("d_flat", C.c_void_p), ("stream", C.c_void_p), ("n_refs", C.c_int), ("lambda_reg", C.c_float)]
+                ("d_flat", C.c_void_p), ("stream", C.c_void_p), ("n_refs", C.c_int), ("lambda_reg", C.c_float), ("bg_degree", C.c_int)]
 
 
 class FitOpts(C.Structure):
@@ -114,11 +114,12 @@ def _check(rc: int, handle=None):
 def dia_create(n_rows: int, n_cols: int, m: int, d_R: torch.Tensor, *, max_epochs: int = 1,
                loss: int = LOSS_GAUSSIAN, huber_c: float = 1.345, noise: int = NOISE_MODEL,
                sigma0: float = 0.0, gain: float = 1.0, d_flat: Optional[torch.Tensor] = None,
-               stream: Optional[torch.cuda.Stream] = None, n_refs: int = 1, lambda_reg: float = 0.0) -> int:
+               stream: Optional[torch.cuda.Stream] = None, n_refs: int = 1, lambda_reg: float = 0.0,
+               bg_degree: int = 0) -> int:
     lib = load_library()
     cfg = _Config(n_rows, n_cols, m, max_epochs, loss, huber_c, noise, sigma0, gain,
                   None if d_flat is None else _dptr(d_flat, torch.float32, "d_flat").value,
-                  None if stream is None else stream.cuda_stream, n_refs, lambda_reg)
+                  None if stream is None else stream.cuda_stream, n_refs, lambda_reg, bg_degree)
     want = (n_rows, n_cols) if n_refs <= 1 else (n_refs, n_rows, n_cols)
     if d_R is not None and tuple(d_R.shape) != want:
         raise DiaError("d_R has the wrong shape")
@@ -164,7 +165,7 @@ class Handle:
     def __init__(self, R: torch.Tensor, m: int, *, max_epochs: int = 1, loss: int = LOSS_GAUSSIAN,
                  huber_c: float = 1.345, noise: int = NOISE_MODEL, sigma0: float = 0.0, gain: float = 1.0,
                  flat: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None,
-                 lambda_reg: float = 0.0):
+                 lambda_reg: float = 0.0, bg_degree: int = 0):
         """R [n_rows][n_cols]: one reference shared by all epochs; R [max_epochs][n_rows][n_cols] (3-D): one
         reference per epoch (many independent image pairs fitted together)."""
         self.R, self.flat, self.m, self.max_epochs = R, flat, m, max_epochs
@@ -174,11 +175,11 @@ class Handle:
             if self.n_refs != max_epochs:
                 raise DiaError("a 3-D reference stack needs max_epochs == R.shape[0]")
         self.n_rows, self.n_cols = R.shape[-2:]
-        self.np = m * m + 1
+        self.np = m * m + (bg_degree + 1) * (bg_degree + 2) // 2
         self.stream = stream
         self._h = dia_create(self.n_rows, self.n_cols, m, R, max_epochs=max_epochs, loss=loss,
                              huber_c=huber_c, noise=noise, sigma0=sigma0, gain=gain, d_flat=flat,
-                             stream=stream, n_refs=self.n_refs, lambda_reg=lambda_reg)
+                             stream=stream, n_refs=self.n_refs, lambda_reg=lambda_reg, bg_degree=bg_degree)
 
     @property
     def raw(self) -> int:

@@ -160,6 +160,9 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
   p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
   p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;  p->n_refs = h->n_refs;
+  p->np = h->np;  p->bg_degree = c.bg_degree;            // Eq. 19: centre ((N-1)/2), normalisation N (R18)
+  p->bg_xc = 0.5f * (float)(c.n_cols - 1);  p->bg_yc = 0.5f * (float)(c.n_rows - 1);
+  p->bg_inv_nx = 1.0f / (float)c.n_cols;  p->bg_inv_ny = 1.0f / (float)c.n_rows;
   p->tiles_x = (c.n_cols - c.m + 1 + dia::kTW - 1) / dia::kTW;
   p->tiles_y = (c.n_rows - c.m + 1 + dia::kTH - 1) / dia::kTH;
   p->loss_kind = c.loss;  p->noise_kind = c.noise;
@@ -181,6 +184,8 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (cfg->n_rows < cfg->m || cfg->n_cols < cfg->m) return fail(nullptr, DIA_ERR_INVALID_ARG, "image smaller than kernel");
   if (cfg->max_epochs < 1) return fail(nullptr, DIA_ERR_INVALID_ARG, "max_epochs must be >= 1");
   if (!(cfg->lambda_reg >= 0.f)) return fail(nullptr, DIA_ERR_INVALID_ARG, "lambda_reg must be >= 0");
+  if (cfg->bg_degree < 0) return fail(nullptr, DIA_ERR_INVALID_ARG, "bg_degree must be >= 0");
+  if (cfg->bg_degree > DIA_MAX_BG_DEGREE) return fail(nullptr, DIA_ERR_UNSUPPORTED, "bg_degree exceeds DIA_MAX_BG_DEGREE");
   if (cfg->n_refs > 1 && cfg->n_refs != cfg->max_epochs)
     return fail(nullptr, DIA_ERR_INVALID_ARG, "n_refs must be 0, 1 or max_epochs");
   if (cfg->loss != DIA_LOSS_GAUSSIAN && cfg->loss != DIA_LOSS_HUBER) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad loss");
@@ -200,7 +205,7 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (!h) return fail(nullptr, DIA_ERR_ALLOC, "host allocation failed");
   h->n_refs = cfg->n_refs > 1 ? cfg->n_refs : 1;
   h->cfg = *cfg;  h->d_R = d_R;  h->stream = (cudaStream_t)cfg->stream;  h->sms = sms;
-  h->np = cfg->m * cfg->m + 1;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
+  h->np = cfg->m * cfg->m + (cfg->bg_degree + 1) * (cfg->bg_degree + 2) / 2;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
 
   int occ = 0;
   for (int aux = 0; aux < 2; ++aux) {
@@ -267,7 +272,7 @@ extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I,
   dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, h->stream>>>(
       h->d_partials, dia::eval_part_cols(h, n_epochs), np1, nullptr, d_loss, d_grad);
   if (h->cfg.lambda_reg > 0.f)
-    dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, h->stream>>>(d_theta, h->cfg.m, lambda_n(h), d_loss, d_grad);
+    dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, h->stream>>>(d_theta, h->cfg.m, h->np, lambda_n(h), d_loss, d_grad);
   ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
   return DIA_OK;

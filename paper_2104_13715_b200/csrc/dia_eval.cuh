@@ -28,6 +28,7 @@ constexpr int kP = 16;                // forward strip / gradient chunk length (
 constexpr int kIPitch = 68;           // I/w tile pitch (floats); 68/4 = 17 is odd => conflict-free rows
 constexpr int kFlushTiles = 32;       // FP32 gradient strips are folded into FP64 at least this often
 constexpr int kSmemBudget = 113 * 1024;   // per CTA, two CTAs per SM
+constexpr int kMaxBg = 16;            // background coefficients held per epoch (degree <= 3 uses 10)
 
 __host__ __device__ constexpr int round_up(int x, int q) { return (x + q - 1) / q * q; }
 
@@ -35,7 +36,6 @@ template <int M>
 struct Geo {
   static constexpr int H = (M - 1) / 2;
   static constexpr int IOFF = H % 4;                         // column shift of the staged I tile
-  static constexpr int NP = M * M + 1;                       // parameters per epoch
   static constexpr int RH = kTH + M - 1;                     // staged R rows
   static constexpr int RSEG = round_up(kP + M - 1, 4);       // floats a thread loads per R row
   static constexpr int RMIN = kTW - kP + RSEG;               // columns touched
@@ -49,7 +49,7 @@ struct Geo {
   static constexpr int ACC_FLOATS = kThreads * KP;           // thread-private FP32 gradient strips
   static constexpr int R_BYTES = R_FLOATS * 4, I_BYTES = I_FLOATS * 4;
   static constexpr int R_STRIDE = round_up(R_BYTES, 128);    // TMA destinations are 128-byte aligned
-  static constexpr int FIXED_BYTES = 4 * (2 * I_FLOATS + K_FLOATS + ACC_FLOATS) + 1024;
+  static constexpr int FIXED_BYTES = 4 * (2 * I_FLOATS + K_FLOATS + ACC_FLOATS) + 2560;
   // two R buffers when they fit next to a second resident CTA, else one (the copy of the next R
   // tile then waits for the gradient phase to finish)
   static constexpr int NRBUF = (FIXED_BYTES + 2 * R_STRIDE <= kSmemBudget) ? 2 : 1;
@@ -60,8 +60,10 @@ struct Geo {
   static constexpr int OFF_W = OFF_I + I_STRIDE;
   static constexpr int OFF_ACC = OFF_W + I_STRIDE;
   static constexpr int OFF_K = OFF_ACC + 4 * ACC_FLOATS;
-  static constexpr int OFF_BAR = round_up(OFF_K + 4 * K_FLOATS, 16);
-  static constexpr size_t SMEM = OFF_BAR + 64 + 128 + 128;   // mbarriers, FP64 scratch, alignment slack
+  static constexpr int OFF_BG = OFF_K + 4 * K_FLOATS;        // background coefficients b_mn (Eq. 18)
+  static constexpr int OFF_BAR = round_up(OFF_BG + 4 * kMaxBg, 16);
+  static constexpr int OFF_BGACC = OFF_BAR + 64 + 128;       // FP64 background-gradient sums, one row per warp
+  static constexpr size_t SMEM = OFF_BGACC + 8 * (kThreads / 32) * kMaxBg + 128;   // + alignment slack
   static_assert(RPITCH % 8 == 4, "pitch");
   static_assert(R_BYTES % 16 == 0 && I_BYTES % 16 == 0, "TMA sizes");
   static_assert(RPITCH <= 256 && RH <= 256, "TMA box limits");
@@ -73,12 +75,14 @@ struct EvalParams {
   const unsigned char* mask; // [E][n_rows][n_cols] or null
   const float* var;          // [E][n_rows][n_cols] or null (FIXED noise)
   const float* flat;         // [n_rows][n_cols] or null
-  const float* theta;        // [E][NP] float32
+  const float* theta;        // [E][np] float32: K row-major, then the background coefficients
   const int* done;           // [E] or null: epochs with done != 0 are skipped
   double* partials;          // [E][NP+1][ncols], ncols = min(tiles, gridDim.x): rows g_K (M*M), g_B0, loss;
                              // one column per CTA that owns tiles of the epoch
   int n_rows, n_cols, n_epochs;
   int n_refs;                // 1: one reference shared by all epochs; else one reference per epoch
+  int np, bg_degree;         // parameters per epoch = M*M + (d+1)(d+2)/2; degree d of the background (Eq. 18)
+  float bg_xc, bg_yc, bg_inv_nx, bg_inv_ny;   // Eq. 19: eta = (x - xc) / N_x, xi = (y - yc) / N_y
   int tiles_x, tiles_y;
   int loss_kind, noise_kind;
   float huber_c, sigma0_sq, inv_gain;
@@ -322,11 +326,14 @@ __device__ __forceinline__ void forward_strip(const float* __restrict__ Ks, cons
   for (int q = 0; q < kP; ++q) tot[q] += rs[q];
 }
 
-// epilogue of the forward phase for one strip: loss terms and the w strip
+// epilogue of the forward phase for one strip: loss terms and the w strip.  With a polynomial background
+// (Eq. 18-19) the terms beyond b_00 are added to the model here, and the sums
+// S_p = sum_q w_q eta_q^p (p = 0..d) of the strip are returned for the background gradient.
 template <int M, bool AUX, bool EDGE>
 __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_t npix, int iy, int ix0, int vr, int vc,
-                                               const float (&tot)[kP], const float* __restrict__ irow,
-                                               float* __restrict__ wrow, float& lsum, float& wsum) {
+                                               float (&tot)[kP], const float* __restrict__ irow,
+                                               float* __restrict__ wrow, const float* __restrict__ Bs, float& lsum,
+                                               float& wsum, float (&Sp)[4]) {
   using G = Geo<M>;
   float iv[kP];
   if (G::IOFF == 0) {
@@ -339,16 +346,47 @@ __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_
 #pragma unroll
     for (int q = 0; q < kP; ++q) iv[q] = irow[q + G::IOFF];
   }
+  const int d = p.bg_degree;
+  const float eta0 = ((float)(ix0 + G::H) - p.bg_xc) * p.bg_inv_nx;
+  if (d > 0) {                                       // CTA-uniform
+    const float xi = ((float)(iy + G::H) - p.bg_yc) * p.bg_inv_ny;
+    float c[4] = {0.f, 0.f, 0.f, 0.f};               // c_p(xi) = sum_n b_pn xi^n, without b_00
+    int t = 0;
+#pragma unroll
+    for (int mm = 0; mm < 4; ++mm) {
+      float xn = 1.f;
+#pragma unroll
+      for (int nn = 0; nn < 4; ++nn) {
+        if (mm <= d && nn <= d - mm) {
+          if (t > 0) c[mm] = fmaf(Bs[t], xn, c[mm]);
+          ++t;
+        }
+        xn *= xi;
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < kP; ++q) {
+      const float eta = fmaf((float)q, p.bg_inv_nx, eta0);
+      tot[q] += fmaf(fmaf(fmaf(c[3], eta, c[2]), eta, c[1]), eta, c[0]);
+    }
+  }
   const size_t gbase = (size_t)(iy + G::H) * p.n_cols + (ix0 + G::H);
   lsum = 0.f; wsum = 0.f;
+  Sp[1] = 0.f; Sp[2] = 0.f; Sp[3] = 0.f;
 #pragma unroll
   for (int q = 0; q < kP; ++q) {
     float li, wi;
     pixel_terms<AUX, EDGE>(p, e, npix, gbase + q, (iy < vr) && (ix0 + q < vc), tot[q], iv[q], li, wi);
     lsum += li;
     wsum += wi;
+    if (d > 0) {
+      const float eta = fmaf((float)q, p.bg_inv_nx, eta0);
+      const float w1 = wi * eta, w2 = w1 * eta;
+      Sp[1] += w1; Sp[2] += w2; Sp[3] = fmaf(w2, eta, Sp[3]);
+    }
     iv[q] = wi;
   }
+  Sp[0] = wsum;
 #pragma unroll
   for (int q = 0; q < kP / 4; ++q)
     reinterpret_cast<float4*>(wrow)[q] = make_float4(iv[4 * q], iv[4 * q + 1], iv[4 * q + 2], iv[4 * q + 3]);
@@ -368,6 +406,8 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   float* const Ws = reinterpret_cast<float*>(sm + G::OFF_W);      // w = dL/dM tile
   float* const accS = reinterpret_cast<float*>(sm + G::OFF_ACC);
   float* const Ks = reinterpret_cast<float*>(sm + G::OFF_K);
+  float* const Bs = reinterpret_cast<float*>(sm + G::OFF_BG);     // background coefficients of the current epoch
+  double* const bgacc = reinterpret_cast<double*>(sm + G::OFF_BGACC) + (threadIdx.x >> 5) * kMaxBg;   // this warp's row
   const unsigned bar0 = smem_u32(sm + G::OFF_BAR);            // barR[0], barR[1], barI
   double* const red64 = reinterpret_cast<double*>(sm + G::OFF_BAR + 64);
 
@@ -442,7 +482,14 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
       double ls = 0.0, gs = 0.0;
       for (int w = 0; w < kThreads / 32; ++w) { ls += red64[w]; gs += red64[8 + w]; }
       out[(size_t)(M * M) * ncols] = gs;
-      out[(size_t)(M * M + 1) * ncols] = ls;
+      out[(size_t)p.np * ncols] = ls;
+      // background coefficients beyond b_00: warp rows in fixed order
+      const double* all = reinterpret_cast<const double*>(sm + G::OFF_BGACC);
+      for (int t = 1; t < p.np - M * M; ++t) {
+        double sacc = 0.0;
+        for (int w = 0; w < kThreads / 32; ++w) sacc += all[w * kMaxBg + t];
+        out[(size_t)(M * M + t) * ncols] = sacc;
+      }
     }
     __syncthreads();                       // red64 / Ks / accS free for the next epoch
   };
@@ -460,18 +507,20 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
     if (e != cur_e) {                      // first tile of an epoch for this CTA
       if (cur_e >= 0) finish_epoch();
       cur_e = e;
-      const float* __restrict__ th = p.theta + (size_t)e * G::NP;
+      const float* __restrict__ th = p.theta + (size_t)e * p.np;
       for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
         const int a = idx / G::KP, b = idx - a * G::KP;
         Ks[idx] = (b < M) ? th[a * M + b] : 0.f;
       }
       B0 = th[M * M];
+      if (tid < kMaxBg) Bs[tid] = (tid < p.np - M * M) ? th[M * M + tid] : 0.f;
+      if (lane < kMaxBg) bgacc[lane] = 0.0;
 #pragma unroll
       for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
       loss64 = 0.0; gb064 = 0.0; flushed = false; since_flush = 0;
       // column of this CTA in epoch e: the local index (mod grid) of the tiles it owns there
       int col = ((int)blockIdx.x - (int)(((long long)e * n_tiles) % grid) + grid) % grid;
-      out = p.partials + ((size_t)e * (G::NP + 1)) * ncols + col;
+      out = p.partials + ((size_t)e * (p.np + 1)) * ncols + col;
       __syncthreads();                     // Ks visible
     }
     const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
@@ -486,12 +535,31 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
       const int iy = tile_y * kTH + f_row, ix0 = tile_x * kTW + f_col;
       const float* irow = Is + f_row * kIPitch + f_col;
       float* wrow = Ws + f_row * kIPitch + f_col;
-      float lsum, wsum;
+      float lsum, wsum, Sp[4];
       const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
-      if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
-      else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, lsum, wsum);
+      if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp);
+      else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp);
       loss64 += (double)lsum;
       gb064 += (double)wsum;
+      if (p.bg_degree > 0) {               // dL/db_mn = sum w eta^m xi^n: strip sums -> warp sum -> this warp's FP64 row
+        const float xi = ((float)(iy + G::H) - p.bg_yc) * p.bg_inv_ny;
+        int tt = 0;
+#pragma unroll
+        for (int mm = 0; mm < 4; ++mm) {
+          float term = Sp[mm];
+#pragma unroll
+          for (int nn = 0; nn < 4; ++nn) {
+            if (mm <= p.bg_degree && nn <= p.bg_degree - mm) {       // CTA-uniform
+              float v = term;
+#pragma unroll
+              for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+              if (lane == 0 && tt > 0) bgacc[tt] += (double)v;
+              ++tt;
+            }
+            term *= xi;
+          }
+        }
+      }
     }
     __syncthreads();                       // (A) w tile complete, I tile consumed
     if (gn < total) {

@@ -119,12 +119,12 @@ __device__ __forceinline__ double laplacian_row(const double* __restrict__ x, in
 
 // Eq. 20: adds lamN |L theta|^2 to loss[e] and 2 lamN L (L theta) to grad[e][0..m*m) for the
 // stand-alone evaluation path (one CTA per epoch, launched after reduce_partials_kernel).
-__global__ void __launch_bounds__(kFitThreads) penalty_kernel(const float* __restrict__ theta, int m, double lamN,
+__global__ void __launch_bounds__(kFitThreads) penalty_kernel(const float* __restrict__ theta, int m, int np, double lamN,
                                                               double* __restrict__ loss, double* __restrict__ grad) {
   __shared__ double xs[kFitThreads * kMaxPerThread], us[kFitThreads * kMaxPerThread];
   __shared__ double sh_rows[2][kFitThreads / 32];
   BlockRed br{sh_rows, 0};
-  const int e = blockIdx.x, nk = m * m, np = nk + 1, tid = threadIdx.x;
+  const int e = blockIdx.x, nk = m * m, tid = threadIdx.x;
   for (int k = tid; k < nk; k += kFitThreads) xs[k] = (double)theta[(size_t)e * np + k];
   __syncthreads();
   double pen = 0.0;
@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
   __shared__ double sh_rows[2][kFitThreads / 32];
   BlockRed sh{sh_rows, 0};
   __shared__ double s_alpha[kMaxHistory];
-  const int np = a.np, nk = np - 1, tid = threadIdx.x;
+  const int np = a.np, nk = a.m * a.m, tid = threadIdx.x;   // nk kernel pixels, np - nk background coefficients
   const dia_fit_opts& o = a.o;
   FitState st = a.b.st[e];                       // every thread holds a private copy; thread 0 writes back
 

@@ -216,6 +216,38 @@ def test_fit_with_laplacian_regularisation(dia):
     h.close()
 
 
+def test_fit_polynomial_background(dia):
+    """Eq. 18-19 inside dia_fit: a planted background gradient is absorbed by the degree-1 coefficients.
+    Lock-step against the oracle (strict), then a free-running regularised fit recovers the planted slope."""
+    w = make_workload(0)
+    n, m = w.n, w.m
+    y, x = np.mgrid[0:n, 0:n].astype(np.float64)
+    eta, xi = (x - (n - 1) / 2) / n, (y - (n - 1) / 2) / n
+    I = (w.I[0].astype(np.float64) + 30.0 * eta - 18.0 * xi).astype(np.float32)[None]     # b_10 = 30, b_01 = -18
+    th0 = np.concatenate([w.theta0[0], [0.0, 0.0]]).astype(np.float32)[None]               # [K, b_00, b_01, b_10]
+    lam = 10.0
+    cfg = oracle.RefConfig(n, n, m, sigma0=w.sigma0, gain=w.gain, bg_degree=1, lambda_reg=lam)
+    h = dia.Handle(_dev(w.R), m, sigma0=w.sigma0, gain=w.gain, bg_degree=1, lambda_reg=lam)
+    og, oo = _both_opts(dia, force_adam_iters=30, force_lbfgs_iters=6)
+    tho, ro = oracle.fit(cfg, w.R, I, th0, oo)
+    thg, rg = h.fit(_dev(I), _dev(th0), og)
+    thg = thg.cpu().numpy()
+    assert rg[0].n_evals == ro[0].n_evals
+    assert np.abs(thg[0][:m * m] - tho[0][:m * m]).max() <= 1e-4 * np.abs(tho[0][:m * m]).max()
+    assert np.abs(thg[0][m * m:] - tho[0][m * m:]).max() <= 1e-4 * max(1.0, np.abs(tho[0][m * m:]).max())
+    assert rg[0].photometric_scale == pytest.approx(ro[0].photometric_scale, rel=1e-4)
+    og, oo = _both_opts(dia, lr_b0=10.0)
+    tho, ro = oracle.fit(cfg, w.R, I, th0, oo)
+    thg, rg = h.fit(_dev(I), _dev(th0), og)
+    thg = thg.cpu().numpy()
+    print("bg fit gpu b =", thg[0][m * m:], "oracle b =", tho[0][m * m:], "P", rg[0].photometric_scale, ro[0].photometric_scale,
+          "iters", rg[0].n_evals, ro[0].n_evals)
+    assert rg[0].status in (0, 1)
+    assert abs(thg[0][m * m + 2] - 30.0) < 3.0 and abs(thg[0][m * m + 1] + 18.0) < 3.0      # b_10, b_01 within noise
+    assert rg[0].photometric_scale == pytest.approx(ro[0].photometric_scale, rel=1e-3)
+    h.close()
+
+
 def test_fit_huber_with_cosmic_rays(dia):
     """BASELINE config 2 shape at reduced size: robust objective, 0.1 % cosmic-ray hits, no mask."""
     w = make_workload(2, n=200, m=9)

@@ -198,6 +198,28 @@ def test_laplacian_regularisation_eq20(dia, c, n, m, lam):
     h.close()
 
 
+@pytest.mark.parametrize("d,c,n,m", [(1, 0, None, None), (2, 4, 333, 19), (3, 1, 300, 15), (3, 3, 260, 9)])
+def test_polynomial_background_eq18(dia, d, c, n, m):
+    """Eq. 18-19: spatially varying background of degree d replaces B0; the gradient gets
+    (d+1)(d+2)/2 background components.  Odd n exercises the cp.async staging path, c3 the flat + mask path."""
+    w = make_workload(c, n=n, m=m, n_epochs=2 if c == 4 else None)
+    nb = (d + 1) * (d + 2) // 2
+    rng = np.random.default_rng(40 + d)
+    E = w.n_epochs
+    def with_bg(th):
+        b = np.concatenate([th[:, -1:], rng.normal(0, 5.0, (E, nb - 1))], axis=1)
+        return np.concatenate([th[:, :-1], b], axis=1).astype(np.float32)
+    h = _handle(dia, w, bg_degree=d)
+    cfg = _ref_cfg(w, bg_degree=d)
+    for name, th, kind in _points(w)[:2]:
+        th = with_bg(np.asarray(th, np.float64))
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=w.mask, want_scale=True)
+        Lg, gg = h.eval_loss_grad(_dev(w.I), _dev(th), mask=_dev(w.mask))
+        assert gg.shape[1] == w.m * w.m + nb
+        _compare(Lg, gg, Lo, go, So, kind, f"bg d={d} c{c} {name}")
+    h.close()
+
+
 def test_emccd_noise_model_eq7(dia):
     """EMCCD noise model, Eq. 7: sigma^2 = E M / (G_total F) with E = 2, G_total = 25.8/300
     e-/ADU -- the affine form of Eq. 6 with no read-noise term, i.e. sigma0 = 0 and gain = G_total / E."""

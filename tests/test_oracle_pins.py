@@ -262,3 +262,55 @@ def test_laplacian_penalty_matches_eq20_matrix_form():
     # a flat kernel has zero Laplacian everywhere, border included
     flat = np.concatenate([np.full(m * m, 0.125), [1.0]]).astype(np.float32)
     assert oracle.eval_loss_grad(c1, R, I, flat)[0][0] == oracle.eval_loss_grad(c0, R, I, flat)[0][0]
+
+
+# ---------------------------------------------------------------- polynomial background, Eq. 18-19
+def _bg_numpy(n_r, n_c, d, b):
+    """Eq. 18-19 (PAPER.md:200-208) with numpy: eta = (x - x_c)/N_x, xi = (y - y_c)/N_y, x = column, y = row,
+    centre = ((N-1)/2), coefficient order m = 0..d outer, n = 0..d-m inner (reading R18)."""
+    y, x = np.mgrid[0:n_r, 0:n_c].astype(np.float64)
+    eta = (x - (n_c - 1) / 2) / n_c
+    xi = (y - (n_r - 1) / 2) / n_r
+    B = np.zeros((n_r, n_c))
+    t = 0
+    for mm in range(d + 1):
+        for nn in range(d - mm + 1):
+            B += b[t] * eta ** mm * xi ** nn
+            t += 1
+    assert t == (d + 1) * (d + 2) // 2
+    return B, eta, xi
+
+
+@pytest.mark.parametrize("d", [1, 2, 3])
+def test_polynomial_background_model_and_gradient(d):
+    """K = delta => M = crop(R) + B(x, y); dL/db_mn = sum_V w eta^m xi^n.  Catches swapped x / y, a wrong
+    centre or normalisation, a wrong coefficient order and a missing basis factor in the gradient."""
+    n_r, n_c, m, h = 11, 14, 3, 1
+    rng = np.random.default_rng(10 + d)
+    R = (100 + 50 * rng.random((n_r, n_c))).astype(np.float32)
+    I = (150 + 50 * rng.random((n_r, n_c))).astype(np.float32)
+    nb = (d + 1) * (d + 2) // 2
+    b = (rng.normal(0, 8, nb)).astype(np.float32)
+    K = np.zeros((m, m), np.float32); K[h, h] = 1.0
+    th = np.concatenate([K.ravel(), b])
+    cfg = oracle.RefConfig(n_r, n_c, m, sigma0=5.0, gain=1.5, bg_degree=d)
+    assert cfg.n_params == m * m + nb
+    B, eta, xi = _bg_numpy(n_r, n_c, d, b.astype(np.float64))
+    M = oracle.model(cfg, R, th)
+    assert np.allclose(M, R[h:-h, h:-h].astype(np.float64) + B[h:-h, h:-h], rtol=1e-13, atol=1e-11)
+    # gradient of the background coefficients from w, rebuilt from the model by hand (D1, Gaussian, MODEL noise)
+    L, g = oracle.eval_loss_grad(cfg, R, I, th)
+    v = 25.0 + M / 1.5
+    r = I[h:-h, h:-h].astype(np.float64) - M
+    w = -r / v + (1 / (2 * 1.5 * v)) * (1 - r * r / v)
+    assert L[0] == pytest.approx((0.5 * r * r / v + 0.5 * np.log(v)).sum(), rel=1e-13)
+    t = 0
+    for mm in range(d + 1):
+        for nn in range(d - mm + 1):
+            assert g[0][m * m + t] == pytest.approx((w * eta[h:-h, h:-h] ** mm * xi[h:-h, h:-h] ** nn).sum(), rel=1e-10, abs=1e-12)
+            t += 1
+    # d = 0 inside the same code path is the scalar B0
+    cfg0 = oracle.RefConfig(n_r, n_c, m, sigma0=5.0, gain=1.5)
+    th0 = np.concatenate([K.ravel(), b[:1]])
+    b1 = b.copy(); b1[1:] = 0
+    assert np.array_equal(oracle.model(cfg0, R, th0), oracle.model(cfg, R, np.concatenate([K.ravel(), b1])))
