@@ -121,6 +121,16 @@ int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs,
             const float* d_I, const unsigned char* d_mask, const float* d_var,
             float* d_theta, dia_fit_result* d_result);
 
+/* Difference image and fit-quality metrics for n_epochs targets at the given theta (the science product,
+ * PAPER.md:20; metrics of Eq. 29-30):
+ *   D_ij = I_ij - M_ij on the valid region V (mask or not), 0 outside V;
+ *   eps_ij = D_ij / sigma_ij over the unmasked pixels of V, sigma from Eq. 6 at the model M (or the caller's
+ *   variance map in DIA_NOISE_FIXED);  d_metrics[e] = { N_used, MFB = mean(eps), MFV = sum (eps - MFB)^2 / (N - 1),
+ *   chi^2 = sum eps^2 }.
+ * d_D [n_epochs][n_rows][n_cols] float32 and d_metrics [n_epochs][4] float64 are DEVICE buffers.  Asynchronous. */
+int dia_difference_image(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
+                         const float* d_var, const float* d_theta, float* d_D, double* d_metrics);
+
 /* Frees the handle's workspace (synchronises the handle's stream first). */
 int dia_destroy(dia_handle* h);
 

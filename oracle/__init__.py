@@ -10,6 +10,7 @@ from .dia_ref import (  # noqa: F401
     eval_loss_grad,
     fit,
     b08_solve,
+    difference_image,
     model,
     huber_Q,
     num_threads,

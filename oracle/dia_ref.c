@@ -219,6 +219,49 @@ int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epoc
   return DIA_REF_OK;
 }
 
+int dia_ref_difference_image(const dia_ref_config* cfg, const float* R, const float* I,
+                             const unsigned char* mask, const float* var, const float* theta,
+                             double* D, double* metrics) {
+  if (!check_cfg(cfg) || !R || !I || !theta || !D || !metrics) return DIA_REF_ERR_INVALID_ARG;
+  if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
+  const int m = cfg->m, h = (m - 1) / 2, nr = cfg->n_rows, nc = cfg->n_cols;
+  for (size_t p = 0; p < (size_t)nr * nc; ++p) D[p] = 0.0;
+  /* first pass: D and eps; MFB (Eq. 29) needs the mean before MFV (Eq. 30) can be formed as printed */
+  double n_used = 0.0, s1 = 0.0, chi2 = 0.0;
+  double* eps = (double*)malloc(sizeof(double) * (size_t)nr * nc);
+  if (!eps) return DIA_REF_ERR_ALLOC;
+  for (int i = h; i < nr - h; ++i)
+    for (int j = h; j < nc - h; ++j) {
+      const size_t p = (size_t)i * nc + j;
+      const double M = model_pixel(cfg, R, nc, m, theta, i, j);
+      D[p] = (double)I[p] - M;
+      eps[p] = 0.0;
+      if (mask && mask[p] == 0) continue;
+      double v;
+      if (cfg->noise == DIA_REF_NOISE_MODEL) {
+        const double F = cfg->flat ? (double)cfg->flat[p] : 1.0;
+        v = cfg->sigma0 * cfg->sigma0 / (F * F) + (M > 0.0 ? M : 0.0) / (cfg->gain * F);      /* Eq. 6, R1 */
+      } else {
+        v = (double)var[p];
+      }
+      eps[p] = D[p] / sqrt(v);
+      n_used += 1.0;  s1 += eps[p];  chi2 += eps[p] * eps[p];
+    }
+  const double mfb = n_used > 0.0 ? s1 / n_used : 0.0;                                       /* Eq. 29 */
+  double s2 = 0.0;
+  for (int i = h; i < nr - h; ++i)
+    for (int j = h; j < nc - h; ++j) {
+      const size_t p = (size_t)i * nc + j;
+      if (mask && mask[p] == 0) continue;
+      s2 += (eps[p] - mfb) * (eps[p] - mfb);
+    }
+  metrics[0] = n_used;  metrics[1] = mfb;
+  metrics[2] = n_used > 1.0 ? s2 / (n_used - 1.0) : 0.0;                                     /* Eq. 30 */
+  metrics[3] = chi2;
+  free(eps);
+  return DIA_REF_OK;
+}
+
 /* Eq. 14: Q = N ln( sqrt(2 pi) erf(c/sqrt 2) + 2 exp(-c^2/2)/c ). */
 double dia_ref_huber_Q(double c, double N) {
   const double pi = 3.14159265358979323846;

@@ -72,6 +72,13 @@ int dia_ref_eval_loss_grad(const dia_ref_config* cfg, const float* R, int n_epoc
                            const float* I, const unsigned char* mask, const float* var,
                            const float* theta, double* loss, double* grad, double* grad_scale);
 
+/* Difference image D = I - M on the valid region (0 elsewhere), [n_rows][n_cols] FP64, and the fit-quality
+ * metrics of Eq. 29-30 over the unmasked valid pixels, with sigma from Eq. 6 at the model
+ * (or the caller's variance map): metrics = { N_used, MFB, MFV, chi^2 }.  One epoch. */
+int dia_ref_difference_image(const dia_ref_config* cfg, const float* R, const float* I,
+                             const unsigned char* mask, const float* var, const float* theta,
+                             double* D, double* metrics);
+
 /* Adam -> L-BFGS fit (DESIGN c.2), one epoch after another.  theta in/out float32. */
 int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
                 int n_epochs, const float* I, const unsigned char* mask, const float* var,

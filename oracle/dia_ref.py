@@ -169,6 +169,21 @@ def b08_solve(cfg: RefConfig, R, I, mask=None, var_fixed=None, n_iters=3, clip_l
     return (theta, H) if want_H else theta
 
 
+def difference_image(cfg: RefConfig, R, I, theta, mask=None, var=None):
+    """-> (D float64 [n_rows][n_cols], metrics float64 [4] = N_used, MFB, MFV, chi^2) for one epoch."""
+    c, keep = cfg._c()
+    R, I = _f32(R), _f32(I)
+    assert I.shape == (cfg.n_rows, cfg.n_cols)
+    theta = _f32(theta).reshape(-1)
+    mask = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    var = _f32(var)
+    D = np.empty((cfg.n_rows, cfg.n_cols), dtype=np.float64)
+    metrics = np.empty(4, dtype=np.float64)
+    _check(_lib().dia_ref_difference_image(C.byref(c), _ptr(R), _ptr(I), _ptr(mask), _ptr(var), _ptr(theta),
+                                           _ptr(D), _ptr(metrics)), "dia_ref_difference_image")
+    return D, metrics
+
+
 def huber_Q(c: float, N: float) -> float:
     return float(_lib().dia_ref_huber_Q(float(c), float(N)))
 

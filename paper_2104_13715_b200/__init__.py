@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     Handle,
     dia_create,
     dia_destroy,
+    dia_difference_image,
     dia_eval_loss_grad,
     dia_fit,
     dia_measure_fp32_peak,

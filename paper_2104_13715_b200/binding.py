@@ -19,7 +19,7 @@ NOISE_MODEL, NOISE_FIXED = 0, 1
 FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
-                    "dia_measure_fp32_peak")
+                    "dia_measure_fp32_peak", "dia_difference_image")
 
 
 class DiaError(RuntimeError):
@@ -87,6 +87,7 @@ def load_library(build_if_missing: bool = True):
     lib.dia_fit.argtypes = [C.c_void_p, C.POINTER(FitOpts), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                             C.c_void_p, C.c_void_p]
     lib.dia_destroy.argtypes = [C.c_void_p]
+    lib.dia_difference_image.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
     lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     _LIB = lib
@@ -145,6 +146,14 @@ def dia_fit(handle: int, opts: FitOpts, n_epochs: int, d_I, d_mask, d_var, d_the
            handle)
 
 
+def dia_difference_image(handle: int, n_epochs: int, d_I, d_mask, d_var, d_theta, d_D, d_metrics) -> None:
+    lib = load_library()
+    _check(lib.dia_difference_image(handle, n_epochs, _dptr(d_I, torch.float32, "d_I"),
+                                    _dptr(d_mask, torch.uint8, "d_mask"), _dptr(d_var, torch.float32, "d_var"),
+                                    _dptr(d_theta, torch.float32, "d_theta"), _dptr(d_D, torch.float32, "d_D"),
+                                    _dptr(d_metrics, torch.float64, "d_metrics")), handle)
+
+
 def dia_destroy(handle: int) -> None:
     _check(load_library().dia_destroy(handle))
 
@@ -201,6 +210,14 @@ class Handle:
         grad = torch.empty((E, self.np), dtype=torch.float64, device=dev) if grad is None else grad
         dia_eval_loss_grad(self._h, E, I, mask, var, theta, loss, grad)
         return loss, grad
+
+    def difference_image(self, I, theta, mask=None, var=None):
+        """-> (D float32 [E][n_rows][n_cols], metrics float64 [E][4] = N_used, MFB, MFV, chi^2), CUDA tensors."""
+        E = self._epochs(I)
+        D = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.float32, device=I.device)
+        metrics = torch.empty((E, 4), dtype=torch.float64, device=I.device)
+        dia_difference_image(self._h, E, I, mask, var, theta, D, metrics)
+        return D, metrics
 
     def fit(self, I, theta0, opts: Optional[FitOpts] = None, mask=None, var=None):
         """Returns (theta_hat float32 [E][np] CUDA tensor, list[FitResult]); synchronises to read results."""

@@ -82,10 +82,13 @@ static void geometry_for(int m, int* rpitch, int* rh) {
 #undef X
   }
 }
-// aux = true: mask / flat field / caller variance map present (read from global memory per pixel)
-static const void* kernel_for(int m, bool aux) {
+// aux = true: mask / flat field / caller variance map present (read from global memory per pixel);
+// diff = true: difference-image instantiation (forward only, generic per-pixel inputs)
+static const void* kernel_for(int m, bool aux, bool diff = false) {
   switch (m) {
-#define X(MM) case MM: return aux ? (const void*)dia::eval_kernel<MM, true> : (const void*)dia::eval_kernel<MM, false>;
+#define X(MM) case MM: return diff ? (const void*)dia::eval_kernel<MM, true, true>                    \
+                                   : aux ? (const void*)dia::eval_kernel<MM, true, false>             \
+                                         : (const void*)dia::eval_kernel<MM, false, false>;
     DIA_FOR_EACH_M(X)
 #undef X
   }
@@ -140,9 +143,9 @@ int eval_part_cols(const dia_handle* h, int n_epochs) {
   const int g = eval_grid(h, n_epochs);
   return h->tiles < g ? h->tiles : g;
 }
-cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm) {
+cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff) {
   void* args[] = {(void*)&p, (void*)&tm};
-  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p)), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
+  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), diff), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
                           h->smem, h->stream);
 }
 }  // namespace dia
@@ -160,7 +163,7 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
   p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
   p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;  p->n_refs = h->n_refs;
-  p->np = h->np;  p->bg_degree = c.bg_degree;            // Eq. 19: centre ((N-1)/2), normalisation N (R18)
+  p->np = h->np;  p->part_rows = h->np + 1;  p->diff = nullptr;  p->bg_degree = c.bg_degree;            // Eq. 19: centre ((N-1)/2), normalisation N (R18)
   p->bg_xc = 0.5f * (float)(c.n_cols - 1);  p->bg_yc = 0.5f * (float)(c.n_rows - 1);
   p->bg_inv_nx = 1.0f / (float)c.n_cols;  p->bg_inv_ny = 1.0f / (float)c.n_rows;
   p->tiles_x = (c.n_cols - c.m + 1 + dia::kTW - 1) / dia::kTW;
@@ -208,8 +211,8 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   h->np = cfg->m * cfg->m + (cfg->bg_degree + 1) * (cfg->bg_degree + 2) / 2;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
 
   int occ = 0;
-  for (int aux = 0; aux < 2; ++aux) {
-    const void* k = kernel_for(cfg->m, aux != 0);
+  for (int aux = 0; aux < 3; ++aux) {        // the two evaluation variants and the difference-image variant
+    const void* k = kernel_for(cfg->m, aux != 0, aux == 2);
     ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
     if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
     int o = 0;
@@ -275,6 +278,27 @@ extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I,
     dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, h->stream>>>(d_theta, h->cfg.m, h->np, lambda_n(h), d_loss, d_grad);
   ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
+  return DIA_OK;
+}
+
+extern "C" int dia_difference_image(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
+                                    const float* d_var, const float* d_theta, float* d_D, double* d_metrics) {
+  int rc = check_eval_args(h, n_epochs, d_I, d_var, d_theta);
+  if (rc != DIA_OK) return rc;
+  if (!d_D || !d_metrics) return fail(h, DIA_ERR_INVALID_ARG, "null output");
+  const size_t npix = (size_t)h->cfg.n_rows * h->cfg.n_cols;
+  cudaError_t ce = cudaMemsetAsync(d_D, 0, sizeof(float) * npix * n_epochs, h->stream);   // pixels outside V read 0
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "memset");
+  dia::EvalParams p;
+  dia::TensorMaps tm;
+  fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm);
+  p.part_rows = 3;
+  p.diff = d_D;
+  ce = dia::launch_eval(h, p, tm, true);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "difference-image launch");
+  dia::diff_metrics_kernel<<<n_epochs, 32, 0, h->stream>>>(h->d_partials, dia::eval_part_cols(h, n_epochs), d_metrics);
+  ce = cudaGetLastError();
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "metrics launch");
   return DIA_OK;
 }
 

@@ -76,11 +76,13 @@ struct EvalParams {
   const float* var;          // [E][n_rows][n_cols] or null (FIXED noise)
   const float* flat;         // [n_rows][n_cols] or null
   const float* theta;        // [E][np] float32: K row-major, then the background coefficients
+  float* diff;               // [E][n_rows][n_cols] difference image (DIFF instantiation only)
   const int* done;           // [E] or null: epochs with done != 0 are skipped
   double* partials;          // [E][NP+1][ncols], ncols = min(tiles, gridDim.x): rows g_K (M*M), g_B0, loss;
                              // one column per CTA that owns tiles of the epoch
   int n_rows, n_cols, n_epochs;
   int n_refs;                // 1: one reference shared by all epochs; else one reference per epoch
+  int part_rows;             // rows of partials per epoch: np + 1 (gradient, loss), or 3 in difference-image mode
   int np, bg_degree;         // parameters per epoch = M*M + (d+1)(d+2)/2; degree d of the background (Eq. 18)
   float bg_xc, bg_yc, bg_inv_nx, bg_inv_ny;   // Eq. 19: eta = (x - xc) / N_x, xi = (y - yc) / N_y
   int tiles_x, tiles_y;
@@ -326,6 +328,77 @@ __device__ __forceinline__ void forward_strip(const float* __restrict__ Ks, cons
   for (int q = 0; q < kP; ++q) tot[q] += rs[q];
 }
 
+// Adds the background terms beyond b_00 (Eq. 18-19) to the model strip.
+template <int M>
+__device__ __forceinline__ void add_background(const EvalParams& p, const float* __restrict__ Bs, int iy, int ix0,
+                                               float (&tot)[kP]) {
+  using G = Geo<M>;
+  const int d = p.bg_degree;
+  if (d <= 0) return;                                // CTA-uniform
+  const float eta0 = ((float)(ix0 + G::H) - p.bg_xc) * p.bg_inv_nx;
+  const float xi = ((float)(iy + G::H) - p.bg_yc) * p.bg_inv_ny;
+  float c[4] = {0.f, 0.f, 0.f, 0.f};                 // c_p(xi) = sum_n b_pn xi^n, without b_00
+  int t = 0;
+#pragma unroll
+  for (int mm = 0; mm < 4; ++mm) {
+    float xn = 1.f;
+#pragma unroll
+    for (int nn = 0; nn < 4; ++nn) {
+      if (mm <= d && nn <= d - mm) {
+        if (t > 0) c[mm] = fmaf(Bs[t], xn, c[mm]);
+        ++t;
+      }
+      xn *= xi;
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < kP; ++q) {
+    const float eta = fmaf((float)q, p.bg_inv_nx, eta0);
+    tot[q] += fmaf(fmaf(fmaf(c[3], eta, c[2]), eta, c[1]), eta, c[0]);
+  }
+}
+
+// Difference-image mode: D = I - M for every pixel of the valid region, written to global
+// memory, and the sums of eps = (I - M)/sigma, eps^2 and the pixel count over the unmasked valid pixels
+// (fit-quality metrics MFB, MFV, Eq. 29-30).
+template <int M, bool EDGE>
+__device__ __forceinline__ void strip_diff(const EvalParams& p, int e, size_t npix, int iy, int ix0, int vr, int vc,
+                                           const float (&tot)[kP], const float* __restrict__ irow, float& s_eps,
+                                           float& s_eps2, float& s_cnt) {
+  using G = Geo<M>;
+  const size_t gbase = (size_t)(iy + G::H) * p.n_cols + (ix0 + G::H);
+  float* __restrict__ Drow = p.diff + (size_t)e * npix + gbase;
+  s_eps = 0.f; s_eps2 = 0.f; s_cnt = 0.f;
+#pragma unroll
+  for (int q = 0; q < kP; ++q) {
+    const bool inside = EDGE ? ((iy < vr) && (ix0 + q < vc)) : true;
+    if (!inside) continue;
+    const float Mv = tot[q];
+    const float res = irow[q + G::IOFF] - Mv;
+    Drow[q] = res;
+    bool use = true;
+    if (p.mask) use = p.mask[(size_t)e * npix + gbase + q] != 0;
+    float v;
+    if (p.noise_kind == 0) {
+      float a_ij = p.sigma0_sq, b_ij = p.inv_gain;
+      if (p.flat) {
+        const float invF = 1.0f / p.flat[gbase + q];
+        a_ij *= invF * invF;
+        b_ij *= invF;
+      }
+      v = fmaf(b_ij, fmaxf(Mv, 0.f), a_ij);
+    } else {
+      v = p.var[(size_t)e * npix + gbase + q];
+    }
+    if (use) {
+      const float eps = res * rsqrtf(v);
+      s_eps += eps;
+      s_eps2 = fmaf(eps, eps, s_eps2);
+      s_cnt += 1.f;
+    }
+  }
+}
+
 // epilogue of the forward phase for one strip: loss terms and the w strip.  With a polynomial background
 // (Eq. 18-19) the terms beyond b_00 are added to the model here, and the sums
 // S_p = sum_q w_q eta_q^p (p = 0..d) of the strip are returned for the background gradient.
@@ -348,28 +421,7 @@ __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_
   }
   const int d = p.bg_degree;
   const float eta0 = ((float)(ix0 + G::H) - p.bg_xc) * p.bg_inv_nx;
-  if (d > 0) {                                       // CTA-uniform
-    const float xi = ((float)(iy + G::H) - p.bg_yc) * p.bg_inv_ny;
-    float c[4] = {0.f, 0.f, 0.f, 0.f};               // c_p(xi) = sum_n b_pn xi^n, without b_00
-    int t = 0;
-#pragma unroll
-    for (int mm = 0; mm < 4; ++mm) {
-      float xn = 1.f;
-#pragma unroll
-      for (int nn = 0; nn < 4; ++nn) {
-        if (mm <= d && nn <= d - mm) {
-          if (t > 0) c[mm] = fmaf(Bs[t], xn, c[mm]);
-          ++t;
-        }
-        xn *= xi;
-      }
-    }
-#pragma unroll
-    for (int q = 0; q < kP; ++q) {
-      const float eta = fmaf((float)q, p.bg_inv_nx, eta0);
-      tot[q] += fmaf(fmaf(fmaf(c[3], eta, c[2]), eta, c[1]), eta, c[0]);
-    }
-  }
+  add_background<M>(p, Bs, iy, ix0, tot);
   const size_t gbase = (size_t)(iy + G::H) * p.n_cols + (ix0 + G::H);
   lsum = 0.f; wsum = 0.f;
   Sp[1] = 0.f; Sp[2] = 0.f; Sp[3] = 0.f;
@@ -395,7 +447,7 @@ __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_
 // ------------------------------------------------------------------------------------------------
 // the fused kernel
 // ------------------------------------------------------------------------------------------------
-template <int M, bool AUX>
+template <int M, bool AUX, bool DIFF>
 __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, const __grid_constant__ TensorMaps tm) {
   using G = Geo<M>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -451,7 +503,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   };
 
   float B0 = 0.f;
-  double loss64 = 0.0, gb064 = 0.0;
+  double loss64 = 0.0, gb064 = 0.0, cnt64 = 0.0;   // DIFF: sum eps^2, sum eps, pixel count
   bool flushed = false;
   int since_flush = 0, cur_e = -1;
   double* out = nullptr;                   // element o of this CTA's partial column at out[o * ncols]
@@ -474,6 +526,20 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   };
   // per-epoch block partials: gradient strips, then g_B0 and the loss
   auto finish_epoch = [&]() {
+    if (DIFF) {                            // rows: sum eps, sum eps^2, count
+      __syncthreads();
+      const double l = warp_sum_f64(loss64), g0 = warp_sum_f64(gb064), c0 = warp_sum_f64(cnt64);
+      if (lane == 0) { red64[warp] = l; red64[8 + warp] = g0; bgacc[0] = c0; }
+      __syncthreads();
+      if (tid == 0) {
+        double ls = 0.0, gs = 0.0, cs = 0.0;
+        const double* all = reinterpret_cast<const double*>(sm + G::OFF_BGACC);
+        for (int w = 0; w < kThreads / 32; ++w) { ls += red64[w]; gs += red64[8 + w]; cs += all[w * kMaxBg]; }
+        out[0] = gs;  out[(size_t)ncols] = ls;  out[(size_t)2 * ncols] = cs;
+      }
+      __syncthreads();
+      return;
+    }
     flush();                               // ends with a barrier after the last reads of accS
     const double l = warp_sum_f64(loss64), g0 = warp_sum_f64(gb064);
     if (lane == 0) { red64[warp] = l; red64[8 + warp] = g0; }
@@ -517,10 +583,10 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
       if (lane < kMaxBg) bgacc[lane] = 0.0;
 #pragma unroll
       for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-      loss64 = 0.0; gb064 = 0.0; flushed = false; since_flush = 0;
+      loss64 = 0.0; gb064 = 0.0; cnt64 = 0.0; flushed = false; since_flush = 0;
       // column of this CTA in epoch e: the local index (mod grid) of the tiles it owns there
       int col = ((int)blockIdx.x - (int)(((long long)e * n_tiles) % grid) + grid) % grid;
-      out = p.partials + ((size_t)e * (p.np + 1)) * ncols + col;
+      out = p.partials + ((size_t)e * p.part_rows) * ncols + col;
       __syncthreads();                     // Ks visible
     }
     const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
@@ -537,11 +603,19 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
       float* wrow = Ws + f_row * kIPitch + f_col;
       float lsum, wsum, Sp[4];
       const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
+      if (DIFF) {
+        float s_eps, s_eps2, s_cnt;
+        add_background<M>(p, Bs, iy, ix0, tot);
+        if (edge) strip_diff<M, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, s_eps, s_eps2, s_cnt);
+        else strip_diff<M, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, s_eps, s_eps2, s_cnt);
+        gb064 += (double)s_eps;  loss64 += (double)s_eps2;  cnt64 += (double)s_cnt;
+      } else {
       if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp);
       else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp);
       loss64 += (double)lsum;
       gb064 += (double)wsum;
-      if (p.bg_degree > 0) {               // dL/db_mn = sum w eta^m xi^n: strip sums -> warp sum -> this warp's FP64 row
+      }
+      if (!DIFF && p.bg_degree > 0) {               // dL/db_mn = sum w eta^m xi^n: strip sums -> warp sum -> this warp's FP64 row
         const float xi = ((float)(iy + G::H) - p.bg_yc) * p.bg_inv_ny;
         int tt = 0;
 #pragma unroll
@@ -568,7 +642,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
     }
 
     // ------------------------------------------------------------------ gradient
-    if (g_active) {
+    if (!DIFF && g_active) {
       float acc[G::KP];
 #pragma unroll
       for (int q = 0; q < G::KP / 4; ++q) {
@@ -604,7 +678,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
     }
     __syncthreads();                       // (B) everyone is done reading this w tile and R buffer
     if (G::NRBUF == 1 && gn < total) stage_R<M>(p, tm, en, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
-    if (++since_flush == kFlushTiles && gn < total && en == e) flush();
+    if (!DIFF && ++since_flush == kFlushTiles && gn < total && en == e) flush();
     g = gn;
     ++it;
   }
@@ -632,6 +706,23 @@ __global__ void reduce_partials_kernel(const double* __restrict__ partials, int 
   if (lane == 0) {
     if (o == np1 - 1) loss[e] = s;
     else grad[(size_t)e * (np1 - 1) + o] = s;
+  }
+}
+
+// Fit-quality metrics from the difference-image partial sums (Eq. 29-30): one warp per epoch.
+// metrics[e] = { N_used, MFB = sum eps / N, MFV = sum (eps - MFB)^2 / (N - 1), chi^2 = sum eps^2 }.
+__global__ void diff_metrics_kernel(const double* __restrict__ partials, int n_blocks, double* __restrict__ metrics) {
+  const int e = blockIdx.x, lane = threadIdx.x & 31;
+  const double* rows = partials + (size_t)e * 3 * n_blocks;
+  const double s1 = warp_row_sum(rows, n_blocks, lane);
+  const double s2 = warp_row_sum(rows + n_blocks, n_blocks, lane);
+  const double cn = warp_row_sum(rows + 2 * (size_t)n_blocks, n_blocks, lane);
+  if (lane == 0) {
+    const double mfb = cn > 0.0 ? s1 / cn : 0.0;
+    metrics[4 * e + 0] = cn;
+    metrics[4 * e + 1] = mfb;
+    metrics[4 * e + 2] = cn > 1.0 ? (s2 - cn * mfb * mfb) / (cn - 1.0) : 0.0;
+    metrics[4 * e + 3] = s2;
   }
 }
 

@@ -220,6 +220,43 @@ def test_polynomial_background_eq18(dia, d, c, n, m):
     h.close()
 
 
+@pytest.mark.parametrize("c,n,m,d", [(0, None, None, 0), (3, 300, 11, 0), (4, 333, 19, 2), (1, 400, 15, 0)])
+def test_difference_image_and_metrics(dia, c, n, m, d):
+    """dia_difference_image: D = I - M element by element (float32 model against the FP64 oracle) and the
+    fit-quality metrics MFB / MFV / chi^2 (Eq. 29-30), with flat + mask (c3), a polynomial
+    background and the cp.async path (c4 at odd n), and after a real fit (c0)."""
+    w = make_workload(c, n=n, m=m, n_epochs=2 if c == 4 else None)
+    nb = (d + 1) * (d + 2) // 2
+    h = _handle(dia, w, bg_degree=d)
+    cfg = _ref_cfg(w, bg_degree=d)
+    th = w.theta_true.astype(np.float32)
+    if d > 0:
+        rng = np.random.default_rng(1)
+        th = np.concatenate([th, rng.normal(0, 4.0, (w.n_epochs, nb - 1)).astype(np.float32)], axis=1)
+    if c == 0:                                   # difference image at the fitted parameters
+        thg, _ = h.fit(_dev(w.I), _dev(w.theta0), dia.FitOpts.default())
+        th = thg.cpu().numpy()
+    D, met = h.difference_image(_dev(w.I), _dev(th), mask=_dev(w.mask))
+    D, met = D.cpu().numpy(), met.cpu().numpy()
+    hh = (w.m - 1) // 2
+    for e in range(w.n_epochs):
+        Do, mo = oracle.difference_image(cfg, w.R, w.I[e], th[e], mask=None if w.mask is None else w.mask[e])
+        Mo = w.I[e].astype(np.float64) - Do
+        # |D_gpu - D_or| against the size of the model image: float32 accumulation of M (~ 1e-6 relative)
+        err = np.abs(D[e] - Do)[hh:-hh, hh:-hh] / np.maximum(np.abs(Mo[hh:-hh, hh:-hh]), 1.0)
+        print(f"diff c{c} e{e}: max |dD|/|M| = {err.max():.2e}; N={met[e][0]:.0f} MFB={met[e][1]:.5f} ({mo[1]:.5f}) "
+              f"MFV={met[e][2]:.5f} ({mo[2]:.5f})")
+        assert err.max() <= 1e-5
+        assert np.all(D[e][:hh] == 0) and np.all(D[e][:, -hh:] == 0)          # outside the valid region
+        assert met[e][0] == mo[0]
+        assert abs(met[e][1] - mo[1]) <= 1e-5 * max(1.0, abs(mo[1]))
+        assert met[e][2] == pytest.approx(mo[2], rel=1e-5) and met[e][3] == pytest.approx(mo[3], rel=1e-5)
+    if c == 0:      # a converged fit of simulated data: MFB ~ 0, MFV ~ 1 - (m^2+1)/N (Table 2, PAPER.md:427)
+        N = (w.n - w.m + 1) ** 2
+        assert abs(met[0][1]) < 4 / np.sqrt(N) and abs(met[0][2] - (1 - 50 / N)) < 4 * np.sqrt(2 / N)
+    h.close()
+
+
 def test_emccd_noise_model_eq7(dia):
     """EMCCD noise model, Eq. 7: sigma^2 = E M / (G_total F) with E = 2, G_total = 25.8/300
     e-/ADU -- the affine form of Eq. 6 with no read-noise term, i.e. sigma0 = 0 and gain = G_total / E."""

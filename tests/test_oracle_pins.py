@@ -314,3 +314,29 @@ def test_polynomial_background_model_and_gradient(d):
     th0 = np.concatenate([K.ravel(), b[:1]])
     b1 = b.copy(); b1[1:] = 0
     assert np.array_equal(oracle.model(cfg0, R, th0), oracle.model(cfg, R, np.concatenate([K.ravel(), b1])))
+
+
+# ---------------------------------------------------------------- difference image and fit-quality metrics
+def test_difference_image_and_mfb_mfv():
+    """D = I - M; MFB, MFV of Eq. 29-30 against numpy mean / var(ddof = 1) of
+    eps = D / sigma with sigma from Eq. 6 at the model.  Catches N vs N-1, a missing mask, sigma vs sigma^2 and
+    a difference image written outside the valid region."""
+    n, m, h = 14, 3, 1
+    R, I, th = _rand_problem(n, m, seed=9)
+    rng = np.random.default_rng(2)
+    flat = (0.9 + 0.2 * rng.random((n, n))).astype(np.float32)
+    mask = (rng.random((n, n)) > 0.2).astype(np.uint8)
+    cfg = oracle.RefConfig(n, n, m, sigma0=4.0, gain=1.7, flat=flat)
+    D, met = oracle.difference_image(cfg, R, I, th, mask=mask)
+    K = th[:-1].astype(np.float64).reshape(m, m)
+    M = scipy.signal.correlate2d(R.astype(np.float64), K, mode="valid") + float(th[-1])
+    Dn = np.zeros((n, n)); Dn[h:-h, h:-h] = I.astype(np.float64)[h:-h, h:-h] - M
+    assert np.allclose(D, Dn, rtol=0, atol=1e-10) and np.all(D[0] == 0) and np.all(D[:, -1] == 0)
+    F = flat.astype(np.float64)[h:-h, h:-h]
+    sig = np.sqrt(16.0 / F ** 2 + M / (1.7 * F))
+    use = mask[h:-h, h:-h] == 1
+    eps = (Dn[h:-h, h:-h] / sig)[use]
+    assert met[0] == eps.size
+    assert met[1] == pytest.approx(eps.mean(), rel=1e-12)
+    assert met[2] == pytest.approx(eps.var(ddof=1), rel=1e-12)
+    assert met[3] == pytest.approx((eps ** 2).sum(), rel=1e-12)
