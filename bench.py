@@ -184,6 +184,47 @@ def stamp_batch_rate(dia, dev, n_stamps=296, n=142, m=19):
             "note": "one reference per epoch (dia_config.n_refs == max_epochs), one launch sequence for the batch"}
 
 
+def other_configs(dia, dev):
+    """BASELINE configs[0..3] (parity-test shapes): evaluations/s of a stand-alone dia_eval_loss_grad and one
+    free-running fit with the paper's settings, for context beside the headline workload."""
+    import torch
+    from workloads import make_workload
+    out = []
+    for c in (0, 1, 2, 3):
+        w = make_workload(c)
+        to = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        loss_kind = dia.LOSS_HUBER if w.loss == "huber" else dia.LOSS_GAUSSIAN
+        h = dia.Handle(to(w.R), w.m, max_epochs=1, loss=loss_kind, sigma0=w.sigma0, gain=w.gain, flat=to(w.flat))
+        I, th0, mk = to(w.I), to(w.theta0), to(w.mask)
+        L = torch.empty(1, dtype=torch.float64, device=dev)
+        G = torch.empty((1, w.m * w.m + 1), dtype=torch.float64, device=dev)
+        for _ in range(5):
+            h.eval_loss_grad(I, th0, mask=mk, loss=L, grad=G)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(50):
+            h.eval_loss_grad(I, th0, mask=mk, loss=L, grad=G)
+        b.record()
+        torch.cuda.synchronize()
+        ms_eval = a.elapsed_time(b) / 50
+        opts = dia.FitOpts.default()
+        h.fit(I, th0, opts, mask=mk)
+        torch.cuda.synchronize()
+        a.record()
+        _, res = h.fit(I, th0, opts, mask=mk)
+        b.record()
+        torch.cuda.synchronize()
+        ms_fit = a.elapsed_time(b)
+        h.close()
+        out.append({"config": c, "n": w.n, "m": w.m, "loss": w.loss, "evals_per_s": 1e3 / ms_eval,
+                    "us_per_eval": 1e3 * ms_eval, "frac_fp32_nominal": 2.0 * useful_fma(w.n, w.m) / (ms_eval * 1e-3) / 1e12 /
+                    (SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9 / 1e12),
+                    "fits_per_s": 1e3 / ms_fit, "ms_per_fit": ms_fit, "n_adam": res[0].n_adam, "n_lbfgs": res[0].n_lbfgs,
+                    "status": res[0].status, "photometric_scale": round(res[0].photometric_scale, 5)})
+    return out
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on the host cores, rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
@@ -348,6 +389,7 @@ def run_gpu(args):
     # ---- many small image pairs, one reference each (the paper's stamp workloads)
     if rank == 0 and not args.no_stamps:
         line["stamps"] = stamp_batch_rate(dia, dev)
+        line["other_configs"] = other_configs(dia, dev)
 
     # ---- the oracle beside it (rank 0, N = 1 only)
     if rank == 0 and world == 1 and not args.no_cpu:

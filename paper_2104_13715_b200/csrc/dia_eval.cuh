@@ -139,12 +139,6 @@ __device__ __forceinline__ unsigned long long l2_policy_evict_first() {
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol));
   return pol;
 }
-__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* tm, int x, int y, unsigned bar,
-                                            unsigned long long pol) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;\n" ::
-          "r"(dst), "l"(tm), "r"(x), "r"(y), "r"(bar), "l"(pol) : "memory");
-}
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* tm, int x, int y, int z, unsigned bar,
                                             unsigned long long pol) {
   asm volatile(
