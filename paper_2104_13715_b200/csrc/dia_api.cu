@@ -163,7 +163,8 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
   p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
   p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;  p->n_refs = h->n_refs;
-  p->np = h->np;  p->part_rows = h->np + 1;  p->diff = nullptr;  p->bg_degree = c.bg_degree;            // Eq. 19: centre ((N-1)/2), normalisation N (R18)
+  p->np = h->np;  p->part_rows = h->np + 1;  p->diff = nullptr;  p->bg_degree = c.bg_degree;
+  // Eq. 19: centre ((N-1)/2), normalisation N (R18)
   p->bg_xc = 0.5f * (float)(c.n_cols - 1);  p->bg_yc = 0.5f * (float)(c.n_rows - 1);
   p->bg_inv_nx = 1.0f / (float)c.n_cols;  p->bg_inv_ny = 1.0f / (float)c.n_rows;
   p->tiles_x = (c.n_cols - c.m + 1 + dia::kTW - 1) / dia::kTW;
@@ -218,7 +219,7 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
     int o = 0;
     ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, dia::kThreads, h->smem);
     if (ce != cudaSuccess || o < 1) { int rc = cuda_fail(nullptr, ce, "occupancy query"); delete h; return rc; }
-    occ = (aux == 0 || o < occ) ? o : occ;   // one grid size for both variants
+    occ = (aux == 0 || o < occ) ? o : occ;   // one grid size for all variants
   }
   h->use_tma = 0;
   const char* no_tma = std::getenv("DIA_DISABLE_TMA");   // test hook: force the cp.async staging path
@@ -314,8 +315,9 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   dia::TensorMaps tm;
   fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
   std::string err;
-    const int unroll = 4;      // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
-  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid(h, n_epochs), dia::eval_part_cols(h, n_epochs), unroll, h->cfg.m, lambda_n(h), h->stream, &err);
+  const int unroll = 4;        // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
+  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid(h, n_epochs),
+                    dia::eval_part_cols(h, n_epochs), unroll, h->cfg.m, lambda_n(h), h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
   return DIA_OK;
 }
@@ -334,6 +336,6 @@ extern "C" int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_
   if (grid_blocks) *grid_blocks = h->grid;
   if (threads_per_block) *threads_per_block = dia::kThreads;
   if (smem_bytes) *smem_bytes = (int)h->smem;
-  if (launches_per_eval) *launches_per_eval = 2;
+  if (launches_per_eval) *launches_per_eval = h->cfg.lambda_reg > 0.f ? 3 : 2;   // eval, reduce (, penalty)
   return DIA_OK;
 }
