@@ -5,6 +5,8 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <atomic>
+#include <cstddef>
 #include <cstring>
 #include <new>
 #include <string>
@@ -19,6 +21,7 @@ struct dia_handle {
   cudaStream_t stream;
   int grid, np, sms;       // grid: resident CTAs (SMs x occupancy), capped by max_epochs x tiles
   int tiles, n_refs;
+  dia::ConstBlock* d_const_stage;   // staging copy of the constant block; non-null iff this handle owns the bank
   size_t smem;
   int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
   CUtensorMap tmR;         // valid iff use_tma
@@ -28,6 +31,9 @@ struct dia_handle {
 };
 
 static thread_local std::string g_create_err;
+// The constant bank (dia::c_blk) is one per process: the first handle that can use it owns it until destroyed;
+// other handles run the shared-memory variant of the kernel.
+static std::atomic<dia_handle*> g_const_owner{nullptr};
 
 static int fail(dia_handle* h, int code, const std::string& msg) {
   if (h) h->err = msg; else g_create_err = msg;
@@ -84,11 +90,12 @@ static void geometry_for(int m, int* rpitch, int* rh) {
 }
 // aux = true: mask / flat field / caller variance map present (read from global memory per pixel);
 // diff = true: difference-image instantiation (forward only, generic per-pixel inputs)
-static const void* kernel_for(int m, bool aux, bool diff = false) {
+static const void* kernel_for(int m, bool aux, bool diff = false, bool kc = false) {
   switch (m) {
 #define X(MM) case MM: return diff ? (const void*)dia::eval_kernel<MM, true, true>                    \
                                    : aux ? (const void*)dia::eval_kernel<MM, true, false>             \
-                                         : (const void*)dia::eval_kernel<MM, false, false>;
+                                         : kc ? (const void*)dia::eval_kernel<MM, false, false, true> \
+                                              : (const void*)dia::eval_kernel<MM, false, false>;
     DIA_FOR_EACH_M(X)
 #undef X
   }
@@ -143,9 +150,29 @@ int eval_part_cols(const dia_handle* h, int n_epochs) {
   const int g = eval_grid(h, n_epochs);
   return h->tiles < g ? h->tiles : g;
 }
+// Constant-bank variant: plain objective (no mask / flat / variance map), large images, few enough epochs.
+bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff) {
+  const int kp = (h->cfg.m + 3) / 4 * 4;
+  return h->d_const_stage && !diff && !eval_is_aux(p) && h->tiles >= 64 && p.n_epochs <= kConstEpochs &&
+         (long long)p.n_epochs * h->cfg.m * kp <= kConstK;
+}
+size_t const_block_bytes(const dia_handle* h, int n_epochs) {
+  const int kp = (h->cfg.m + 3) / 4 * 4;
+  return offsetof(ConstBlock, K) + sizeof(float) * (size_t)n_epochs * h->cfg.m * kp;
+}
+const void* eval_kernel_ptr_kc(const dia_handle* h) { return kernel_for(h->cfg.m, false, false, true); }
+ConstBlock* const_stage(const dia_handle* h) { return h->d_const_stage; }
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff) {
   void* args[] = {(void*)&p, (void*)&tm};
-  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), diff), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
+  const bool kc = eval_uses_const(h, p, diff);
+  if (kc) {      // refresh the constant block from theta (and the done flags) first, stream-ordered
+    const int kp = (h->cfg.m + 3) / 4 * 4;
+    pack_const_kernel<<<1, 256, 0, h->stream>>>(p.theta, p.done, p.n_epochs, p.np, h->cfg.m, kp, h->d_const_stage);
+    cudaError_t ce = cudaMemcpyToSymbolAsync(c_blk, h->d_const_stage, const_block_bytes(h, p.n_epochs), 0,
+                                             cudaMemcpyDeviceToDevice, h->stream);
+    if (ce != cudaSuccess) return ce;
+  }
+  return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), diff, kc), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
                           h->smem, h->stream);
 }
 }  // namespace dia
@@ -210,10 +237,11 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   h->n_refs = cfg->n_refs > 1 ? cfg->n_refs : 1;
   h->cfg = *cfg;  h->d_R = d_R;  h->stream = (cudaStream_t)cfg->stream;  h->sms = sms;
   h->np = cfg->m * cfg->m + (cfg->bg_degree + 1) * (cfg->bg_degree + 2) / 2;  h->smem = smem_for(cfg->m);  h->d_partials = nullptr;
+  h->d_const_stage = nullptr;
 
   int occ = 0;
-  for (int aux = 0; aux < 3; ++aux) {        // the two evaluation variants and the difference-image variant
-    const void* k = kernel_for(cfg->m, aux != 0, aux == 2);
+  for (int aux = 0; aux < 4; ++aux) {        // evaluation (plain, generic), difference image, constant-bank variant
+    const void* k = kernel_for(cfg->m, aux == 1 || aux == 2, aux == 2, aux == 3);
     ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
     if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
     int o = 0;
@@ -238,8 +266,23 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   }
   ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * (tiles < h->grid ? tiles : h->grid) * (h->np + 1));
   if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
+  const char* no_const = std::getenv("DIA_DISABLE_CONST");   // test hook: force the shared-memory variant
+  if (tiles >= 64 && !(no_const && no_const[0] == '1')) {   // large images: try to take the constant bank
+    dia_handle* expected = nullptr;
+    if (g_const_owner.compare_exchange_strong(expected, h)) {
+      if (cudaMalloc(&h->d_const_stage, sizeof(dia::ConstBlock)) != cudaSuccess) {
+        cudaGetLastError();  h->d_const_stage = nullptr;  g_const_owner.store(nullptr);
+      }
+    }
+  }
   int rc = dia::fit_workspace_create(&h->fit, cfg->max_epochs, h->np);
-  if (rc != DIA_OK) { cudaFree(h->d_partials); fail(nullptr, rc, "fit workspace allocation failed"); delete h; return rc; }
+  if (rc != DIA_OK) {
+    cudaFree(h->d_partials);
+    if (h->d_const_stage) { cudaFree(h->d_const_stage); g_const_owner.store(nullptr); }
+    fail(nullptr, rc, "fit workspace allocation failed");
+    delete h;
+    return rc;
+  }
   *out = h;
   return DIA_OK;
 }
@@ -249,6 +292,11 @@ extern "C" int dia_destroy(dia_handle* h) {
   cudaStreamSynchronize(h->stream);
   dia::fit_workspace_destroy(&h->fit);
   cudaFree(h->d_partials);
+  if (h->d_const_stage) {
+    cudaFree(h->d_const_stage);
+    dia_handle* me = h;
+    g_const_owner.compare_exchange_strong(me, nullptr);
+  }
   delete h;
   return DIA_OK;
 }

@@ -24,6 +24,10 @@ constexpr int kMaxPerThread = 4;      // ceil((31*31+1) / 256)
 inline bool eval_is_aux(const EvalParams& p) { return p.mask || p.flat || p.var || p.noise_kind != 0; }
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff = false);
 const void* eval_kernel_ptr(const dia_handle* h, bool aux);
+bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff);
+size_t const_block_bytes(const dia_handle* h, int n_epochs);
+const void* eval_kernel_ptr_kc(const dia_handle* h);
+ConstBlock* const_stage(const dia_handle* h);
 size_t eval_smem_bytes(const dia_handle* h);
 
 enum { PH_ADAM = 0, PH_LBFGS = 1, PH_DONE = 2 };
@@ -479,7 +483,9 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     TensorMaps tme = tm;
     void* eval_args[] = {(void*)&pe, (void*)&tme};
     cudaKernelNodeParams ke = {};
-    ke.func = (void*)eval_kernel_ptr(h, eval_is_aux(p)); ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
+    const bool kc = eval_uses_const(h, p, false);
+    ke.func = kc ? (void*)eval_kernel_ptr_kc(h) : (void*)eval_kernel_ptr(h, eval_is_aux(p));
+    ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
     ke.sharedMemBytes = (unsigned)eval_smem_bytes(h); ke.kernelParams = eval_args; ke.extra = nullptr;
     StepArgs sa;
     sa.b = w->b; sa.partials = p.partials; sa.n_blocks = part_cols; sa.np = w->np; sa.hist_cap = w->hist_cap;
@@ -492,9 +498,25 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     // The body holds `unroll` (eval ; step) pairs: re-evaluating the WHILE condition costs several
     // microseconds, which matters when an evaluation takes ~10 us (small images).  Pairs that run after
     // every epoch has stopped find done[e] set and return at once.
+    // constant-bank variant: refresh the constant block (active epochs, kernel pixels) before every evaluation
+    const float* pk_theta = p.theta;  const int* pk_done = p.done;
+    int pk_ne = n_epochs, pk_np = w->np, pk_m = m, pk_kp = (m + 3) / 4 * 4;
+    ConstBlock* pk_dst = const_stage(h);
+    void* pack_args[] = {(void*)&pk_theta, (void*)&pk_done, (void*)&pk_ne, (void*)&pk_np, (void*)&pk_m, (void*)&pk_kp,
+                         (void*)&pk_dst};
+    cudaKernelNodeParams kpk = {};
+    kpk.func = (void*)pack_const_kernel; kpk.gridDim = dim3(1); kpk.blockDim = dim3(256);
+    kpk.sharedMemBytes = 0; kpk.kernelParams = pack_args; kpk.extra = nullptr;
     cudaGraphNode_t prev = nullptr;
     for (int u = 0; u < unroll; ++u) {
       cudaGraphNode_t n_eval, n_step;
+      if (kc) {
+        cudaGraphNode_t n_pack, n_copy;
+        DIA_CU(cudaGraphAddKernelNode(&n_pack, body, prev ? &prev : nullptr, prev ? 1 : 0, &kpk));
+        DIA_CU(cudaGraphAddMemcpyNodeToSymbol(&n_copy, body, &n_pack, 1, c_blk, pk_dst, const_block_bytes(h, n_epochs), 0,
+                                              cudaMemcpyDeviceToDevice));
+        prev = n_copy;
+      }
       DIA_CU(cudaGraphAddKernelNode(&n_eval, body, prev ? &prev : nullptr, prev ? 1 : 0, &ke));
       DIA_CU(cudaGraphAddKernelNode(&n_step, body, &n_eval, 1, &ks));
       prev = n_step;

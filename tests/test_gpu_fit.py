@@ -248,6 +248,25 @@ def test_fit_polynomial_background(dia):
     h.close()
 
 
+def test_fit_constant_bank_graph_matches_shared_memory_graph(dia, monkeypatch):
+    """dia_fit on a large image refreshes the constant block inside the graph before every evaluation (pack
+    kernel + device-to-device copy to the symbol) and drops finished epochs from it; the result must equal the
+    shared-memory variant bit for bit, epochs finishing at different iterations included."""
+    w = make_workload(4, n=600, n_epochs=3, m=9)           # 10 x 10 tiles
+    og = dia.FitOpts.default(max_adam_iters=400, max_lbfgs_iters=40)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=3, sigma0=w.sigma0, gain=w.gain)
+    thc, rc = h.fit(_dev(w.I), _dev(w.theta0), og)
+    h.close()
+    monkeypatch.setenv("DIA_DISABLE_CONST", "1")
+    h2 = dia.Handle(_dev(w.R), w.m, max_epochs=3, sigma0=w.sigma0, gain=w.gain)
+    ths, rs = h2.fit(_dev(w.I), _dev(w.theta0), og)
+    h2.close()
+    assert torch.equal(thc, ths)
+    for a, b in zip(rc, rs):
+        assert (a.n_adam, a.n_lbfgs, a.n_evals, a.status, a.loss) == (b.n_adam, b.n_lbfgs, b.n_evals, b.status, b.loss)
+    assert len({r.n_evals for r in rc}) > 1                 # the epochs did stop at different iterations
+
+
 def test_fit_huber_with_cosmic_rays(dia):
     """BASELINE config 2 shape at reduced size: robust objective, 0.1 % cosmic-ray hits, no mask."""
     w = make_workload(2, n=200, m=9)

@@ -283,6 +283,28 @@ def test_emccd_noise_model_eq7(dia):
         h.close()
 
 
+def test_constant_bank_variant_matches_shared_memory_variant(dia, monkeypatch):
+    """Large images evaluate with the kernel pixels in the constant bank (uniform-register operands); the
+    shared-memory variant (test hook DIA_DISABLE_CONST, or a second live handle, which cannot own the bank)
+    must give the same bits, and both must match the oracle.  Batch of 3 epochs, one of them twice."""
+    w = make_workload(4, n=640, n_epochs=3, m=19)          # 10 x 10 = 100 tiles >= 64
+    th = w.theta_true.astype(np.float32)
+    cfg = _ref_cfg(w)
+    Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, want_scale=True)
+    h = _handle(dia, w)                                    # owns the constant bank
+    Lc, gc = h.eval_loss_grad(_dev(w.I), _dev(th))
+    _compare(Lc, gc, Lo, go, So, "S", "const bank")
+    h2 = _handle(dia, w)                                   # second live handle: shared-memory variant
+    L2, g2 = h2.eval_loss_grad(_dev(w.I), _dev(th))
+    assert torch.equal(Lc, L2) and torch.equal(gc, g2)
+    h.close(); h2.close()
+    monkeypatch.setenv("DIA_DISABLE_CONST", "1")
+    h3 = _handle(dia, w)
+    L3, g3 = h3.eval_loss_grad(_dev(w.I), _dev(th))
+    assert torch.equal(Lc, L3) and torch.equal(gc, g3)
+    h3.close()
+
+
 def test_rectangular_image(dia):
     w = make_workload(1, n=200, m=9)
     R, I = w.R[:137, :], w.I[:, :137, :]
