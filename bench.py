@@ -45,7 +45,7 @@ UNIT = "evals/s"
 SM_COUNT, FP32_LANES_PER_SM = 148, 128          # B200 (B200_PROFILING.md: 148 SMs; 128 FP32 lanes per SM)
 # dram__bytes_read.sum + dram__bytes_write.sum of one eval_kernel<19,false> launch over the 16-epoch batch,
 # from the ncu --set full capture summarised in profiles/ (None until captured)
-TRAFFIC_BYTES_PER_LAUNCH = 1.413e9     # profiles/r01_eval_kernel_full.md
+TRAFFIC_BYTES_PER_LAUNCH = 1.430e9     # profiles/r01_eval_kernel_full.md
 
 
 def useful_fma(n=N, m=M, epochs=1):
@@ -319,7 +319,8 @@ def run_gpu(args):
     iters = max(r.n_evals for r in res)
     total_evals = evals_per_step_rank * world          # every rank runs the same lock-step counts
     value = total_evals * args.steps / (ms * 1e-3)
-    launches = args.steps * (1 + 2 * iters)            # fit_init + (eval_kernel, fit_step_kernel) per iteration
+    lpe = h.info()["launches_per_eval"]                # (pack_const,) eval_kernel, fit_step_kernel per iteration
+    launches = args.steps * (1 + lpe * iters)          # + fit_init_kernel once per fit
 
     # ---- end to end through host buffers
     for _ in range(max(1, args.warmup // 2)):

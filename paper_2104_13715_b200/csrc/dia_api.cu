@@ -384,6 +384,13 @@ extern "C" int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_
   if (grid_blocks) *grid_blocks = h->grid;
   if (threads_per_block) *threads_per_block = dia::kThreads;
   if (smem_bytes) *smem_bytes = (int)h->smem;
-  if (launches_per_eval) *launches_per_eval = h->cfg.lambda_reg > 0.f ? 3 : 2;   // eval, reduce (, penalty)
+  // kernels per stand-alone evaluation of the plain objective: (pack,) eval, reduce (, penalty); a dia_fit
+  // iteration launches the same number (its step kernel takes the place of the reduce kernel)
+  if (launches_per_eval) {
+    const int kp = (h->cfg.m + 3) / 4 * 4;
+    const bool kc = h->d_const_stage && !h->cfg.d_flat && h->cfg.noise == DIA_NOISE_MODEL && h->tiles >= 64 &&
+                    h->cfg.max_epochs <= dia::kConstEpochs && (long long)h->cfg.max_epochs * h->cfg.m * kp <= dia::kConstK;
+    *launches_per_eval = 2 + (kc ? 1 : 0) + (h->cfg.lambda_reg > 0.f ? 1 : 0);
+  }
   return DIA_OK;
 }
