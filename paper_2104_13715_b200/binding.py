@@ -251,26 +251,50 @@ class Handle:
         return torch.cuda.stream(self.stream) if self.stream is not None else torch.cuda.stream(torch.cuda.current_stream())
 
     def fit_host(self, I_host: torch.Tensor, theta0_host: torch.Tensor, opts: Optional[FitOpts] = None,
-                 mask_host: Optional[torch.Tensor] = None):
+                 mask_host: Optional[torch.Tensor] = None, chunks: Optional[int] = None):
         """dia_fit with HOST inputs and outputs (pinned tensors make the copies asynchronous): copies I, theta0
         (and the mask) to the device, fits, copies theta-hat and the result structs back and synchronises.
+        The batch is cut into `chunks` groups of epochs (default 4 when there are at least 8 epochs): the copy of
+        group k+1 runs on a second stream while group k is being fitted, so only the first copy is exposed.
         Returns (theta_hat [E][np] float32 host tensor, list[FitResult], bytes host->device, bytes device->host)."""
         E = 1 if I_host.dim() == 2 else I_host.shape[0]
         dev = self.R.device
         self._staging(E, dev, mask_host is not None)
         opts = opts or FitOpts.default()
+        if chunks is None:
+            chunks = 4 if E >= 8 else 1
+        chunks = max(1, min(chunks, E))
+        bounds = [(k * E) // chunks for k in range(chunks + 1)]
+        hI = I_host.reshape(self._dI.shape)
+        hth = theta0_host.reshape(E, self.np)
+        hmask = None if mask_host is None else mask_host.reshape(self._dmask.shape)
+        nres = C.sizeof(FitResult)
+        if getattr(self, "_copy_stream", None) is None:
+            self._copy_stream = torch.cuda.Stream(device=dev)
         with self._stream_ctx():
-            self._dI.copy_(I_host.reshape(self._dI.shape), non_blocking=True)
-            self._dth.copy_(theta0_host.reshape(E, self.np), non_blocking=True)
-            if mask_host is not None:
-                self._dmask.copy_(mask_host.reshape(self._dmask.shape), non_blocking=True)
-            dia_fit(self._h, opts, E, self._dI, self._dmask, None, self._dth, self._dres)
+            fit_stream = torch.cuda.current_stream()
+            self._copy_stream.wait_stream(fit_stream)            # staging buffers are free again
+            ready = []
+            with torch.cuda.stream(self._copy_stream):
+                for k in range(chunks):
+                    a, b = bounds[k], bounds[k + 1]
+                    self._dI[a:b].copy_(hI[a:b], non_blocking=True)
+                    self._dth[a:b].copy_(hth[a:b], non_blocking=True)
+                    if hmask is not None:
+                        self._dmask[a:b].copy_(hmask[a:b], non_blocking=True)
+                    ev = torch.cuda.Event()
+                    ev.record()
+                    ready.append(ev)
+            for k in range(chunks):
+                a, b = bounds[k], bounds[k + 1]
+                fit_stream.wait_event(ready[k])
+                dia_fit(self._h, opts, b - a, self._dI[a:b], None if hmask is None else self._dmask[a:b], None,
+                        self._dth[a:b], self._dres[a * nres:b * nres])
             self._hth.copy_(self._dth, non_blocking=True)
             self._hres.copy_(self._dres, non_blocking=True)
-            torch.cuda.current_stream().synchronize()
+            fit_stream.synchronize()
         raw = self._hres.numpy().tobytes()
-        n = C.sizeof(FitResult)
-        res = [FitResult.from_buffer_copy(raw[i * n:(i + 1) * n]) for i in range(E)]
+        res = [FitResult.from_buffer_copy(raw[i * nres:(i + 1) * nres]) for i in range(E)]
         h2d = self._dI.numel() * 4 + self._dth.numel() * 4 + (self._dmask.numel() if mask_host is not None else 0)
         d2h = self._hth.numel() * 4 + self._hres.numel()
         return self._hth, res, h2d, d2h

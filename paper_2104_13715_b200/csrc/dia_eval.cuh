@@ -77,11 +77,11 @@ struct Geo {
 // constant-bank offset j * M * KP depends on uniform values only.
 constexpr int kConstEpochs = 48;                    // active epochs one launch can address
 constexpr int kConstK = 15872;                      // floats of padded kernel rows [j][M][KP]
-struct ConstBlock {
+struct alignas(16) ConstBlock {
   int n_active;                                     // epochs to evaluate in this launch
   int pad[3];
   int active[kConstEpochs];                         // epoch index of active position j
-  float K[kConstK];
+  alignas(16) float K[kConstK];
 };
 static_assert(sizeof(ConstBlock) <= 65536 - 1024, "constant bank");
 __constant__ ConstBlock c_blk;
@@ -294,8 +294,12 @@ __device__ __forceinline__ void row_chain(const float* __restrict__ Ks, int koff
   using G = Geo<M>;
   float k[G::KP], r[G::RSEG];
   if (KC) {                                          // warp-uniform loads from the constant bank
+    const float4* k4 = reinterpret_cast<const float4*>(c_blk.K + koff + a * G::KP);
 #pragma unroll
-    for (int q = 0; q < G::KP; ++q) k[q] = c_blk.K[koff + a * G::KP + q];
+    for (int q = 0; q < G::KP / 4; ++q) {
+      const float4 v = k4[q];
+      k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
+    }
   } else {
     const float4* k4 = reinterpret_cast<const float4*>(Ks + a * G::KP);
 #pragma unroll

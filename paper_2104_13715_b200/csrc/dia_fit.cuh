@@ -59,10 +59,17 @@ struct FitWorkspace {
   float* d_theta32;  // alias of b.theta32 (what the eval kernel reads)
   int* d_done;
   int max_epochs, np, hist_cap;
-  cudaGraph_t graph;
-  cudaGraphExec_t exec;
-  unsigned char key[256];
-  int key_len;
+  // instantiated fit graphs, keyed by (pointers, epoch count, options); least recently used entry is replaced
+  struct CachedGraph {
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    unsigned char key[256];
+    int key_len;
+    unsigned long long last_use;
+  };
+  static constexpr int kGraphCache = 8;
+  CachedGraph cache[kGraphCache];
+  unsigned long long use_counter;
 };
 
 struct StepArgs {
@@ -435,8 +442,10 @@ inline int fit_workspace_create(FitWorkspace* w, int max_epochs, int np) {
 }
 
 inline void fit_workspace_destroy(FitWorkspace* w) {
-  if (w->exec) cudaGraphExecDestroy(w->exec);
-  if (w->graph) cudaGraphDestroy(w->graph);
+  for (auto& c : w->cache) {
+    if (c.exec) cudaGraphExecDestroy(c.exec);
+    if (c.graph) cudaGraphDestroy(c.graph);
+  }
   void* ptrs[] = {w->b.theta64, w->b.g, w->b.m1, w->b.m2, w->b.d, w->b.S, w->b.Y, w->b.rho, w->b.yy,
                   w->b.st, w->b.theta32, w->b.done, w->b.remaining};
   for (void* p : ptrs) cudaFree(p);
@@ -456,10 +465,16 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
   auto put = [&](const void* src, size_t n) { std::memcpy(key + len, src, n); len += (int)n; };
   put(&n_epochs, sizeof(int)); put(&p.I, sizeof(void*)); put(&p.mask, sizeof(void*)); put(&p.var, sizeof(void*));
   put(&d_theta, sizeof(void*)); put(&d_result, sizeof(void*)); put(&o, sizeof(o)); put(&unroll, sizeof(int)); put(&lamN, sizeof(double));
-  if (!(w->exec && len == w->key_len && std::memcmp(key, w->key, len) == 0)) {
-    if (w->exec) { cudaGraphExecDestroy(w->exec); w->exec = nullptr; }
-    if (w->graph) { cudaGraphDestroy(w->graph); w->graph = nullptr; }
-    DIA_CU(cudaGraphCreate(&w->graph, 0));
+  FitWorkspace::CachedGraph* slot = nullptr;
+  for (auto& c : w->cache)
+    if (c.exec && c.key_len == len && std::memcmp(key, c.key, len) == 0) slot = &c;
+  if (!slot) {
+    slot = &w->cache[0];
+    for (auto& c : w->cache)
+      if (!c.exec) { slot = &c; break; } else if (c.last_use < slot->last_use) slot = &c;
+    if (slot->exec) { cudaGraphExecDestroy(slot->exec); slot->exec = nullptr; }
+    if (slot->graph) { cudaGraphDestroy(slot->graph); slot->graph = nullptr; }
+    DIA_CU(cudaGraphCreate(&slot->graph, 0));
     // node 1: init
     const float* theta_in = d_theta;
     int np = w->np, ne = n_epochs;
@@ -468,15 +483,15 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     kp.func = (void*)fit_init_kernel; kp.gridDim = dim3(n_epochs); kp.blockDim = dim3(256);
     kp.sharedMemBytes = 0; kp.kernelParams = init_args; kp.extra = nullptr;
     cudaGraphNode_t n_init;
-    DIA_CU(cudaGraphAddKernelNode(&n_init, w->graph, nullptr, 0, &kp));
+    DIA_CU(cudaGraphAddKernelNode(&n_init, slot->graph, nullptr, 0, &kp));
     // node 2: WHILE
     cudaGraphConditionalHandle cond;
-    DIA_CU(cudaGraphConditionalHandleCreate(&cond, w->graph, 1, cudaGraphCondAssignDefault));
+    DIA_CU(cudaGraphConditionalHandleCreate(&cond, slot->graph, 1, cudaGraphCondAssignDefault));
     cudaGraphNodeParams cp = {};
     cp.type = cudaGraphNodeTypeConditional;
     cp.conditional.handle = cond; cp.conditional.type = cudaGraphCondTypeWhile; cp.conditional.size = 1;
     cudaGraphNode_t n_while;
-    DIA_CU(cudaGraphAddNode(&n_while, w->graph, &n_init, 1, &cp));
+    DIA_CU(cudaGraphAddNode(&n_while, slot->graph, &n_init, 1, &cp));
     cudaGraph_t body = cp.conditional.phGraph_out[0];
     // body: eval -> step
     EvalParams pe = p;
@@ -521,10 +536,11 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
       DIA_CU(cudaGraphAddKernelNode(&n_step, body, &n_eval, 1, &ks));
       prev = n_step;
     }
-    DIA_CU(cudaGraphInstantiate(&w->exec, w->graph, 0));
-    std::memcpy(w->key, key, len); w->key_len = len;
+    DIA_CU(cudaGraphInstantiate(&slot->exec, slot->graph, 0));
+    std::memcpy(slot->key, key, len); slot->key_len = len;
   }
-  DIA_CU(cudaGraphLaunch(w->exec, stream));
+  slot->last_use = ++w->use_counter;
+  DIA_CU(cudaGraphLaunch(slot->exec, stream));
   return DIA_OK;
 }
 

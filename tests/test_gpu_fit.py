@@ -267,6 +267,22 @@ def test_fit_constant_bank_graph_matches_shared_memory_graph(dia, monkeypatch):
     assert len({r.n_evals for r in rc}) > 1                 # the epochs did stop at different iterations
 
 
+def test_fit_host_chunked_pipeline_matches_device_fit(dia):
+    """Handle.fit_host cuts the batch into groups whose host->device copies overlap the fit of the previous
+    group; the fitted parameters must equal those of one device-resident dia_fit over the whole batch."""
+    w = make_workload(4, n=200, n_epochs=9, m=7)
+    og = dia.FitOpts.default(force_adam_iters=40, force_lbfgs_iters=10)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=9, sigma0=w.sigma0, gain=w.gain)
+    thd, rd = h.fit(_dev(w.I), _dev(w.theta0), og)
+    hI, hth = torch.from_numpy(w.I).pin_memory(), torch.from_numpy(w.theta0).pin_memory()
+    for chunks in (None, 1, 3, 9):
+        thh, rh, h2d, d2h = h.fit_host(hI, hth, og, chunks=chunks)
+        assert torch.equal(thh, thd.cpu())
+        assert [r.n_evals for r in rh] == [r.n_evals for r in rd] and [r.loss for r in rh] == [r.loss for r in rd]
+        assert h2d == w.I.nbytes + w.theta0.nbytes
+    h.close()
+
+
 def test_fit_huber_with_cosmic_rays(dia):
     """BASELINE config 2 shape at reduced size: robust objective, 0.1 % cosmic-ray hits, no mask."""
     w = make_workload(2, n=200, m=9)
