@@ -88,14 +88,28 @@ static void geometry_for(int m, int* rpitch, int* rh) {
 #undef X
   }
 }
+// The kernel instantiations live in one translation unit per m (dia_eval_inst.cu); each exports its kernels and
+// the host shadow of its own constant block.
+namespace dia {
+#define X(MM) const void* eval_kernel_ptr_m##MM(int variant); const void* const_symbol_m##MM();
+DIA_FOR_EACH_M(X)
+#undef X
+}  // namespace dia
+
 // aux = true: mask / flat field / caller variance map present (read from global memory per pixel);
-// diff = true: difference-image instantiation (forward only, generic per-pixel inputs)
+// diff = true: difference-image instantiation; kc = true: kernel pixels in the constant bank
 static const void* kernel_for(int m, bool aux, bool diff = false, bool kc = false) {
+  const int variant = diff ? 2 : aux ? 1 : kc ? 3 : 0;
   switch (m) {
-#define X(MM) case MM: return diff ? (const void*)dia::eval_kernel<MM, true, true>                    \
-                                   : aux ? (const void*)dia::eval_kernel<MM, true, false>             \
-                                         : kc ? (const void*)dia::eval_kernel<MM, false, false, true> \
-                                              : (const void*)dia::eval_kernel<MM, false, false>;
+#define X(MM) case MM: return dia::eval_kernel_ptr_m##MM(variant);
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return nullptr;
+}
+static const void* const_symbol_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::const_symbol_m##MM();
     DIA_FOR_EACH_M(X)
 #undef X
   }
@@ -162,13 +176,14 @@ size_t const_block_bytes(const dia_handle* h, int n_epochs) {
 }
 const void* eval_kernel_ptr_kc(const dia_handle* h) { return kernel_for(h->cfg.m, false, false, true); }
 ConstBlock* const_stage(const dia_handle* h) { return h->d_const_stage; }
+const void* const_symbol(const dia_handle* h) { return const_symbol_for(h->cfg.m); }
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff) {
   void* args[] = {(void*)&p, (void*)&tm};
   const bool kc = eval_uses_const(h, p, diff);
   if (kc) {      // refresh the constant block from theta (and the done flags) first, stream-ordered
     const int kp = (h->cfg.m + 3) / 4 * 4;
     pack_const_kernel<<<1, 256, 0, h->stream>>>(p.theta, p.done, p.n_epochs, p.np, h->cfg.m, kp, h->d_const_stage);
-    cudaError_t ce = cudaMemcpyToSymbolAsync(c_blk, h->d_const_stage, const_block_bytes(h, p.n_epochs), 0,
+    cudaError_t ce = cudaMemcpyToSymbolAsync(const_symbol_for(h->cfg.m), h->d_const_stage, const_block_bytes(h, p.n_epochs), 0,
                                              cudaMemcpyDeviceToDevice, h->stream);
     if (ce != cudaSuccess) return ce;
   }

@@ -84,7 +84,7 @@ struct alignas(16) ConstBlock {
   alignas(16) float K[kConstK];
 };
 static_assert(sizeof(ConstBlock) <= 65536 - 1024, "constant bank");
-__constant__ ConstBlock c_blk;
+static __constant__ ConstBlock c_blk;      // one copy per translation unit (per kernel size), see dia_eval_inst.cu
 
 struct EvalParams {
   const float* R;            // [n_refs][n_rows][n_cols]
@@ -721,6 +721,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   if (cur_j >= 0) finish_epoch();
 }
 
+#ifndef DIA_INST_M      // the small stand-alone kernels belong to the API translation unit only
 // Fixed-order sum of one row of block partials by one warp: lane l adds columns l, l+32, ... in order,
 // then the 32 lane sums are combined by a fixed butterfly -- deterministic for a given n_blocks.
 __device__ __forceinline__ double warp_row_sum(const double* __restrict__ row, int n_blocks, int lane) {
@@ -782,5 +783,7 @@ __global__ void pack_const_kernel(const float* __restrict__ theta, const int* __
     dst->K[idx] = (b < m) ? theta[(size_t)s_active[j] * np + a * m + b] : 0.f;
   }
 }
+
+#endif  // DIA_INST_M
 
 }  // namespace dia

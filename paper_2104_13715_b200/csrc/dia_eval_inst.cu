@@ -1,0 +1,31 @@
+// dia_eval_inst.cu -- one translation unit per kernel size: compiled once for every odd m with
+// -DDIA_INST_M=<m> (paper_2104_13715_b200/build.py runs these compilations in parallel).  Each unit holds the
+// four instantiations of the fused kernel for its m and its own copy of the constant block, and exports two
+// accessors that dia_api.cu uses to launch the kernels and to address the constant symbol.
+#include "dia_eval.cuh"
+
+#ifndef DIA_INST_M
+#error "compile with -DDIA_INST_M=<odd kernel size>"
+#endif
+
+#define DIA_CAT2(a, b) a##b
+#define DIA_CAT(a, b) DIA_CAT2(a, b)
+
+namespace dia {
+
+// variant: 0 = plain objective, 1 = generic (mask / flat / variance map), 2 = difference image,
+//          3 = plain objective with the kernel pixels in the constant bank
+const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
+  switch (variant) {
+    case 0: return (const void*)eval_kernel<DIA_INST_M, false, false, false>;
+    case 1: return (const void*)eval_kernel<DIA_INST_M, true, false, false>;
+    case 2: return (const void*)eval_kernel<DIA_INST_M, true, true, false>;
+    case 3: return (const void*)eval_kernel<DIA_INST_M, false, false, true>;
+  }
+  return nullptr;
+}
+
+// host shadow of this unit's constant block (what cudaMemcpyToSymbol / graph memcpy nodes take)
+const void* DIA_CAT(const_symbol_m, DIA_INST_M)() { return (const void*)&c_blk; }
+
+}  // namespace dia

@@ -28,6 +28,7 @@ bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff);
 size_t const_block_bytes(const dia_handle* h, int n_epochs);
 const void* eval_kernel_ptr_kc(const dia_handle* h);
 ConstBlock* const_stage(const dia_handle* h);
+const void* const_symbol(const dia_handle* h);
 size_t eval_smem_bytes(const dia_handle* h);
 
 enum { PH_ADAM = 0, PH_LBFGS = 1, PH_DONE = 2 };
@@ -528,7 +529,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
       if (kc) {
         cudaGraphNode_t n_pack, n_copy;
         DIA_CU(cudaGraphAddKernelNode(&n_pack, body, prev ? &prev : nullptr, prev ? 1 : 0, &kpk));
-        DIA_CU(cudaGraphAddMemcpyNodeToSymbol(&n_copy, body, &n_pack, 1, c_blk, pk_dst, const_block_bytes(h, n_epochs), 0,
+        DIA_CU(cudaGraphAddMemcpyNodeToSymbol(&n_copy, body, &n_pack, 1, const_symbol(h), pk_dst, const_block_bytes(h, n_epochs), 0,
                                               cudaMemcpyDeviceToDevice));
         prev = n_copy;
       }
