@@ -11,6 +11,7 @@ from .dia_ref import (  # noqa: F401
     fit,
     b08_solve,
     difference_image,
+    hessian,
     model,
     huber_Q,
     num_threads,

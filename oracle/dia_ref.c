@@ -262,6 +262,77 @@ int dia_ref_difference_image(const dia_ref_config* cfg, const float* R, const fl
   return DIA_REF_OK;
 }
 
+/* D3: second derivative of the pixel term l = rho(z) + (1/2) ln v with respect to M, with r = I - M,
+ * v = a + b' M, z = r / sqrt(v).  Gaussian: w = -r/v - b' r^2/(2 v^2) + b'/(2v), so
+ *   dw/dM = 1/v + 2 b' r / v^2 + b'^2 r^2 / v^3 - b'^2 / (2 v^2).
+ * Huber, linear branch (|z| > c, psi = +-c): w = -psi/s - psi z b'/(2v) + b'/(2v), s = sqrt v, z = r/s; with
+ * ds/dM = b'/(2s), dz/dM = -1/s - z b'/(2v):
+ *   dw/dM = psi b'/(2 s v) - psi b'/(2v) dz/dM + psi z b'^2/(2 v^2) - b'^2/(2 v^2). */
+static double pixel_d2(const dia_ref_config* cfg, double r, double v, double bp) {
+  const double sd = sqrt(v), z = r / sd;
+  if (cfg->loss == DIA_REF_LOSS_HUBER && fabs(z) > cfg->huber_c) {
+    const double psi = (z > 0.0) ? cfg->huber_c : -cfg->huber_c;
+    const double dz = -1.0 / sd - z * bp / (2.0 * v);
+    return psi * bp / (2.0 * sd * v) - psi * bp / (2.0 * v) * dz + psi * z * bp * bp / (2.0 * v * v) -
+           bp * bp / (2.0 * v * v);
+  }
+  return 1.0 / v + 2.0 * bp * r / (v * v) + bp * bp * r * r / (v * v * v) - bp * bp / (2.0 * v * v);
+}
+
+int dia_ref_hessian(const dia_ref_config* cfg, const float* R, const float* I, const unsigned char* mask,
+                    const float* var, const float* theta, double* H) {
+  if (!check_cfg(cfg) || !R || !I || !theta || !H) return DIA_REF_ERR_INVALID_ARG;
+  if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
+  const int m = cfg->m, h = (m - 1) / 2, nk = m * m, np = dia_ref_num_params(cfg), nbg = np - nk;
+  const int nr = cfg->n_rows, nc = cfg->n_cols;
+  double* X = (double*)malloc(sizeof(double) * np);
+  if (!X) return DIA_REF_ERR_ALLOC;
+  for (size_t q = 0; q < (size_t)np * np; ++q) H[q] = 0.0;
+  for (int i = h; i < nr - h; ++i)
+    for (int j = h; j < nc - h; ++j) {
+      const size_t p = (size_t)i * nc + j;
+      if (mask && mask[p] == 0) continue;
+      const double M = model_pixel(cfg, R, nc, m, theta, i, j);
+      double v, bp;
+      if (cfg->noise == DIA_REF_NOISE_MODEL) {
+        const double F = cfg->flat ? (double)cfg->flat[p] : 1.0;
+        const double b_ij = 1.0 / (cfg->gain * F);
+        v = cfg->sigma0 * cfg->sigma0 / (F * F) + b_ij * (M > 0.0 ? M : 0.0);
+        bp = (M > 0.0) ? b_ij : 0.0;
+      } else {
+        v = (double)var[p];
+        bp = 0.0;
+      }
+      const double d2 = pixel_d2(cfg, (double)I[p] - M, v, bp);
+      for (int a = 0; a < m; ++a)
+        for (int b = 0; b < m; ++b) X[a * m + b] = (double)R[(size_t)(i - h + a) * nc + (j - h + b)];
+      background(cfg, theta + nk, i, j, X + nk);
+      for (int q = 0; q < np; ++q) {
+        const double xq = d2 * X[q];
+        for (int s = q; s < np; ++s) H[(size_t)q * np + s] += xq * X[s];
+      }
+    }
+  for (int q = 0; q < np; ++q)
+    for (int s = 0; s < q; ++s) H[(size_t)q * np + s] = H[(size_t)s * np + q];
+  (void)nbg;
+  if (cfg->lambda_reg > 0.0) {           /* Eq. 20: + 2 lambda N L'L on the kernel block */
+    const double N = (double)(nr - m + 1) * (double)(nc - m + 1);
+    double* e = (double*)calloc((size_t)3 * nk, sizeof(double));
+    if (!e) { free(X); return DIA_REF_ERR_ALLOC; }
+    double* u = e + nk; double* w2 = u + nk;
+    for (int k = 0; k < nk; ++k) {
+      e[k] = 1.0;
+      laplacian_apply(m, e, u);
+      laplacian_apply(m, u, w2);
+      for (int q = 0; q < nk; ++q) H[(size_t)q * np + k] += 2.0 * cfg->lambda_reg * N * w2[q];
+      e[k] = 0.0;
+    }
+    free(e);
+  }
+  free(X);
+  return DIA_REF_OK;
+}
+
 /* Eq. 14: Q = N ln( sqrt(2 pi) erf(c/sqrt 2) + 2 exp(-c^2/2)/c ). */
 double dia_ref_huber_Q(double c, double N) {
   const double pi = 3.14159265358979323846;

@@ -79,6 +79,13 @@ int dia_ref_difference_image(const dia_ref_config* cfg, const float* R, const fl
                              const unsigned char* mask, const float* var, const float* theta,
                              double* D, double* metrics);
 
+/* Hessian of the objective at theta, H [np][np] row-major FP64 (np = dia_ref_num_params): the observed Fisher
+ * information of Eq. 15 when theta is the MLE; its inverse is the covariance of Eq. 16-17.
+ * Analytic: H = sum_V h_ij X X' (+ 2 lambda N L'L), X the design vector (shifted reference pixels, background
+ * basis) and h_ij = d^2 l_ij / dM^2 (D3).  One epoch. */
+int dia_ref_hessian(const dia_ref_config* cfg, const float* R, const float* I, const unsigned char* mask,
+                    const float* var, const float* theta, double* H);
+
 /* Adam -> L-BFGS fit (DESIGN c.2), one epoch after another.  theta in/out float32. */
 int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
                 int n_epochs, const float* I, const unsigned char* mask, const float* var,

@@ -184,6 +184,20 @@ def difference_image(cfg: RefConfig, R, I, theta, mask=None, var=None):
     return D, metrics
 
 
+def hessian(cfg: RefConfig, R, I, theta, mask=None, var=None) -> np.ndarray:
+    """-> H float64 [np][np], the Hessian of the objective at theta for one epoch."""
+    c, keep = cfg._c()
+    R, I = _f32(R), _f32(I)
+    assert I.shape == (cfg.n_rows, cfg.n_cols)
+    theta = _f32(theta).reshape(-1)
+    mask = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    var = _f32(var)
+    H = np.empty((cfg.n_params, cfg.n_params), dtype=np.float64)
+    _check(_lib().dia_ref_hessian(C.byref(c), _ptr(R), _ptr(I), _ptr(mask), _ptr(var), _ptr(theta), _ptr(H)),
+           "dia_ref_hessian")
+    return H
+
+
 def huber_Q(c: float, N: float) -> float:
     return float(_lib().dia_ref_huber_Q(float(c), float(N)))
 

@@ -268,3 +268,69 @@ def test_noisy_fit_statistics_mfv(golden):
     mfv = eps.var(ddof=1)
     assert abs(mfv - (1 - 50 / N)) < 4 * math.sqrt(2 / N)
     assert res[0].photometric_scale == pytest.approx(1.2, abs=0.02)
+
+
+# ---------------------------------------------------------------- Hessian (Eq. 15-17)
+@pytest.mark.parametrize("loss", [oracle.LOSS_GAUSSIAN, oracle.LOSS_HUBER])
+@pytest.mark.parametrize("noise_mode", [oracle.NOISE_MODEL, oracle.NOISE_FIXED])
+def test_hessian_vs_finite_differences_of_gradient(loss, noise_mode):
+    """D3: h = d^2 l/dM^2.  The paper takes the Hessian by autodiff, so the
+    derived closed form is checked against central differences of the oracle's gradient, itself pinned
+    above.  Catches a dropped or mis-signed term of dw/dM, a missing symmetrisation and a wrong
+    background-block index."""
+    R, I, th, flat = _dyadic_problem()
+    n, m = R.shape[0], 3
+    I = I.copy()
+    I[5, 6] += 400.0
+    var = (20.0 + 0.5 * I.clip(0)).astype(np.float32) if noise_mode == oracle.NOISE_FIXED else None
+    cfg = oracle.RefConfig(n, n, m, loss=loss, huber_c=1.345, noise=noise_mode, sigma0=5.0, gain=1.6,
+                           flat=flat, bg_degree=1, lambda_reg=0.3)
+    th = np.concatenate([th, [0.5, -0.25]]).astype(np.float32)
+    H = oracle.hessian(cfg, R, I, th, var=var)
+    assert np.array_equal(H, H.T)
+    fd = np.zeros_like(H)
+    for k in range(th.size):
+        step = 2.0 ** -16 if k < m * m else 2.0 ** -9
+        tp, tm = th.copy(), th.copy()
+        tp[k] += np.float32(step)
+        tm[k] -= np.float32(step)
+        assert float(tp[k]) - float(tm[k]) == 2 * step
+        _, gp = oracle.eval_loss_grad(cfg, R, I, tp, var=var)
+        _, gm = oracle.eval_loss_grad(cfg, R, I, tm, var=var)
+        fd[:, k] = (gp[0] - gm[0]) / (2 * step)
+    d = np.sqrt(np.abs(np.diag(H)))
+    assert np.abs((H - fd) / np.outer(d, d)).max() < 1e-6
+
+
+def test_hessian_vs_torch_autograd():
+    """The paper's own route: float64 autograd Hessian of Eq. 8 with Eq. 6."""
+    torch = pytest.importorskip("torch")
+    R, I, th, flat = _dyadic_problem(n=12, m=3, seed=5)
+    n, m, h = 12, 3, 1
+    s0, G = 4.0, 2.0
+    cfg = oracle.RefConfig(n, n, m, sigma0=s0, gain=G, flat=flat)
+    H = oracle.hessian(cfg, R, I, th)
+    Rt = torch.from_numpy(R.astype(np.float64))[None, None]
+    Fv = torch.from_numpy(flat.astype(np.float64))[h:n - h, h:n - h]
+    Iv = torch.from_numpy(I.astype(np.float64))[h:n - h, h:n - h]
+
+    def f(t):
+        M = torch.nn.functional.conv2d(Rt, t[:-1].reshape(1, 1, m, m))[0, 0] + t[-1]
+        var = s0 ** 2 / Fv ** 2 + M / (G * Fv)
+        return 0.5 * ((Iv - M) ** 2 / var).sum() + 0.5 * torch.log(var).sum()
+
+    ref = torch.autograd.functional.hessian(f, torch.tensor(th.astype(np.float64))).numpy()
+    assert np.abs(H - ref).max() <= 1e-11 * np.abs(ref).max()
+
+
+def test_hessian_fixed_weights_is_normal_matrix():
+    """FIXED noise, Gaussian loss: H = X' diag(1/var) X, the B08 normal matrix (PAPER.md:66-75);
+    its inverse is the textbook weighted-least-squares covariance (Eq. 16-17)."""
+    R, I, th, _ = _dyadic_problem(n=18, m=5, seed=9)
+    var = (30.0 + 0.4 * I.clip(0)).astype(np.float32)
+    cfg = oracle.RefConfig(18, 18, 5, noise=oracle.NOISE_FIXED)
+    H = oracle.hessian(cfg, R, I, th, var=var)
+    X = _design(R, 5)
+    wv = 1.0 / var.astype(np.float64)[2:-2, 2:-2].ravel()
+    ref = X.T @ (X * wv[:, None])
+    assert np.abs(H - ref).max() <= 1e-12 * np.abs(ref).max()
