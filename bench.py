@@ -386,6 +386,13 @@ def run_gpu(args):
                             "n_adam": [r.n_adam for r in res_f], "n_lbfgs": [r.n_lbfgs for r in res_f],
                             "n_evals": [r.n_evals for r in res_f], "status": [r.status for r in res_f],
                             "photometric_scale": [round(r.photometric_scale, 5) for r in res_f]}
+        # Hessian at the fitted theta of epoch 0 (Eq. 15): np rows, max_epochs rows per launch
+        h.hessian(dI[0], th_hat[0])
+        ms_h, _ = timed(lambda: h.hessian(dI[0], th_hat[0]), 1)
+        if rank == 0:
+            rows = M * M + 1
+            line["fits"]["hessian"] = {"ms": ms_h, "rows": rows, "launches": -(-rows // E),
+                                       "tflops": useful_fma(epochs=rows) * 2 / (ms_h * 1e-3) / 1e12}
 
     # ---- many small image pairs, one reference each (the paper's stamp workloads)
     if rank == 0 and not args.no_stamps:

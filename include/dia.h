@@ -121,6 +121,22 @@ int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs,
             const float* d_I, const unsigned char* d_mask, const float* d_var,
             float* d_theta, dia_fit_result* d_result);
 
+/* Hessian of the objective at theta for ONE target image: the observed Fisher information of Eq. 15
+ * when theta is the MLE; its inverse is the covariance matrix of Eq. 16-17, whose diagonal
+ * gives the parameter uncertainties (the caller inverts it and checks positive-definiteness).
+ * The paper takes second derivatives by automatic differentiation; here they are analytic like the gradient:
+ * with X the design vector of a pixel (the m*m shifted reference pixels, then the background basis) and
+ * h_ij = d^2 l_ij / dM^2 (D3), row q of H is sum_V (h_ij X_q) X -- the gradient sum of
+ * dia_eval_loss_grad with the per-pixel weight h_ij X_q in place of w_ij -- so the fused kernel computes the
+ * np rows as np "epochs" that share the target image, max_epochs rows per launch (create the handle with
+ * max_epochs >= 16 to batch them); the penalty of Eq. 20 adds 2 lambda N L'L, and H is symmetrised.
+ *   d_I [n_rows][n_cols], d_mask / d_var as in dia_eval_loss_grad for one epoch; d_theta [np] float32;
+ *   d_H [np][np] float64 DEVICE, row-major, out.
+ * The first call allocates a small workspace (synchronises once); later calls are asynchronous.  Handles created
+ * with one reference per epoch (n_refs > 1) are rejected with DIA_ERR_UNSUPPORTED. */
+int dia_hessian(dia_handle* h, const float* d_I, const unsigned char* d_mask, const float* d_var,
+                const float* d_theta, double* d_H);
+
 /* Difference image and fit-quality metrics for n_epochs targets at the given theta (the science product,
  * PAPER.md:20; metrics of Eq. 29-30):
  *   D_ij = I_ij - M_ij on the valid region V (mask or not), 0 outside V;

@@ -19,7 +19,7 @@ NOISE_MODEL, NOISE_FIXED = 0, 1
 FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
-                    "dia_measure_fp32_peak", "dia_difference_image")
+                    "dia_measure_fp32_peak", "dia_difference_image", "dia_hessian")
 
 
 class DiaError(RuntimeError):
@@ -88,6 +88,7 @@ def load_library(build_if_missing: bool = True):
                             C.c_void_p, C.c_void_p]
     lib.dia_destroy.argtypes = [C.c_void_p]
     lib.dia_difference_image.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6
+    lib.dia_hessian.argtypes = [C.c_void_p] * 6
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
     lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     _LIB = lib
@@ -154,6 +155,13 @@ def dia_difference_image(handle: int, n_epochs: int, d_I, d_mask, d_var, d_theta
                                     _dptr(d_metrics, torch.float64, "d_metrics")), handle)
 
 
+def dia_hessian(handle: int, d_I, d_mask, d_var, d_theta, d_H) -> None:
+    lib = load_library()
+    _check(lib.dia_hessian(handle, _dptr(d_I, torch.float32, "d_I"), _dptr(d_mask, torch.uint8, "d_mask"),
+                           _dptr(d_var, torch.float32, "d_var"), _dptr(d_theta, torch.float32, "d_theta"),
+                           _dptr(d_H, torch.float64, "d_H")), handle)
+
+
 def dia_destroy(handle: int) -> None:
     _check(load_library().dia_destroy(handle))
 
@@ -218,6 +226,12 @@ class Handle:
         metrics = torch.empty((E, 4), dtype=torch.float64, device=I.device)
         dia_difference_image(self._h, E, I, mask, var, theta, D, metrics)
         return D, metrics
+
+    def hessian(self, I, theta, mask=None, var=None):
+        """-> H float64 [np][np] CUDA tensor: Hessian of the objective at theta for the single target I."""
+        H = torch.empty((self.np, self.np), dtype=torch.float64, device=I.device)
+        dia_hessian(self._h, I, mask, var, theta, H)
+        return H
 
     def fit(self, I, theta0, opts: Optional[FitOpts] = None, mask=None, var=None):
         """Returns (theta_hat float32 [E][np] CUDA tensor, list[FitResult]); synchronises to read results."""

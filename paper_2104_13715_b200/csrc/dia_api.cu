@@ -13,6 +13,7 @@
 
 #include "dia_eval.cuh"
 #include "dia_fit.cuh"
+#include "dia_hess.cuh"
 #include "dia_probe.cuh"
 
 struct dia_handle {
@@ -27,6 +28,7 @@ struct dia_handle {
   CUtensorMap tmR;         // valid iff use_tma
   double* d_partials;      // [max_epochs][np+1][min(tiles, grid)]
   dia::FitWorkspace fit;   // device optimiser state + cached graph
+  dia::HessWorkspace hess; // dia_hessian scratch, allocated on first use
   std::string err;
 };
 
@@ -200,11 +202,12 @@ static double lambda_n(const dia_handle* h) {
 
 static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
                         const float* d_var, const float* d_theta, const int* d_done, dia::EvalParams* p,
-                        dia::TensorMaps* tm) {
+                        dia::TensorMaps* tm, int hess_q0 = -1) {
   const dia_config& c = h->cfg;
   p->R = h->d_R;  p->I = d_I;  p->mask = d_mask;  p->var = d_var;  p->flat = c.d_flat;
   p->theta = d_theta;  p->done = d_done;  p->partials = h->d_partials;
   p->n_rows = c.n_rows;  p->n_cols = c.n_cols;  p->n_epochs = n_epochs;  p->n_refs = h->n_refs;
+  p->hess_q0 = hess_q0;
   p->np = h->np;  p->part_rows = h->np + 1;  p->diff = nullptr;  p->bg_degree = c.bg_degree;
   // Eq. 19: centre ((N-1)/2), normalisation N (R18)
   p->bg_xc = 0.5f * (float)(c.n_cols - 1);  p->bg_yc = 0.5f * (float)(c.n_rows - 1);
@@ -217,7 +220,7 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->use_tma = 0;
   std::memset(tm, 0, sizeof(*tm));
   if (h->use_tma && aligned16(d_I) &&
-      make_tensor_map(&tm->I, d_I, c.n_cols, c.n_rows, n_epochs, dia::kIPitch, dia::kTH)) {
+      make_tensor_map(&tm->I, d_I, c.n_cols, c.n_rows, hess_q0 >= 0 ? 1 : n_epochs, dia::kIPitch, dia::kTH)) {
     tm->R = h->tmR;
     p->use_tma = 1;
   }
@@ -306,6 +309,7 @@ extern "C" int dia_destroy(dia_handle* h) {
   if (!h) return DIA_ERR_INVALID_ARG;
   cudaStreamSynchronize(h->stream);
   dia::fit_workspace_destroy(&h->fit);
+  dia::hess_workspace_destroy(&h->hess);
   cudaFree(h->d_partials);
   if (h->d_const_stage) {
     cudaFree(h->d_const_stage);
@@ -325,23 +329,65 @@ static int check_eval_args(dia_handle* h, int n_epochs, const void* d_I, const v
   return DIA_OK;
 }
 
-extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
-                                  const float* d_var, const float* d_theta, double* d_loss, double* d_grad) {
-  int rc = check_eval_args(h, n_epochs, d_I, d_var, d_theta);
-  if (rc != DIA_OK) return rc;
-  if (!d_loss || !d_grad) return fail(h, DIA_ERR_INVALID_ARG, "null output");
+// loss and gradient of n_epochs parameter sets; hess_q0 >= 0: rows hess_q0.. of the Hessian of target 0 instead
+static int eval_into(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask, const float* d_var,
+                     const float* d_theta, double* d_loss, double* d_grad, int hess_q0) {
   dia::EvalParams p;
   dia::TensorMaps tm;
-  fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm);
+  fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, hess_q0);
   cudaError_t ce = dia::launch_eval(h, p, tm);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "eval launch");
   const int np1 = h->np + 1;
   dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, h->stream>>>(
       h->d_partials, dia::eval_part_cols(h, n_epochs), np1, nullptr, d_loss, d_grad);
-  if (h->cfg.lambda_reg > 0.f)
+  if (h->cfg.lambda_reg > 0.f && hess_q0 < 0)
     dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, h->stream>>>(d_theta, h->cfg.m, h->np, lambda_n(h), d_loss, d_grad);
   ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "reduce launch");
+  return DIA_OK;
+}
+
+extern "C" int dia_eval_loss_grad(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
+                                  const float* d_var, const float* d_theta, double* d_loss, double* d_grad) {
+  int rc = check_eval_args(h, n_epochs, d_I, d_var, d_theta);
+  if (rc != DIA_OK) return rc;
+  if (!d_loss || !d_grad) return fail(h, DIA_ERR_INVALID_ARG, "null output");
+  return eval_into(h, n_epochs, d_I, d_mask, d_var, d_theta, d_loss, d_grad, -1);
+}
+
+extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char* d_mask, const float* d_var,
+                           const float* d_theta, double* d_H) {
+  int rc = check_eval_args(h, 1, d_I, d_var, d_theta);
+  if (rc != DIA_OK) return rc;
+  if (!d_H) return fail(h, DIA_ERR_INVALID_ARG, "null output");
+  if (h->n_refs > 1) return fail(h, DIA_ERR_UNSUPPORTED, "dia_hessian needs a handle with one shared reference");
+  const int np = h->np;
+  dia::HessWorkspace& w = h->hess;
+  if (!w.loss) {
+    cudaError_t ce = cudaMalloc(&w.loss, sizeof(double) * (size_t)np);
+    if (ce == cudaSuccess && h->cfg.lambda_reg > 0.f) {
+      ce = cudaMalloc(&w.ident, sizeof(float) * (size_t)np * np);
+      if (ce == cudaSuccess) dia::hess_identity_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(w.ident, np);
+    }
+    if (ce != cudaSuccess) {
+      dia::hess_workspace_destroy(&w);
+      h->err = std::string("hessian workspace: ") + cudaGetErrorString(ce);
+      return DIA_ERR_ALLOC;
+    }
+  }
+  // rows q0 .. q0 + n - 1 of H per launch: the fused kernel with the weight h X_q in place of w (D3)
+  for (int q0 = 0; q0 < np; q0 += h->cfg.max_epochs) {
+    const int n = np - q0 < h->cfg.max_epochs ? np - q0 : h->cfg.max_epochs;
+    rc = eval_into(h, n, d_I, d_mask, d_var, d_theta, w.loss + q0, d_H + (size_t)q0 * np, q0);
+    if (rc != DIA_OK) return rc;
+  }
+  // Eq. 20: the penalty lambda N |L theta|^2 adds 2 lambda N L'L; its gradient is linear in theta, so the
+  // gradient at the unit vector e_q is row q
+  if (h->cfg.lambda_reg > 0.f)
+    dia::penalty_kernel<<<np, dia::kFitThreads, 0, h->stream>>>(w.ident, h->cfg.m, np, lambda_n(h), w.loss, d_H);
+  dia::hess_symmetrise_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(d_H, np);
+  cudaError_t ce = cudaGetLastError();
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "hessian launch");
   return DIA_OK;
 }
 

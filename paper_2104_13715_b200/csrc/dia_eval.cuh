@@ -99,6 +99,9 @@ struct EvalParams {
                              // one column per CTA that owns tiles of the epoch
   int n_rows, n_cols, n_epochs;
   int n_refs;                // 1: one reference shared by all epochs; else one reference per epoch
+  int hess_q0;               // < 0: loss and gradient.  >= 0 (AUX instantiation only, dia_hessian): every "epoch" e
+                             // shares target / mask / variance map 0 and theta 0 and produces row hess_q0 + e of the
+                             // Hessian, sum_V h X_q X with h = d^2 l / dM^2 (D3), in place of the gradient
   int part_rows;             // rows of partials per epoch: np + 1 (gradient, loss), or 3 in difference-image mode
   int np, bg_degree;         // parameters per epoch = M*M + (d+1)(d+2)/2; degree d of the background (Eq. 18)
   float bg_xc, bg_yc, bg_inv_nx, bg_inv_ny;   // Eq. 19: eta = (x - xc) / N_x, xi = (y - yc) / N_y
@@ -213,6 +216,7 @@ __device__ __forceinline__ void stage_I(const EvalParams& p, const TensorMaps& t
   using G = Geo<M>;
   const int ty = tile / p.tiles_x, tx = tile - ty * p.tiles_x;
   const int y0 = ty * kTH + G::H, x0 = tx * kTW + G::H - G::IOFF;
+  if (p.hess_q0 >= 0) e = 0;
   if (p.use_tma) {
     if (threadIdx.x == 0) {
       fence_proxy_async();
@@ -243,6 +247,7 @@ __device__ __forceinline__ void pixel_terms(const EvalParams& p, int e, size_t n
   bool use = EDGE ? inside : true;
   float v, bp;
   if (AUX) {
+    if (p.hess_q0 >= 0) e = 0;
     if (use && p.mask) use = p.mask[(size_t)e * npix + gidx] != 0;
     if (p.noise_kind == 0) {
       float a_ij = p.sigma0_sq, b_ij = p.inv_gain;
@@ -267,6 +272,9 @@ __device__ __forceinline__ void pixel_terms(const EvalParams& p, int e, size_t n
   const float z2 = res * res * inv_v;
   li = 0.5f * z2;
   wi = fmaf(-res, inv_v, hb * (1.0f - z2));
+  const bool hess = AUX && p.hess_q0 >= 0;
+  // D3: h = dw/dM = 1/v + 2 b' r / v^2 + b'^2 r^2 / v^3 - b'^2 / (2 v^2), with hb = b'/(2v)
+  if (hess) wi = inv_v * (1.0f + 4.0f * hb * res) + 4.0f * hb * hb * (z2 - 0.5f);
   if (p.loss_kind == 1) {                          // Huber, Eq. 12
     const float rsd = rsqrtf(v);
     const float z = res * rsd;
@@ -274,6 +282,8 @@ __device__ __forceinline__ void pixel_terms(const EvalParams& p, int e, size_t n
       const float psi = copysignf(p.huber_c, z);
       li = p.huber_c * (fabsf(z) - 0.5f * p.huber_c);
       wi = fmaf(-psi, rsd, hb * (1.0f - psi * z));
+      // D3, linear branch: dz/dM = -1/s - z hb;  h = psi hb / s - psi hb dz/dM + 2 hb^2 (psi z - 1)
+      if (hess) wi = psi * hb * (rsd + (rsd + z * hb)) + 2.0f * hb * hb * (psi * z - 1.0f);
     }
   }
   if (!AUX || p.noise_kind == 0) li = fmaf(0.5f, logf(v), li);
@@ -426,7 +436,8 @@ template <int M, bool AUX, bool EDGE>
 __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_t npix, int iy, int ix0, int vr, int vc,
                                                float (&tot)[kP], const float* __restrict__ irow,
                                                float* __restrict__ wrow, const float* __restrict__ Bs, float& lsum,
-                                               float& wsum, float (&Sp)[4]) {
+                                               float& wsum, float (&Sp)[4], const float* __restrict__ xrow = nullptr,
+                                               int hx_m = 0, int hx_n = 0) {
   using G = Geo<M>;
   float iv[kP];
   if (G::IOFF == 0) {
@@ -449,6 +460,19 @@ __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_
   for (int q = 0; q < kP; ++q) {
     float li, wi;
     pixel_terms<AUX, EDGE>(p, e, npix, gbase + q, (iy < vr) && (ix0 + q < vc), tot[q], iv[q], li, wi);
+    if (AUX && p.hess_q0 >= 0) {           // Hessian row q: weight h X_q, X_q a shifted reference pixel or eta^m xi^n
+      float xq;
+      if (xrow) {
+        xq = xrow[q];
+      } else {
+        const float eta = fmaf((float)q, p.bg_inv_nx, eta0);
+        const float xi = ((float)(iy + G::H) - p.bg_yc) * p.bg_inv_ny;
+        xq = 1.f;
+        for (int k = 0; k < hx_m; ++k) xq *= eta;
+        for (int k = 0; k < hx_n; ++k) xq *= xi;
+      }
+      wi *= xq;
+    }
     lsum += li;
     wsum += wi;
     if (d > 0) {
@@ -530,6 +554,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   };
 
   float B0 = 0.f;
+  int hx_off = -1, hx_m = 0, hx_n = 0;     // Hessian mode: X_q = Rs[pixel + hx_off], or eta^hx_m xi^hx_n if hx_off < 0
   double loss64 = 0.0, gb064 = 0.0, cnt64 = 0.0;   // DIFF: sum eps^2, sum eps, pixel count
   bool flushed = false;
   int since_flush = 0, cur_j = -1;
@@ -605,7 +630,20 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
     if (j != cur_j) {                      // first tile of an epoch for this CTA
       if (cur_j >= 0) finish_epoch();
       cur_j = j;
-      const float* __restrict__ th = p.theta + (size_t)e * p.np;
+      const bool hess = AUX && p.hess_q0 >= 0;
+      const float* __restrict__ th = p.theta + (hess ? (size_t)0 : (size_t)e * p.np);
+      if (hess) {                          // design-vector component of this Hessian row
+        const int hq = p.hess_q0 + e;
+        hx_off = -1; hx_m = 0; hx_n = 0;
+        if (hq < M * M) {
+          hx_off = (hq / M) * G::RPITCH + (hq % M);
+        } else {
+          int tq = M * M;
+          for (int mm = 0; mm <= p.bg_degree; ++mm)
+            for (int nn = 0; nn <= p.bg_degree - mm; ++nn, ++tq)
+              if (tq == hq) { hx_m = mm; hx_n = nn; }
+        }
+      }
       if (!KC) {
         for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
           const int a = idx / G::KP, b = idx - a * G::KP;
@@ -645,8 +683,9 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
         else strip_diff<M, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, s_eps, s_eps2, s_cnt);
         gb064 += (double)s_eps;  loss64 += (double)s_eps2;  cnt64 += (double)s_cnt;
       } else {
-      if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp);
-      else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp);
+      const float* xrow = (AUX && hx_off >= 0) ? Rs + f_row * G::RPITCH + f_col + hx_off : nullptr;
+      if (edge) strip_epilogue<M, AUX, true>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp, xrow, hx_m, hx_n);
+      else strip_epilogue<M, AUX, false>(p, e, npix, iy, ix0, vr, vc, tot, irow, wrow, Bs, lsum, wsum, Sp, xrow, hx_m, hx_n);
       loss64 += (double)lsum;
       gb064 += (double)wsum;
       }

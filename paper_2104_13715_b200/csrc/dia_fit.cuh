@@ -21,7 +21,7 @@ constexpr int kMaxHistory = 128;
 constexpr int kFitThreads = 256;
 constexpr int kMaxPerThread = 4;      // ceil((31*31+1) / 256)
 
-inline bool eval_is_aux(const EvalParams& p) { return p.mask || p.flat || p.var || p.noise_kind != 0; }
+inline bool eval_is_aux(const EvalParams& p) { return p.mask || p.flat || p.var || p.noise_kind != 0 || p.hess_q0 >= 0; }
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff = false);
 const void* eval_kernel_ptr(const dia_handle* h, bool aux);
 bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff);

@@ -1,0 +1,37 @@
+// Helpers of dia_hessian (include/dia.h; Eq. 15-17).  The rows of the Hessian themselves come
+// from the fused kernel in Hessian mode (EvalParams::hess_q0, dia_eval.cuh).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace dia {
+
+struct HessWorkspace {
+  double* loss = nullptr;      // [np] scratch for the loss row of the partials (unused in Hessian mode)
+  float* ident = nullptr;      // [np][np] identity: unit parameter vectors for the penalty's second derivative
+};
+
+inline void hess_workspace_destroy(HessWorkspace* w) {
+  cudaFree(w->loss); cudaFree(w->ident);
+  *w = HessWorkspace();
+}
+
+__global__ void hess_identity_kernel(float* __restrict__ A, int np) {
+  const int total = np * np;
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x)
+    A[idx] = (idx / np == idx % np) ? 1.f : 0.f;
+}
+
+// H <- (H + H') / 2: rows p and q were accumulated in different FP32 orders
+__global__ void hess_symmetrise_kernel(double* __restrict__ H, int np) {
+  const int total = np * np;
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+    const int p = idx / np, q = idx - p * np;
+    if (p < q) {
+      const double a = 0.5 * (H[idx] + H[(size_t)q * np + p]);
+      H[idx] = a;
+      H[(size_t)q * np + p] = a;
+    }
+  }
+}
+
+}  // namespace dia

@@ -1,0 +1,121 @@
+"""GPU-vs-oracle parity of dia_hessian (Eq. 15-17), through the C ABI.
+
+Both sides evaluate the closed form sum_V h X X' (D3), the device in float32 per pixel with FP64
+partial sums, the oracle in FP64.  Entries are compared in the metric that matters for the covariance:
+  e_H = max_pq |H_gpu - H_or|_pq / sqrt(H_or,pp H_or,qq)  <= 2e-6
+and the uncertainties the paper reports (sigma_P, sigma_B0, Eq. 17) must agree to 2e-5 relative.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_H = 2e-6
+TOL_SIGMA = 2e-5
+
+
+@pytest.fixture(scope="module")
+def dia():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2104_13715_b200 as dia
+    dia.load_library()
+    return dia
+
+
+def _dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda().contiguous()
+
+
+def _e_H(Hg, Ho):
+    d = np.sqrt(np.abs(np.diag(Ho)))
+    return float(np.abs((Hg - Ho) / np.outer(d, d)).max())
+
+
+def _sigmas(H, nk):
+    """Eq. 16-17: covariance = H^-1; sigma of P = sum K (a linear combination) and of B0."""
+    np.linalg.cholesky(H)                      # the positive-definiteness check of PAPER.md:183
+    cov = np.linalg.inv(H)
+    one = np.zeros(H.shape[0])
+    one[:nk] = 1.0
+    return float(np.sqrt(one @ cov @ one)), float(np.sqrt(cov[nk, nk]))
+
+
+@pytest.mark.parametrize("c,n,m,E", [(0, None, None, 16), (1, 256, 15, 16), (4, 192, 19, 1), (4, 333, 11, 7)])
+def test_hessian_plain_objective(dia, c, n, m, E):
+    """Gaussian loss, noise model of Eq. 6, at the fitted theta (the MLE of Eq. 15); max_epochs = 1 walks the
+    single-launch path, 333 the cp.async staging path and a chunk size that does not divide 2 np."""
+    w = make_workload(c, n=n, m=m, n_epochs=1)
+    cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=E, sigma0=w.sigma0, gain=w.gain)
+    if E > 1:
+        thg, _ = h.fit(_dev(w.I), _dev(w.theta0), dia.FitOpts.default())
+        th = thg.cpu().numpy()[0]
+    else:
+        th = w.theta_true[0].astype(np.float32)
+    Ho = oracle.hessian(cfg, w.R, w.I[0], th)
+    Hg = h.hessian(_dev(w.I[0]), _dev(th)).cpu().numpy()
+    assert np.array_equal(Hg, Hg.T)
+    e = _e_H(Hg, Ho)
+    nk = w.m * w.m
+    sPg, sBg = _sigmas(Hg, nk)
+    sPo, sBo = _sigmas(Ho, nk)
+    print(f"hessian c{c} n={w.n} m={w.m}: e_H={e:.2e}  sigma_P {sPg:.6e} ({sPo:.6e})  sigma_B0 {sBg:.5e} ({sBo:.5e})")
+    assert e <= TOL_H
+    assert abs(sPg - sPo) <= TOL_SIGMA * sPo and abs(sBg - sBo) <= TOL_SIGMA * sBo
+    Hg2 = h.hessian(_dev(w.I[0]), _dev(th)).cpu().numpy()
+    assert np.array_equal(Hg, Hg2)             # deterministic
+    h.close()
+
+
+def test_hessian_huber_mask_flat_background_penalty(dia):
+    """Every option at once: Huber loss, flat field and mask (c3), a degree-1 background and the Laplacian
+    penalty, whose second derivative is 2 lambda N L'L."""
+    w = make_workload(3, n=200, m=9, n_epochs=1)
+    lam, d = 0.5, 1
+    cfg = oracle.RefConfig(w.n, w.n, w.m, loss=oracle.LOSS_HUBER, huber_c=1.345, sigma0=w.sigma0, gain=w.gain,
+                           flat=w.flat, bg_degree=d, lambda_reg=lam)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=8, loss=dia.LOSS_HUBER, huber_c=1.345, sigma0=w.sigma0,
+                   gain=w.gain, flat=_dev(w.flat), bg_degree=d, lambda_reg=lam)
+    th = np.concatenate([w.theta_true[0], [3.0, -2.0]]).astype(np.float32)
+    mask = None if w.mask is None else w.mask[0]
+    Ho = oracle.hessian(cfg, w.R, w.I[0], th, mask=mask)
+    Hg = h.hessian(_dev(w.I[0]), _dev(th), mask=_dev(mask)).cpu().numpy()
+    e = _e_H(Hg, Ho)
+    print(f"hessian huber+mask+flat+bg+penalty: e_H={e:.2e}")
+    # a pixel whose |z| sits within float32 rounding of the Huber threshold may take the other branch on the
+    # device; the inputs are seeded, and none does here
+    assert e <= TOL_H
+    nk = w.m * w.m
+    sPg, sBg = _sigmas(Hg, nk)
+    sPo, sBo = _sigmas(Ho, nk)
+    assert abs(sPg - sPo) <= TOL_SIGMA * sPo and abs(sBg - sBo) <= TOL_SIGMA * sBo
+    h.close()
+
+
+def test_hessian_fixed_variance_is_normal_matrix(dia):
+    """DIA_NOISE_FIXED, Gaussian loss: H = X' diag(1/var) X, the B08 normal matrix, whatever theta is."""
+    w = make_workload(0, n=150, m=7, n_epochs=1)
+    var = (w.sigma0 ** 2 + np.clip(w.I[0], 0, None) / w.gain).astype(np.float32)
+    cfg = oracle.RefConfig(w.n, w.n, w.m, noise=oracle.NOISE_FIXED)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=4, noise=dia.NOISE_FIXED)
+    th = w.theta_true[0].astype(np.float32)
+    Ho = oracle.hessian(cfg, w.R, w.I[0], th, var=var)
+    H1 = h.hessian(_dev(w.I[0]), _dev(th), var=_dev(var)).cpu().numpy()
+    H2 = h.hessian(_dev(w.I[0]), _dev(w.theta0[0]), var=_dev(var)).cpu().numpy()
+    print(f"hessian fixed variance: e_H {_e_H(H1, Ho):.2e}")
+    assert _e_H(H1, Ho) <= TOL_H
+    assert np.array_equal(H1, H2)
+
+
+def test_hessian_argument_errors(dia):
+    w = make_workload(0, n_epochs=2)
+    R2 = np.stack([w.R, w.R])
+    h = dia.Handle(_dev(R2), w.m, max_epochs=2, sigma0=w.sigma0, gain=w.gain)
+    with pytest.raises(dia.DiaError):
+        h.hessian(_dev(w.I[0]), _dev(w.theta_true[0].astype(np.float32)))
+    h.close()
