@@ -225,6 +225,60 @@ def other_configs(dia, dev):
     return out
 
 
+def sweeps(dia, dev):
+    """--sweep: the shapes of the paper's speed tests (Fig. 8: image size at m = 19 and 25, PAPER.md:604, 620;
+    Fig. 9: kernel size on a 1024^2 crop) on crops of the c4 pair; stand-alone single-epoch
+    dia_eval_loss_grad.  GB/s counts the algorithmic bytes 8 n^2 (R + I once)."""
+    import torch
+    from workloads import make_workload
+    w = make_workload(4, n_epochs=1)
+    peak = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    cases = [(n, m) for m in (19, 25) for n in (512, 1024, 2048, 4096)]
+    cases += [(1024, m) for m in (3, 5, 7, 11, 15, 23, 31)]
+    out = []
+    for n, m in cases:
+        R = torch.from_numpy(np.ascontiguousarray(w.R[:n, :n])).to(dev)
+        I = torch.from_numpy(np.ascontiguousarray(w.I[:, :n, :n])).to(dev)
+        th = torch.full((1, m * m + 1), 1.0 / (m * m), dtype=torch.float32, device=dev)
+        th[0, -1] = 0.0
+        h = dia.Handle(R, m, max_epochs=1, sigma0=w.sigma0, gain=w.gain)
+        L = torch.empty(1, dtype=torch.float64, device=dev)
+        G = torch.empty((1, m * m + 1), dtype=torch.float64, device=dev)
+        for _ in range(5):
+            h.eval_loss_grad(I, th, loss=L, grad=G)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(50):
+            h.eval_loss_grad(I, th, loss=L, grad=G)
+        b.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / 50
+        h.close()
+        out.append({"n": n, "m": m, "us_per_eval": round(1e3 * ms, 2), "evals_per_s": round(1e3 / ms, 1),
+                    "tflops": round(2.0 * useful_fma(n, m) / (ms * 1e-3) / 1e12, 3),
+                    "frac_fp32_nominal": round(2.0 * useful_fma(n, m) / (ms * 1e-3) / 1e12 / peak, 4),
+                    "algorithmic_GBps": round(8.0 * n * n / (ms * 1e-3) / 1e9, 1)})
+    return out
+
+
+def run_sweep(args):
+    import torch
+    if not torch.cuda.is_available():
+        print("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle", file=sys.stderr)
+        return 2
+    import paper_2104_13715_b200 as dia
+    dia.load_library()
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    with ClockSampler(dev.index or 0) as clocks:
+        rows = sweeps(dia, dev)
+    print(json.dumps({"sweep": rows, "clocks": clocks.summary(), "data": "synthetic (crops of the c4 pair)",
+                      "note": "L2-resident for n <= 2048 (the pair fits the 126 MB L2): repeated evaluations of one pair, as in a fit"}),
+          flush=True)
+    return 0
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on the host cores, rank 0 only."""
     rank = int(os.environ.get("RANK", "0"))
@@ -423,9 +477,12 @@ def main():
     ap.add_argument("--no-fit", action="store_true", help="skip the free-running fit (fits/s)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--no-stamps", action="store_true", help="skip the many-small-pairs leg")
+    ap.add_argument("--sweep", action="store_true", help="image-size and kernel-size sweeps (the paper's Fig. 8-9 shapes) only")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     return run_gpu(args)
 
 

@@ -166,11 +166,15 @@ int eval_part_cols(const dia_handle* h, int n_epochs) {
   const int g = eval_grid(h, n_epochs);
   return h->tiles < g ? h->tiles : g;
 }
-// Constant-bank variant: plain objective (no mask / flat / variance map), large images, few enough epochs.
+// Constant-bank variant: plain objective (no mask / flat / variance map), few enough epochs, and enough work per
+// launch: refreshing the bank costs ~5.5 us (pack kernel + copy to the symbol) and buys ~9 % of the kernel time,
+// which pays from about 60 us on -- two or more tiles per resident CTA at m = 19 (bench.py --sweep).
 bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff) {
-  const int kp = (h->cfg.m + 3) / 4 * 4;
-  return h->d_const_stage && !diff && !eval_is_aux(p) && h->tiles >= 64 && p.n_epochs <= kConstEpochs &&
-         (long long)p.n_epochs * h->cfg.m * kp <= kConstK;
+  const int m = h->cfg.m, kp = (m + 3) / 4 * 4;
+  const long long items = (long long)p.n_epochs * h->tiles;
+  const long long waves = (items + h->grid - 1) / h->grid;
+  return h->d_const_stage && !diff && !eval_is_aux(p) && waves * m * m >= 2 * 19 * 19 && p.n_epochs <= kConstEpochs &&
+         (long long)p.n_epochs * m * kp <= kConstK;
 }
 size_t const_block_bytes(const dia_handle* h, int n_epochs) {
   const int kp = (h->cfg.m + 3) / 4 * 4;

@@ -102,6 +102,26 @@ def test_eval_parity(dia, c, n, E):
     h.close()
 
 
+@pytest.mark.parametrize("c,n,m", [(0, None, None), (1, 160, 9), (2, 200, 9), (3, 160, 7)])
+def test_eval_parity_at_oracle_iterates(dia, c, n, m):
+    """Points P3 and P4 of the protocol: the oracle's Adam iterate at 25 % of its Adam phase
+    (gradient far from cancelling: e_norm required) and the oracle's fitted theta (near-stationary: e_S
+    required, e_norm reported).  The iterates come from the oracle alone."""
+    w = make_workload(c, n=n, m=m, n_epochs=1)
+    cfg = _ref_cfg(w)
+    th4, res = oracle.fit(cfg, w.R, w.I, w.theta0, mask=w.mask)
+    k = max(1, res[0].n_adam // 4)
+    th3, _ = oracle.fit(cfg, w.R, w.I, w.theta0,
+                        oracle.RefFitOpts.default(force_adam_iters=k, force_lbfgs_iters=0), mask=w.mask)
+    h = _handle(dia, w)
+    for name, th, kind in (("P3", th3, "norm"), ("P4", th4, "S")):
+        th = np.asarray(th, np.float32)
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=w.mask, want_scale=True)
+        Lg, gg = h.eval_loss_grad(_dev(w.I), _dev(th), mask=_dev(w.mask))
+        _compare(Lg, gg, Lo, go, So, kind, f"c{c} n={w.n} {name} (oracle Adam iterate {k} / fitted theta)")
+    h.close()
+
+
 @pytest.mark.parametrize("loss", ["gaussian", "huber"])
 @pytest.mark.parametrize("m", [1, 3, 5, 9, 11, 13, 17, 21, 23, 27, 29, 31])
 def test_eval_parity_all_kernel_sizes(dia, loss, m):
