@@ -228,22 +228,24 @@ def other_configs(dia, dev):
 def sweeps(dia, dev):
     """--sweep: the shapes of the paper's speed tests (Fig. 8: image size at m = 19 and 25, PAPER.md:604, 620;
     Fig. 9: kernel size on a 1024^2 crop) on crops of the c4 pair; stand-alone single-epoch
-    dia_eval_loss_grad.  GB/s counts the algorithmic bytes 8 n^2 (R + I once)."""
+    dia_eval_loss_grad.  GB/s counts the algorithmic bytes 4 n^2 (1 + E) (R once, every I once)."""
     import torch
     from workloads import make_workload
     w = make_workload(4, n_epochs=1)
     peak = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9 / 1e12
-    cases = [(n, m) for m in (19, 25) for n in (512, 1024, 2048, 4096)]
-    cases += [(1024, m) for m in (3, 5, 7, 11, 15, 23, 31)]
+    cases = [(n, m, 1) for m in (19, 25) for n in (512, 1024, 2048, 4096)]
+    cases += [(1024, m, 1) for m in (3, 5, 7, 11, 15, 23, 31)]
+    # small kernels on a batch larger than L2 (16 copies of the target: 1 GiB): the HBM-side regime of SURVEY.md 8(d)
+    cases += [(4096, m, 16) for m in (3, 5, 7)]
     out = []
-    for n, m in cases:
+    for n, m, E in cases:
         R = torch.from_numpy(np.ascontiguousarray(w.R[:n, :n])).to(dev)
-        I = torch.from_numpy(np.ascontiguousarray(w.I[:, :n, :n])).to(dev)
-        th = torch.full((1, m * m + 1), 1.0 / (m * m), dtype=torch.float32, device=dev)
-        th[0, -1] = 0.0
-        h = dia.Handle(R, m, max_epochs=1, sigma0=w.sigma0, gain=w.gain)
-        L = torch.empty(1, dtype=torch.float64, device=dev)
-        G = torch.empty((1, m * m + 1), dtype=torch.float64, device=dev)
+        I = torch.from_numpy(np.ascontiguousarray(w.I[:, :n, :n])).to(dev).repeat(E, 1, 1).contiguous()
+        th = torch.full((E, m * m + 1), 1.0 / (m * m), dtype=torch.float32, device=dev)
+        th[:, -1] = 0.0
+        h = dia.Handle(R, m, max_epochs=E, sigma0=w.sigma0, gain=w.gain)
+        L = torch.empty(E, dtype=torch.float64, device=dev)
+        G = torch.empty((E, m * m + 1), dtype=torch.float64, device=dev)
         for _ in range(5):
             h.eval_loss_grad(I, th, loss=L, grad=G)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -255,10 +257,10 @@ def sweeps(dia, dev):
         torch.cuda.synchronize()
         ms = a.elapsed_time(b) / 50
         h.close()
-        out.append({"n": n, "m": m, "us_per_eval": round(1e3 * ms, 2), "evals_per_s": round(1e3 / ms, 1),
-                    "tflops": round(2.0 * useful_fma(n, m) / (ms * 1e-3) / 1e12, 3),
-                    "frac_fp32_nominal": round(2.0 * useful_fma(n, m) / (ms * 1e-3) / 1e12 / peak, 4),
-                    "algorithmic_GBps": round(8.0 * n * n / (ms * 1e-3) / 1e9, 1)})
+        out.append({"n": n, "m": m, "epochs": E, "us_per_eval": round(1e3 * ms / E, 2), "evals_per_s": round(1e3 * E / ms, 1),
+                    "tflops": round(2.0 * useful_fma(n, m, E) / (ms * 1e-3) / 1e12, 3),
+                    "frac_fp32_nominal": round(2.0 * useful_fma(n, m, E) / (ms * 1e-3) / 1e12 / peak, 4),
+                    "algorithmic_GBps": round(4.0 * n * n * (1 + E) / (ms * 1e-3) / 1e9, 1)})
     return out
 
 
