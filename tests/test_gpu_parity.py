@@ -434,3 +434,19 @@ def test_full_size_sampled_c4(dia):
             assert torch.allclose(La, Lg + Lc, rtol=1e-7, atol=0)
             assert float((ga - (gg + gc)).abs().max()) <= 2e-6 * float(ga.abs().max())
     h.close()
+
+
+@pytest.mark.parametrize("c,E", [(2, 1), (3, 1), (4, 2)])
+def test_full_size_direct(dia, c, E):
+    """BASELINE configs 2, 3 and 4 at their full sizes (1024^2 Huber, 2048^2 flat + mask, 4096^2 batched -- the
+    constant-bank launch bench.py times), every output against the oracle evaluated over all pixels (the
+    OpenMP oracle needs about a second per 4096^2 epoch)."""
+    w = make_workload(c, n_epochs=E)
+    h = _handle(dia, w)
+    cfg = _ref_cfg(w)
+    I, mask = _dev(w.I), _dev(w.mask)
+    for name, th, kind in _points(w)[:2]:
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, mask=w.mask, want_scale=True)
+        Lg, gg = h.eval_loss_grad(I, _dev(th), mask=mask)
+        _compare(Lg, gg, Lo, go, So, kind, f"c{c} full size {name}")
+    h.close()
