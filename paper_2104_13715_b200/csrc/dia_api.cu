@@ -9,6 +9,7 @@
 #include <cstddef>
 #include <cstring>
 #include <new>
+#include <mutex>
 #include <string>
 
 #include "dia_eval.cuh"
@@ -22,7 +23,7 @@ struct dia_handle {
   cudaStream_t stream;
   int grid, np, sms;       // grid: resident CTAs (SMs x occupancy), capped by max_epochs x tiles
   int tiles, n_refs;
-  dia::ConstBlock* d_const_stage;   // staging copy of the constant block; non-null iff this handle owns the bank
+  dia::ConstBlock* d_const_stage;   // staging copy of the constant block; non-null iff this handle may use the bank
   size_t smem;
   int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
   CUtensorMap tmR;         // valid iff use_tma
@@ -33,9 +34,24 @@ struct dia_handle {
 };
 
 static thread_local std::string g_create_err;
-// The constant bank (dia::c_blk) is one per process: the first handle that can use it owns it until destroyed;
-// other handles run the shared-memory variant of the kernel.
-static std::atomic<dia_handle*> g_const_owner{nullptr};
+// There is one constant block (dia::c_blk) per kernel size and device.  Every evaluation that uses it refreshes it
+// on the handle's stream right before its launch, so handles that share a stream can share the block; the first
+// stream to claim the block of a kernel size keeps it until its last handle is destroyed, and handles on other
+// streams (or devices) run the shared-memory variant of the kernel.
+struct ConstSlot { void* stream = nullptr; int device = -1; int refs = 0; };
+static std::mutex g_const_mutex;
+static ConstSlot g_const_slot[DIA_MAX_KERNEL_SIZE + 1];
+static bool const_slot_acquire(int m, void* stream, int device) {
+  std::lock_guard<std::mutex> lock(g_const_mutex);
+  ConstSlot& sl = g_const_slot[m];
+  if (sl.refs > 0 && (sl.stream != stream || sl.device != device)) return false;
+  sl.stream = stream;  sl.device = device;  ++sl.refs;
+  return true;
+}
+static void const_slot_release(int m) {
+  std::lock_guard<std::mutex> lock(g_const_mutex);
+  if (g_const_slot[m].refs > 0) --g_const_slot[m].refs;
+}
 
 static int fail(dia_handle* h, int code, const std::string& msg) {
   if (h) h->err = msg; else g_create_err = msg;
@@ -290,17 +306,18 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
   const char* no_const = std::getenv("DIA_DISABLE_CONST");   // test hook: force the shared-memory variant
   if (tiles >= 64 && !(no_const && no_const[0] == '1')) {   // large images: try to take the constant bank
-    dia_handle* expected = nullptr;
-    if (g_const_owner.compare_exchange_strong(expected, h)) {
+    int device = -1;
+    cudaGetDevice(&device);
+    if (const_slot_acquire(cfg->m, cfg->stream, device)) {
       if (cudaMalloc(&h->d_const_stage, sizeof(dia::ConstBlock)) != cudaSuccess) {
-        cudaGetLastError();  h->d_const_stage = nullptr;  g_const_owner.store(nullptr);
+        cudaGetLastError();  h->d_const_stage = nullptr;  const_slot_release(cfg->m);
       }
     }
   }
   int rc = dia::fit_workspace_create(&h->fit, cfg->max_epochs, h->np);
   if (rc != DIA_OK) {
     cudaFree(h->d_partials);
-    if (h->d_const_stage) { cudaFree(h->d_const_stage); g_const_owner.store(nullptr); }
+    if (h->d_const_stage) { cudaFree(h->d_const_stage); const_slot_release(cfg->m); }
     fail(nullptr, rc, "fit workspace allocation failed");
     delete h;
     return rc;
@@ -317,8 +334,7 @@ extern "C" int dia_destroy(dia_handle* h) {
   cudaFree(h->d_partials);
   if (h->d_const_stage) {
     cudaFree(h->d_const_stage);
-    dia_handle* me = h;
-    g_const_owner.compare_exchange_strong(me, nullptr);
+    const_slot_release(h->cfg.m);
   }
   delete h;
   return DIA_OK;
@@ -452,9 +468,9 @@ extern "C" int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_
   // kernels per stand-alone evaluation of the plain objective: (pack,) eval, reduce (, penalty); a dia_fit
   // iteration launches the same number (its step kernel takes the place of the reduce kernel)
   if (launches_per_eval) {
-    const int kp = (h->cfg.m + 3) / 4 * 4;
-    const bool kc = h->d_const_stage && !h->cfg.d_flat && h->cfg.noise == DIA_NOISE_MODEL && h->tiles >= 64 &&
-                    h->cfg.max_epochs <= dia::kConstEpochs && (long long)h->cfg.max_epochs * h->cfg.m * kp <= dia::kConstK;
+    dia::EvalParams p = {};               // a full batch of the plain objective
+    p.n_epochs = h->cfg.max_epochs;  p.flat = h->cfg.d_flat;  p.noise_kind = h->cfg.noise;  p.hess_q0 = -1;
+    const bool kc = dia::eval_uses_const(h, p, false);
     *launches_per_eval = 2 + (kc ? 1 : 0) + (h->cfg.lambda_reg > 0.f ? 1 : 0);
   }
   return DIA_OK;

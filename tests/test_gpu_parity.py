@@ -304,22 +304,39 @@ def test_emccd_noise_model_eq7(dia):
 
 
 def test_constant_bank_variant_matches_shared_memory_variant(dia, monkeypatch):
-    """Large images evaluate with the kernel pixels in the constant bank (uniform-register operands); the
-    shared-memory variant (test hook DIA_DISABLE_CONST, or a second live handle, which cannot own the bank)
-    must give the same bits, and both must match the oracle.  Batch of 3 epochs, one of them twice."""
-    w = make_workload(4, n=640, n_epochs=3, m=19)          # 10 x 10 = 100 tiles >= 64
+    """Long launches evaluate with the kernel pixels in the constant bank (uniform-register operands); the
+    shared-memory variant (test hook DIA_DISABLE_CONST, or a handle on another stream than the one that claimed
+    the block) must give the same bits, and both must match the oracle.  Handles on one stream share the block:
+    interleaved evaluations of two of them with different theta must not see each other's kernel pixels."""
+    w = make_workload(4, n=640, n_epochs=3, m=19)          # 3 x 100 tiles on 296 resident CTAs: two waves
     th = w.theta_true.astype(np.float32)
     cfg = _ref_cfg(w)
     Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, want_scale=True)
-    h = _handle(dia, w)                                    # owns the constant bank
+    h = _handle(dia, w)                                    # claims the block of m = 19 for this stream
+    assert h.info()["launches_per_eval"] == 3              # pack, eval, reduce
     Lc, gc = h.eval_loss_grad(_dev(w.I), _dev(th))
     _compare(Lc, gc, Lo, go, So, "S", "const bank")
-    h2 = _handle(dia, w)                                   # second live handle: shared-memory variant
-    L2, g2 = h2.eval_loss_grad(_dev(w.I), _dev(th))
-    assert torch.equal(Lc, L2) and torch.equal(gc, g2)
-    h.close(); h2.close()
+    h2 = _handle(dia, w)                                   # same stream: shares the block
+    assert h2.info()["launches_per_eval"] == 3
+    th_b = _dev(w.theta0)
+    Lb, gb = h2.eval_loss_grad(_dev(w.I), th_b)
+    for _ in range(3):                                     # interleaved, back to back on the stream
+        L1, g1 = h.eval_loss_grad(_dev(w.I), _dev(th))
+        L2, g2 = h2.eval_loss_grad(_dev(w.I), th_b)
+        assert torch.equal(Lc, L1) and torch.equal(gc, g1)
+        assert torch.equal(Lb, L2) and torch.equal(gb, g2)
+    side = torch.cuda.Stream()
+    h4 = _handle(dia, w, stream=side)                      # another stream: shared-memory variant
+    assert h4.info()["launches_per_eval"] == 2
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        L4, g4 = h4.eval_loss_grad(_dev(w.I), _dev(th))
+    side.synchronize()
+    assert torch.equal(Lc, L4) and torch.equal(gc, g4)
+    h.close(); h2.close(); h4.close()
     monkeypatch.setenv("DIA_DISABLE_CONST", "1")
     h3 = _handle(dia, w)
+    assert h3.info()["launches_per_eval"] == 2
     L3, g3 = h3.eval_loss_grad(_dev(w.I), _dev(th))
     assert torch.equal(Lc, L3) and torch.equal(gc, g3)
     h3.close()
