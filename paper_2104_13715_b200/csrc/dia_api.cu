@@ -238,6 +238,7 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->huber_c = c.huber_c;  p->sigma0_sq = c.sigma0 * c.sigma0;
   p->inv_gain = c.noise == DIA_NOISE_MODEL ? 1.0f / c.gain : 0.f;
   p->use_tma = 0;
+  p->cp8 = (c.n_cols % 2 == 0) && (reinterpret_cast<uintptr_t>(h->d_R) & 7) == 0 && (reinterpret_cast<uintptr_t>(d_I) & 7) == 0;
   std::memset(tm, 0, sizeof(*tm));
   if (h->use_tma && aligned16(d_I) &&
       make_tensor_map(&tm->I, d_I, c.n_cols, c.n_rows, hess_q0 >= 0 ? 1 : n_epochs, dia::kIPitch, dia::kTH)) {

@@ -109,6 +109,7 @@ struct EvalParams {
   int loss_kind, noise_kind;
   float huber_c, sigma0_sq, inv_gain;
   int use_tma;               // 1: rows are 16-byte aligned, tensor maps are valid
+  int cp8;                   // cp.async staging path: 1 = rows are 8-byte aligned (even n_cols), copy pixel pairs
 };
 
 struct TensorMaps {          // passed by value as a __grid_constant__ kernel parameter
@@ -123,6 +124,9 @@ __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)_
 
 __device__ __forceinline__ void cp_async_4(unsigned dst, const void* gmem, int src_bytes) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(dst), "l"(gmem), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_8(unsigned dst, const void* gmem, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(gmem), "r"(src_bytes) : "memory");
 }
 __device__ __forceinline__ void cp_async_mbar_arrive(unsigned bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
@@ -196,6 +200,15 @@ __device__ __forceinline__ void stage_R(const EvalParams& p, const TensorMaps& t
     }
   } else {
     const float* Rref = p.R + (size_t)ref * p.n_rows * p.n_cols;
+    if (p.cp8) {                           // even n_cols: pixel pairs are 8-byte aligned and in or out together
+      for (int idx = threadIdx.x; idx < G::RH * (G::RPITCH / 2); idx += kThreads) {
+        const int rr = idx / (G::RPITCH / 2), cc = 2 * (idx - rr * (G::RPITCH / 2));
+        const int gy = y0 + rr, gx = x0 + cc;
+        const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
+        const float* src = ok ? Rref + (size_t)gy * p.n_cols + gx : Rref;
+        cp_async_8(dst + 8u * (unsigned)idx, src, ok ? 8 : 0);
+      }
+    } else
     for (int idx = threadIdx.x; idx < G::RH * G::RPITCH; idx += kThreads) {
       const int rr = idx / G::RPITCH, cc = idx - rr * G::RPITCH;
       const int gy = y0 + rr, gx = x0 + cc;
@@ -225,6 +238,15 @@ __device__ __forceinline__ void stage_I(const EvalParams& p, const TensorMaps& t
     }
   } else {
     const float* Iep = p.I + (size_t)e * p.n_rows * p.n_cols;
+    if (p.cp8) {
+      for (int idx = threadIdx.x; idx < kTH * (kIPitch / 2); idx += kThreads) {
+        const int rr = idx / (kIPitch / 2), cc = 2 * (idx - rr * (kIPitch / 2));
+        const int gy = y0 + rr, gx = x0 + cc;
+        const bool ok = (gy < p.n_rows) && (gx < p.n_cols);
+        const float* src = ok ? Iep + (size_t)gy * p.n_cols + gx : Iep;
+        cp_async_8(dst + 8u * (unsigned)idx, src, ok ? 8 : 0);
+      }
+    } else
     for (int idx = threadIdx.x; idx < kTH * kIPitch; idx += kThreads) {
       const int rr = idx / kIPitch, cc = idx - rr * kIPitch;
       const int gy = y0 + rr, gx = x0 + cc;
