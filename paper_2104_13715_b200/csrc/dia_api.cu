@@ -174,11 +174,20 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 namespace dia {
 const void* eval_kernel_ptr(const dia_handle* h, bool aux) { return kernel_for(h->cfg.m, aux); }
 size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
+// Many small images (at least one epoch per resident CTA): each CTA takes whole epochs, unless that balances the
+// CTAs more than 3 % worse than dealing the (epoch, tile) items out one by one.
+bool eval_by_epoch(const dia_handle* h, int n_epochs) {
+  const long long g = h->grid, items = (long long)n_epochs * h->tiles;
+  if (n_epochs < g || h->tiles < 2) return false;
+  const long long by_epoch = (n_epochs + g - 1) / g * h->tiles, by_item = (items + g - 1) / g;
+  return 100 * by_epoch <= 103 * by_item;
+}
 int eval_grid(const dia_handle* h, int n_epochs) {
   const long long items = (long long)n_epochs * h->tiles;
   return items < h->grid ? (int)items : h->grid;
 }
 int eval_part_cols(const dia_handle* h, int n_epochs) {
+  if (eval_by_epoch(h, n_epochs)) return 1;
   const int g = eval_grid(h, n_epochs);
   return h->tiles < g ? h->tiles : g;
 }
@@ -189,7 +198,8 @@ bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff) {
   const int m = h->cfg.m, kp = (m + 3) / 4 * 4;
   const long long items = (long long)p.n_epochs * h->tiles;
   const long long waves = (items + h->grid - 1) / h->grid;
-  return h->d_const_stage && !diff && !eval_is_aux(p) && waves * m * m >= 2 * 19 * 19 && p.n_epochs <= kConstEpochs &&
+  return h->d_const_stage && !diff && !eval_is_aux(p) && !eval_by_epoch(h, p.n_epochs) && waves * m * m >= 2 * 19 * 19 &&
+         p.n_epochs <= kConstEpochs &&
          (long long)p.n_epochs * m * kp <= kConstK;
 }
 size_t const_block_bytes(const dia_handle* h, int n_epochs) {
@@ -238,6 +248,7 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->huber_c = c.huber_c;  p->sigma0_sq = c.sigma0 * c.sigma0;
   p->inv_gain = c.noise == DIA_NOISE_MODEL ? 1.0f / c.gain : 0.f;
   p->use_tma = 0;
+  p->epoch_per_cta = dia::eval_by_epoch(h, n_epochs) ? 1 : 0;
   p->cp8 = (c.n_cols % 2 == 0) && (reinterpret_cast<uintptr_t>(h->d_R) & 7) == 0 && (reinterpret_cast<uintptr_t>(d_I) & 7) == 0;
   std::memset(tm, 0, sizeof(*tm));
   if (h->use_tma && aligned16(d_I) &&

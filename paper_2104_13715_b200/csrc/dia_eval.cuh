@@ -109,6 +109,9 @@ struct EvalParams {
   int loss_kind, noise_kind;
   float huber_c, sigma0_sq, inv_gain;
   int use_tma;               // 1: rows are 16-byte aligned, tensor maps are valid
+  int epoch_per_cta;         // item order: 0 = CTA b takes items b, b + grid, ... of the epoch-major list;
+                             // 1 = CTA b takes every tile of epochs b, b + grid, ... (many small images: one
+                             // change of epoch per image instead of one per tile; partials have one column)
   int cp8;                   // cp.async staging path: 1 = rows are 8-byte aligned (even n_cols), copy pixel pairs
 };
 
@@ -565,10 +568,15 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   // stay in uniform registers and the constant-bank offset of the kernel row is a uniform value.
   const int n_act = KC ? c_blk.n_active : p.n_epochs;
   const int grid = (int)gridDim.x;
-  const int ncols = min(n_tiles, grid);    // CTAs (columns of partials) that contribute to one epoch
+  const bool by_epoch = !KC && p.epoch_per_cta;
+  const int ncols = by_epoch ? 1 : min(n_tiles, grid);   // CTAs (columns of partials) that contribute to one epoch
   auto step = [&](int& j, int& t) {          // the next item of this CTA
-    t += grid;
-    while (t >= n_tiles) { t -= n_tiles; ++j; }
+    if (by_epoch) {
+      if (++t >= n_tiles) { t = 0; j += grid; }
+    } else {
+      t += grid;
+      while (t >= n_tiles) { t -= n_tiles; ++j; }
+    }
   };
   auto skip_done = [&](int& j, int& t) {     // ... that belongs to an epoch which is still being fitted
     if (!KC)
@@ -635,7 +643,8 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
   };
 
   int j = 0, t = (int)blockIdx.x - grid;
-  step(j, t);                                // first item: t = blockIdx.x, wrapped into (j, t)
+  if (by_epoch) { j = (int)blockIdx.x; t = 0; }
+  else step(j, t);                           // first item: t = blockIdx.x, wrapped into (j, t)
   skip_done(j, t);
   if (j < n_act) {
     const int e0 = KC ? c_blk.active[j] : j;
@@ -679,7 +688,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, c
       for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
       loss64 = 0.0; gb064 = 0.0; cnt64 = 0.0; flushed = false; since_flush = 0;
       // column of this CTA in epoch e: the local index (mod grid) of the tiles it owns there
-      int col = ((int)blockIdx.x - (int)(((long long)j * n_tiles) % grid) + grid) % grid;
+      int col = by_epoch ? 0 : ((int)blockIdx.x - (int)(((long long)j * n_tiles) % grid) + grid) % grid;
       out = p.partials + ((size_t)e * p.part_rows) * ncols + col;
       __syncthreads();                     // Ks visible
     }

@@ -202,6 +202,38 @@ def test_many_small_pairs_one_reference_each(dia):
     h.close()
 
 
+@pytest.mark.parametrize("S,grid_limit", [(16, 8), (20, 8), (9, 3)])
+def test_many_small_pairs_whole_epochs_per_cta(dia, monkeypatch, S, grid_limit):
+    """With at least one image pair per resident CTA each CTA takes whole pairs (one change of epoch per pair, one
+    column of partials) when that balances as well as dealing tiles out one by one: 16 pairs on 8 CTAs and 9 on
+    3 do, 20 on 8 do not.  The test hook DIA_GRID_LIMIT stands in for a batch of several hundred pairs.
+    Loss, gradient and a lock-step fit must match the oracle in both orders, and the difference image too."""
+    monkeypatch.setenv("DIA_GRID_LIMIT", str(grid_limit))
+    n, m = 100, 9                                          # 92^2 valid pixels: 2 x 2 tiles per pair
+    R, I, th0, tht = _stamp_batch(S, n, m)
+    h = dia.Handle(_dev(R), m, max_epochs=S, sigma0=5.0, gain=1.0)
+    assert h.info()["grid_blocks"] == grid_limit
+    cfg = oracle.RefConfig(n, n, m, sigma0=5.0, gain=1.0)
+    for th, kind in ((th0, "norm"), (tht, "S")):
+        Lg, gg = h.eval_loss_grad(_dev(I), _dev(th))
+        Lo = np.empty(S); go = np.empty((S, m * m + 1)); So = np.empty((S, m * m + 1))
+        for k in range(S):
+            l, g_, s_ = oracle.eval_loss_grad(cfg, R[k], I[k], th[k], want_scale=True)
+            Lo[k], go[k], So[k] = l[0], g_[0], s_[0]
+        _compare(Lg, gg, Lo, go, So, kind, f"stamps S={S} grid={grid_limit}")
+    opts = dia.FitOpts.default(force_adam_iters=6, force_lbfgs_iters=3)
+    thg, res = h.fit(_dev(I), _dev(th0), opts)
+    thg = thg.cpu().numpy()
+    D, met = h.difference_image(_dev(I), _dev(tht))
+    for k in (0, S // 2, S - 1):
+        tho, _ = oracle.fit(cfg, R[k], I[k], th0[k], oracle.RefFitOpts.default(force_adam_iters=6, force_lbfgs_iters=3))
+        assert np.abs(thg[k] - tho[0]).max() <= 1e-5 * np.abs(tho[0]).max()
+        Do, mo = oracle.difference_image(cfg, R[k], I[k], tht[k])
+        assert np.abs(D[k].cpu().numpy() - Do).max() <= 1e-5 * np.abs(I[k]).max()
+        assert met[k].cpu().numpy() == pytest.approx(mo, rel=1e-5, abs=1e-5)
+    h.close()
+
+
 @pytest.mark.parametrize("c,n,m,lam", [(0, None, None, 1.0), (4, 300, 19, 0.1), (2, 200, 9, 100.0)])
 def test_laplacian_regularisation_eq20(dia, c, n, m, lam):
     """Eq. 20-21: L0 + lambda N_data theta' L' L theta, evaluated on the device."""
