@@ -317,7 +317,9 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * (tiles < h->grid ? tiles : h->grid) * (h->np + 1));
   if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
   const char* no_const = std::getenv("DIA_DISABLE_CONST");   // test hook: force the shared-memory variant
-  if (tiles >= 64 && !(no_const && no_const[0] == '1')) {   // large images: try to take the constant bank
+  // a full batch would be a long enough launch (eval_uses_const): try to claim the constant block of this kernel size
+  const long long full_waves = ((long long)tiles * cfg->max_epochs + h->grid - 1) / h->grid;
+  if (full_waves * cfg->m * cfg->m >= 2 * 19 * 19 && !(no_const && no_const[0] == '1')) {
     int device = -1;
     cudaGetDevice(&device);
     if (const_slot_acquire(cfg->m, cfg->stream, device)) {

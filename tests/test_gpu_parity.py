@@ -374,6 +374,25 @@ def test_constant_bank_variant_matches_shared_memory_variant(dia, monkeypatch):
     h3.close()
 
 
+def test_constant_bank_variant_on_a_batch_of_medium_images(dia, monkeypatch):
+    """The constant-bank variant is chosen by launch length, not image size: 24 epochs of 300^2 (25 tiles each,
+    three waves of the 296 resident CTAs) use it; same bits as the shared-memory variant, and the oracle's values."""
+    w = make_workload(4, n=300, n_epochs=24, m=19)
+    th = w.theta_true.astype(np.float32)
+    h = _handle(dia, w)
+    assert h.info()["launches_per_eval"] == 3
+    Lc, gc = h.eval_loss_grad(_dev(w.I), _dev(th))
+    Lo, go, So = oracle.eval_loss_grad(_ref_cfg(w), w.R, w.I, th, want_scale=True)
+    _compare(Lc, gc, Lo, go, So, "S", "const bank, 24 x 300^2")
+    h.close()
+    monkeypatch.setenv("DIA_DISABLE_CONST", "1")
+    h3 = _handle(dia, w)
+    assert h3.info()["launches_per_eval"] == 2
+    L3, g3 = h3.eval_loss_grad(_dev(w.I), _dev(th))
+    assert torch.equal(Lc, L3) and torch.equal(gc, g3)
+    h3.close()
+
+
 def test_rectangular_image(dia):
     w = make_workload(1, n=200, m=9)
     R, I = w.R[:137, :], w.I[:, :137, :]
