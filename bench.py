@@ -234,7 +234,7 @@ def sweeps(dia, dev):
     w = make_workload(4, n_epochs=1)
     peak = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9 / 1e12
     cases = [(n, m, 1) for m in (19, 25) for n in (512, 1024, 2048, 4096)]
-    cases += [(1024, m, 1) for m in (3, 5, 7, 11, 15, 23, 31)]
+    cases += [(1024, m, 1) for m in (3, 5, 7, 11, 15, 23, 31, 39, 47)] + [(4096, 47, 1)]
     # small kernels on a batch larger than L2 (16 copies of the target: 1 GiB): the HBM-side regime of SURVEY.md 8(d)
     cases += [(4096, m, 16) for m in (3, 5, 7)]
     out = []

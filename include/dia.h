@@ -43,7 +43,8 @@ enum { DIA_NOISE_MODEL = 0 /* Eq. 6: sigma depends on theta */,
 enum { DIA_FIT_CONVERGED_GRAD = 0, DIA_FIT_CONVERGED_CHANGE = 1, DIA_FIT_MAX_ITERS = 2,
        DIA_FIT_NONFINITE = 3 };
 
-#define DIA_MAX_KERNEL_SIZE 31            /* m odd, 1 <= m <= 31 in this build */
+#define DIA_MAX_KERNEL_SIZE 47            /* m odd, 1 <= m <= 47: the largest kernel of the paper's real-data fits
+                                             (PAPER.md:475); m >= 33 runs one CTA per SM instead of two */
 #define DIA_MAX_BG_DEGREE 3               /* polynomial background degree d <= 3 in this build */
 
 typedef struct {

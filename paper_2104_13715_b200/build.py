@@ -1,6 +1,6 @@
 """Builds paper_2104_13715_b200/libdia_b200.so with nvcc for sm_100a (in-tree).
 
-The fused kernel is instantiated for every odd kernel size m <= 31 in four variants; each m is its own
+The fused kernel is instantiated for every odd kernel size m <= 47 in four variants; each m is its own
 translation unit (csrc/dia_eval_inst.cu compiled with -DDIA_INST_M=<m>), so the 17 compilations run in parallel.
 """
 from __future__ import annotations
@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libdia_b200.so")
-KERNEL_SIZES = list(range(1, 32, 2))
+KERNEL_SIZES = list(range(1, 48, 2))
 HEADERS = ["dia_eval.cuh", "dia_fit.cuh", "dia_probe.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

@@ -88,7 +88,8 @@ extern "C" void dia_default_fit_opts(dia_fit_opts* o) {
 // kernel-size dispatch: one instantiation per odd m
 // ---------------------------------------------------------------------------------------------
 #ifndef DIA_FOR_EACH_M
-#define DIA_FOR_EACH_M(X) X(1) X(3) X(5) X(7) X(9) X(11) X(13) X(15) X(17) X(19) X(21) X(23) X(25) X(27) X(29) X(31)
+#define DIA_FOR_EACH_M(X) X(1) X(3) X(5) X(7) X(9) X(11) X(13) X(15) X(17) X(19) X(21) X(23) X(25) X(27) X(29) X(31) \
+  X(33) X(35) X(37) X(39) X(41) X(43) X(45) X(47)
 #endif
 
 static size_t smem_for(int m) {

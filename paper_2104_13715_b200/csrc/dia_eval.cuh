@@ -28,6 +28,7 @@ constexpr int kP = 16;                // forward strip / gradient chunk length (
 constexpr int kIPitch = 68;           // I/w tile pitch (floats); 68/4 = 17 is odd => conflict-free rows
 constexpr int kFlushTiles = 32;       // FP32 gradient strips are folded into FP64 at least this often
 constexpr int kSmemBudget = 113 * 1024;   // per CTA, two CTAs per SM
+constexpr int kSmemBudget1 = 226 * 1024;  // per CTA when only one fits (m >= 33)
 constexpr int kMaxBg = 16;            // background coefficients held per epoch (degree <= 3 uses 10)
 
 __host__ __device__ constexpr int round_up(int x, int q) { return (x + q - 1) / q * q; }
@@ -50,9 +51,12 @@ struct Geo {
   static constexpr int R_BYTES = R_FLOATS * 4, I_BYTES = I_FLOATS * 4;
   static constexpr int R_STRIDE = round_up(R_BYTES, 128);    // TMA destinations are 128-byte aligned
   static constexpr int FIXED_BYTES = 4 * (2 * I_FLOATS + K_FLOATS + ACC_FLOATS) + 2560;
+  // two CTAs per SM while one R buffer fits into half of the shared memory (m <= 31), else one CTA with up to
+  // 255 registers per thread
+  static constexpr int CTAS = (FIXED_BYTES + R_STRIDE <= kSmemBudget) ? 2 : 1;
   // two R buffers when they fit next to a second resident CTA, else one (the copy of the next R
   // tile then waits for the gradient phase to finish)
-  static constexpr int NRBUF = (FIXED_BYTES + 2 * R_STRIDE <= kSmemBudget) ? 2 : 1;
+  static constexpr int NRBUF = (FIXED_BYTES + 2 * R_STRIDE <= (CTAS == 2 ? kSmemBudget : kSmemBudget1)) ? 2 : 1;
   // shared-memory map (byte offsets from a 128-byte aligned base)
   static constexpr int OFF_R = 0;
   static constexpr int OFF_I = NRBUF * R_STRIDE;
@@ -517,7 +521,7 @@ __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_
 // the fused kernel
 // ------------------------------------------------------------------------------------------------
 template <int M, bool AUX, bool DIFF, bool KC = false>
-__global__ void __launch_bounds__(kThreads, 2) eval_kernel(const EvalParams p, const __grid_constant__ TensorMaps tm) {
+__global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) eval_kernel(const EvalParams p, const __grid_constant__ TensorMaps tm) {
   using G = Geo<M>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // 128-byte aligned base (TMA destinations)

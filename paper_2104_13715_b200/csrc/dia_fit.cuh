@@ -19,7 +19,9 @@ namespace dia {
 
 constexpr int kMaxHistory = 128;
 constexpr int kFitThreads = 256;
-constexpr int kMaxPerThread = 4;      // ceil((31*31+1) / 256)
+constexpr int kPerThreadSmall = 4;    // parameters per thread of the optimiser kernel: ceil((31*31+10) / 256) ...
+constexpr int kPerThreadLarge = 9;    // ... and ceil((47*47+10) / 256) for 33 <= m <= 47
+constexpr int kMaxPerThread = kPerThreadLarge;
 
 inline bool eval_is_aux(const EvalParams& p) { return p.mask || p.flat || p.var || p.noise_kind != 0 || p.hess_q0 >= 0; }
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff = false);
@@ -167,6 +169,7 @@ __global__ void fit_init_kernel(FitBuffers b, const float* __restrict__ theta_in
 }
 
 // One optimiser transition for epoch blockIdx.x, run after every evaluation.
+template <int PER>
 __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a) {
   const int e = blockIdx.x;
   if (a.b.done[e]) return;
@@ -188,8 +191,8 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
   const int hist = o.lbfgs_history;
 
   // ---- second-level reduction of the evaluation's block partials: one warp per output, fixed order
-  __shared__ double gsum[kFitThreads * kMaxPerThread];
-  double gn[kMaxPerThread];
+  __shared__ double gsum[kFitThreads * PER];
+  double gn[PER];
   double Ln = 0.0;
   {
     const double* src = a.partials + (size_t)e * (np + 1) * a.n_blocks;
@@ -210,7 +213,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     }
     __syncthreads();
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < PER; ++q) {
       const int k = tid + q * kFitThreads;
       gn[q] = (k < np) ? gsum[k] : 0.0;
     }
@@ -218,14 +221,15 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     __syncthreads();
   }
   if (a.lamN > 0.0) {                            // Eq. 20 penalty at the evaluation point (uniform branch)
-    __shared__ double xs[kFitThreads * kMaxPerThread], us[kFitThreads * kMaxPerThread];
+    __shared__ double xs[kFitThreads * PER];
+    double* const us = gsum;                     // gsum is dead: gn / Ln hold its content (keeps static shared memory < 48 KB)
     for (int k = tid; k < nk; k += kFitThreads) xs[k] = (double)th32[k];
     __syncthreads();
     double pen = 0.0;
     for (int k = tid; k < nk; k += kFitThreads) { const double u = laplacian_row(xs, a.m, k); us[k] = u; pen += u * u; }
     pen = block_sum(pen, sh);
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < PER; ++q) {
       const int k = tid + q * kFitThreads;
       if (k < nk) gn[q] += 2.0 * a.lamN * laplacian_row(us, a.m, k);
     }
@@ -240,7 +244,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     if (!isfinite(Ln)) {
       st.status = DIA_FIT_NONFINITE; st.L = Ln; finished = true;
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) gcur[k] = gn[q]; }
+      for (int q = 0; q < PER; ++q) { const int k = tid + q * kFitThreads; if (k < np) gcur[k] = gn[q]; }
     } else {
       bool sw;
       if (o.force_adam_iters >= 0) sw = t > o.force_adam_iters;
@@ -248,7 +252,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
       if (!sw) {
         st.b1t *= o.adam_beta1; st.b2t *= o.adam_beta2;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) {
+        for (int q = 0; q < PER; ++q) {
           const int k = tid + q * kFitThreads;
           if (k < np) {
             double* m1 = a.b.m1 + (size_t)e * np; double* m2 = a.b.m2 + (size_t)e * np;
@@ -268,7 +272,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
         // switch: L-BFGS starts from this iterate and reuses this evaluation (R6)
         double gi = 0.0;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) {
+        for (int q = 0; q < PER; ++q) {
           const int k = tid + q * kFitThreads;
           if (k < np) { gcur[k] = gn[q]; const double ag = fabs(gn[q]); gi = (ag > gi || ag != ag) ? ag : gi; }
         }
@@ -282,7 +286,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     if (o.lbfgs_backtrack && (bad || Ln > st.L + 1e-4 * st.alpha * st.gtd) && st.nbt < 20) {
       st.alpha *= 0.5; st.nbt += 1;
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) {
+      for (int q = 0; q < PER; ++q) {
         const int k = tid + q * kFitThreads;
         if (k < np) th32[k] = (float)(theta[k] + st.alpha * dvec[k]);
       }
@@ -290,9 +294,9 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
       st.status = DIA_FIT_NONFINITE; finished = true;
     } else {
       double sty = 0.0, yty = 0.0;
-      double sv[kMaxPerThread], yv[kMaxPerThread];
+      double sv[PER], yv[PER];
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) {
+      for (int q = 0; q < PER; ++q) {
         const int k = tid + q * kFitThreads;
         sv[q] = 0.0; yv[q] = 0.0;
         if (k < np) { sv[q] = st.alpha * dvec[k]; yv[q] = gn[q] - gcur[k]; sty += sv[q] * yv[q]; yty += yv[q] * yv[q]; }
@@ -304,7 +308,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
         if (st.n_pairs < hist) { id = (st.head + st.n_pairs) % hist; st.n_pairs += 1; }
         else { id = st.head; st.head = (st.head + 1) % hist; }
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) {
+        for (int q = 0; q < PER; ++q) {
           const int k = tid + q * kFitThreads;
           if (k < np) { Sm[(size_t)id * np + k] = sv[q]; Ym[(size_t)id * np + k] = yv[q]; }
         }
@@ -312,7 +316,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
       }
       const double dL = fabs(Ln - st.L);
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) {
+      for (int q = 0; q < PER; ++q) {
         const int k = tid + q * kFitThreads;
         if (k < np) { theta[k] += sv[q]; gcur[k] = gn[q]; }
       }
@@ -328,10 +332,10 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
 
   if (at_top && !finished) {
     // ---- L-BFGS loop head: stop test, two-loop recursion, first trial point
-    double q4[kMaxPerThread];
+    double q4[PER];
     double gi = 0.0, g1 = 0.0;
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < PER; ++q) {
       const int k = tid + q * kFitThreads;
       q4[q] = (k < np) ? gcur[k] : 0.0;
       const double ag = fabs(q4[q]);
@@ -346,51 +350,51 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     if (stop) {
       finished = true;
     } else {
-      double gq[kMaxPerThread];
+      double gq[PER];
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) gq[q] = q4[q];
+      for (int q = 0; q < PER; ++q) gq[q] = q4[q];
       // two-loop recursion (N&W Alg. 7.4)
       for (int i = st.n_pairs - 1; i >= 0; --i) {
         const int id = (st.head + i) % hist;
         double part = 0.0;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) part += Sm[(size_t)id * np + k] * q4[q]; }
+        for (int q = 0; q < PER; ++q) { const int k = tid + q * kFitThreads; if (k < np) part += Sm[(size_t)id * np + k] * q4[q]; }
         const double al = rho[id] * block_sum(part, sh);
         if (tid == 0) s_alpha[i] = al;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) q4[q] -= al * Ym[(size_t)id * np + k]; }
+        for (int q = 0; q < PER; ++q) { const int k = tid + q * kFitThreads; if (k < np) q4[q] -= al * Ym[(size_t)id * np + k]; }
       }
       __syncthreads();
       double gamma = 1.0;
       if (st.n_pairs > 0) { const int id = (st.head + st.n_pairs - 1) % hist; gamma = (1.0 / rho[id]) / yy[id]; }
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) q4[q] *= gamma;
+      for (int q = 0; q < PER; ++q) q4[q] *= gamma;
       for (int i = 0; i < st.n_pairs; ++i) {
         const int id = (st.head + i) % hist;
         double part = 0.0;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) part += Ym[(size_t)id * np + k] * q4[q]; }
+        for (int q = 0; q < PER; ++q) { const int k = tid + q * kFitThreads; if (k < np) part += Ym[(size_t)id * np + k] * q4[q]; }
         const double beta = rho[id] * block_sum(part, sh);
         const double c = s_alpha[i] - beta;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) { const int k = tid + q * kFitThreads; if (k < np) q4[q] += c * Sm[(size_t)id * np + k]; }
+        for (int q = 0; q < PER; ++q) { const int k = tid + q * kFitThreads; if (k < np) q4[q] += c * Sm[(size_t)id * np + k]; }
       }
       double part = 0.0;
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) { q4[q] = -q4[q]; part += gq[q] * q4[q]; }
+      for (int q = 0; q < PER; ++q) { q4[q] = -q4[q]; part += gq[q] * q4[q]; }
       double gtd = block_sum(part, sh);
       if (!(gtd < 0.0)) {                                 // not a descent direction: drop the history
         st.n_pairs = 0; st.head = 0;
         part = 0.0;
 #pragma unroll
-        for (int q = 0; q < kMaxPerThread; ++q) { q4[q] = -gq[q]; part += gq[q] * q4[q]; }
+        for (int q = 0; q < PER; ++q) { q4[q] = -gq[q]; part += gq[q] * q4[q]; }
         gtd = block_sum(part, sh);
       }
       double alpha = o.lbfgs_lr;
       if (st.n_pairs == 0) alpha *= (g1 > 1.0) ? 1.0 / g1 : 1.0;     // R7 first-step scaling
       st.alpha = alpha; st.gtd = gtd; st.nbt = 0;
 #pragma unroll
-      for (int q = 0; q < kMaxPerThread; ++q) {
+      for (int q = 0; q < PER; ++q) {
         const int k = tid + q * kFitThreads;
         if (k < np) { dvec[k] = q4[q]; th32[k] = (float)(theta[k] + alpha * q4[q]); }
       }
@@ -400,7 +404,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
   if (finished) {
     double gi = 0.0, P = 0.0;
 #pragma unroll
-    for (int q = 0; q < kMaxPerThread; ++q) {
+    for (int q = 0; q < PER; ++q) {
       const int k = tid + q * kFitThreads;
       if (k < np) {
         const double ag = fabs(gcur[k]);
@@ -509,7 +513,9 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     sa.m = m; sa.lamN = lamN;
     void* step_args[] = {(void*)&sa};
     cudaKernelNodeParams ks = {};
-    ks.func = (void*)fit_step_kernel; ks.gridDim = dim3(n_epochs); ks.blockDim = dim3(kFitThreads);
+    ks.func = w->np <= kFitThreads * kPerThreadSmall ? (void*)fit_step_kernel<kPerThreadSmall>
+                                                      : (void*)fit_step_kernel<kPerThreadLarge>;
+    ks.gridDim = dim3(n_epochs); ks.blockDim = dim3(kFitThreads);
     ks.sharedMemBytes = 0; ks.kernelParams = step_args; ks.extra = nullptr;
     // The body holds `unroll` (eval ; step) pairs: re-evaluating the WHILE condition costs several
     // microseconds, which matters when an evaluation takes ~10 us (small images).  Pairs that run after

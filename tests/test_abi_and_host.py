@@ -102,7 +102,7 @@ def test_status_strings_and_host_side_argument_errors():
         assert rc == -2 and out.value is None                                   # DIA_ERR_CUDA, no fallback
         cfg.m = 4
         assert lib.dia_create(C.byref(cfg), C.cast(buf, C.c_void_p), C.byref(out)) == -1
-        cfg.m, cfg.n_rows, cfg.n_cols = 33, 64, 64
+        cfg.m, cfg.n_rows, cfg.n_cols = 49, 64, 64
         assert lib.dia_create(C.byref(cfg), C.cast(buf, C.c_void_p), C.byref(out)) == -4
         peak = C.c_double()
         assert lib.dia_measure_fp32_peak(None, C.byref(peak)) == -2

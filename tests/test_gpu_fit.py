@@ -321,3 +321,20 @@ def test_fit_nonfinite_status(dia):
     th, r = h.fit(_dev(w.I), _dev(th0), dia.FitOpts.default())
     assert r[0].status == 3 and r[0].n_evals == 1
     h.close()
+
+
+@pytest.mark.parametrize("m,lam", [(35, 0.0), (47, 0.0), (47, 0.05)])
+def test_fit_lockstep_large_kernels(dia, m, lam):
+    """Kernels of the paper's real-data fits (median 27 x 27, maximum 47 x 47 on 142^2 stamps):
+    m >= 33 runs one CTA per SM, and more than 1024 parameters take the wide instantiation of the optimiser
+    kernel.  Two stamps, lock-step Adam + L-BFGS, with and without the Laplacian penalty."""
+    w = make_workload(0, n=142, m=m, n_epochs=2)
+    og, oo = _both_opts(dia, force_adam_iters=8, force_lbfgs_iters=4)
+    cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=2, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
+    assert h.info()["grid_blocks"] <= 148          # one resident CTA per SM
+    tho, ro = oracle.fit(cfg, w.R, w.I, w.theta0, oo)
+    thg, rg = h.fit(_dev(w.I), _dev(w.theta0), og)
+    h.close()
+    assert [r.n_evals for r in rg] == [r.n_evals for r in ro]
+    _assert_fit_close(tho, ro, thg.cpu().numpy(), rg, f"lockstep m={m} lambda={lam}")

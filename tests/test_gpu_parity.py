@@ -123,7 +123,7 @@ def test_eval_parity_at_oracle_iterates(dia, c, n, m):
 
 
 @pytest.mark.parametrize("loss", ["gaussian", "huber"])
-@pytest.mark.parametrize("m", [1, 3, 5, 9, 11, 13, 17, 21, 23, 27, 29, 31])
+@pytest.mark.parametrize("m", [1, 3, 5, 9, 11, 13, 17, 21, 23, 27, 29, 31, 33, 35, 37, 39, 41, 43, 45, 47])
 def test_eval_parity_all_kernel_sizes(dia, loss, m):
     """Every instantiated kernel size, both objectives, FIXED and MODEL noise."""
     w = make_workload(2 if loss == "huber" else 1, n=150, m=m)
@@ -466,7 +466,7 @@ def test_argument_errors(dia):
     with pytest.raises(dia.DiaError):
         dia.Handle(R, 4)                       # even m
     with pytest.raises(dia.DiaError):
-        dia.Handle(R, 33)                      # above DIA_MAX_KERNEL_SIZE
+        dia.Handle(R, 49)                      # above DIA_MAX_KERNEL_SIZE
     with pytest.raises(dia.DiaError):
         dia.Handle(R, 5, gain=0.0)
     h = dia.Handle(R, 5, sigma0=5.0)
