@@ -453,6 +453,7 @@ def run_gpu(args):
     # ---- many small image pairs, one reference each (the paper's stamp workloads)
     if rank == 0 and not args.no_stamps:
         line["stamps"] = stamp_batch_rate(dia, dev)
+        line["stamps_m27"] = stamp_batch_rate(dia, dev, m=27)     # median kernel size of the paper's real-data fits
         line["other_configs"] = other_configs(dia, dev)
 
     # ---- the oracle beside it (rank 0, N = 1 only)
