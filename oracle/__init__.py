@@ -12,6 +12,7 @@ from .dia_ref import (  # noqa: F401
     b08_solve,
     difference_image,
     hessian,
+    covariance,
     model,
     huber_Q,
     num_threads,

@@ -6,7 +6,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["dia_ref.c", "dia_ref_fit.c", "dia_ref_b08.c"]
+SOURCES = ["dia_ref.c", "dia_ref_fit.c", "dia_ref_b08.c", "dia_ref_cov.c"]
 LIB = os.path.join(HERE, "libdia_ref.so")
 
 

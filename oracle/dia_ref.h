@@ -86,6 +86,13 @@ int dia_ref_difference_image(const dia_ref_config* cfg, const float* R, const fl
 int dia_ref_hessian(const dia_ref_config* cfg, const float* R, const float* I, const unsigned char* mask,
                     const float* var, const float* theta, double* H);
 
+/* Covariance estimate Sigma = H^-1 (Eq. 16), parameter uncertainties sqrt(Sigma_pp) (Eq. 17,
+ * PAPER.md:189-191) and the validity tests of PAPER.md:193 (determinant of Sigma not negative, every eigenvalue of
+ * Sigma positive).  H [n][n] row-major FP64 symmetric; the first n_kernel parameters are the kernel pixels, whose sum
+ * is the photometric scale factor P (Eq. 3).  Out: cov [n][n], sigma [n],
+ * info[5] = { valid (1/0), ln|det H|, sigma_P = sqrt(u' Sigma u), smallest eigenvalue of Sigma, sign of det H }. */
+int dia_ref_covariance(int n, int n_kernel, const double* H, double* cov, double* sigma, double* info);
+
 /* Adam -> L-BFGS fit (DESIGN c.2), one epoch after another.  theta in/out float32. */
 int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
                 int n_epochs, const float* I, const unsigned char* mask, const float* var,

@@ -198,6 +198,20 @@ def hessian(cfg: RefConfig, R, I, theta, mask=None, var=None) -> np.ndarray:
     return H
 
 
+def covariance(H, n_kernel: int):
+    """-> (cov float64 [n][n], sigma float64 [n], info float64 [5]) from the Hessian H (Eq. 16-17 and the validity
+    tests of PAPER.md:193); info = (valid, ln|det H|, sigma_P, min eigenvalue of cov, sign det H)."""
+    H = np.ascontiguousarray(H, dtype=np.float64)
+    n = H.shape[0]
+    assert H.shape == (n, n)
+    cov = np.empty((n, n), dtype=np.float64)
+    sigma = np.empty(n, dtype=np.float64)
+    info = np.empty(5, dtype=np.float64)
+    _check(_lib().dia_ref_covariance(int(n), int(n_kernel), _ptr(H), _ptr(cov), _ptr(sigma), _ptr(info)),
+           "dia_ref_covariance")
+    return cov, sigma, info
+
+
 def huber_Q(c: float, N: float) -> float:
     return float(_lib().dia_ref_huber_Q(float(c), float(N)))
 

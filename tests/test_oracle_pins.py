@@ -340,3 +340,79 @@ def test_difference_image_and_mfb_mfv():
     assert met[1] == pytest.approx(eps.mean(), rel=1e-12)
     assert met[2] == pytest.approx(eps.var(ddof=1), rel=1e-12)
     assert met[3] == pytest.approx((eps ** 2).sum(), rel=1e-12)
+
+
+# ---------------------------------------------------------------- covariance (Eq. 16-17, PAPER.md:185-193)
+def _spd(n, seed, cond=1e4):
+    rng = np.random.default_rng(seed)
+    Q, _ = np.linalg.qr(rng.normal(size=(n, n)))
+    ev = np.exp(rng.uniform(0.0, math.log(cond), n))
+    return (Q * ev) @ Q.T, ev
+
+
+def test_covariance_closed_form_2x2_and_diagonal():
+    """[[a, b], [b, d]]^-1 = [[d, -b], [-b, a]] / (ad - b^2) (a swapped or unsigned off-diagonal fails); a diagonal
+    H gives sigma_p = 1/sqrt(H_pp) (a missing square root, or sigma taken from H instead of H^-1, fails)."""
+    a, b, d = 4.0, 1.5, 3.0
+    cov, sig, info = oracle.covariance(np.array([[a, b], [b, d]]), 1)
+    det = a * d - b * b
+    np.testing.assert_allclose(cov, np.array([[d, -b], [-b, a]]) / det, rtol=1e-14)
+    np.testing.assert_allclose(sig, [math.sqrt(d / det), math.sqrt(a / det)], rtol=1e-14)
+    assert info[0] == 1.0 and info[4] == 1.0
+    assert info[1] == pytest.approx(math.log(det), rel=1e-14)
+    assert info[2] == pytest.approx(math.sqrt(d / det), rel=1e-14)        # u = (1, 0): sigma_P = sigma_0
+    np.testing.assert_allclose(info[3], 1.0 / np.linalg.eigvalsh(np.array([[a, b], [b, d]])).max(), rtol=1e-12)
+    h = np.array([4.0, 0.25, 100.0, 1.0])
+    cov, sig, info = oracle.covariance(np.diag(h), 3)
+    np.testing.assert_allclose(sig, 1.0 / np.sqrt(h), rtol=1e-15)
+    assert info[2] == pytest.approx(math.sqrt((1.0 / h[:3]).sum()), rel=1e-14)   # independent terms add in variance
+    assert info[3] == pytest.approx(0.01, rel=1e-14)
+
+
+@pytest.mark.parametrize("n,seed", [(5, 0), (50, 1), (123, 2)])
+def test_covariance_against_numpy_spd(n, seed):
+    """numpy.linalg (LAPACK) inverse, log-determinant and spectrum of a random SPD matrix with known eigenvalues."""
+    H, ev = _spd(n, seed)
+    nk = n - 1
+    cov, sig, info = oracle.covariance(H, nk)
+    ref = np.linalg.inv(H)
+    scale = np.sqrt(np.outer(np.diag(ref), np.diag(ref)))
+    assert (np.abs(cov - ref) / scale).max() < 1e-9
+    np.testing.assert_allclose(H @ cov, np.eye(n), atol=1e-9)
+    np.testing.assert_allclose(sig, np.sqrt(np.diag(ref)), rtol=1e-9)
+    assert info[0] == 1.0 and info[4] == 1.0
+    assert info[1] == pytest.approx(np.log(ev).sum(), rel=1e-10)          # planted spectrum, not a library call
+    assert info[3] == pytest.approx(1.0 / ev.max(), rel=1e-8)
+    u = np.zeros(n); u[:nk] = 1.0
+    assert info[2] == pytest.approx(math.sqrt(u @ ref @ u), rel=1e-8)
+
+
+def test_covariance_validity_flags():
+    """a negative determinant, or any eigenvalue <= 0, makes Sigma invalid.  One negative eigenvalue
+    flips the determinant; two leave it positive, so only the eigenvalue test catches that case."""
+    rng = np.random.default_rng(7)
+    Q, _ = np.linalg.qr(rng.normal(size=(6, 6)))
+    for ev, sign in (([3, 2, 1, 0.5, 0.1, -0.2], -1.0), ([3, 2, 1, 0.5, -0.1, -0.2], 1.0)):
+        ev = np.array(ev, float)
+        H = (Q * ev) @ Q.T
+        cov, sig, info = oracle.covariance(H, 5)
+        assert info[0] == 0.0
+        assert info[4] == sign
+        assert info[3] == pytest.approx((1.0 / ev).min(), rel=1e-10)
+        assert info[1] == pytest.approx(np.log(np.abs(ev)).sum(), rel=1e-10)
+        np.testing.assert_allclose(H @ cov, np.eye(6), atol=1e-10)         # the inverse itself still exists
+    cov, sig, info = oracle.covariance(np.array([[1.0, 2.0], [2.0, 4.0]]), 1)   # singular
+    assert info[0] == 0.0
+
+
+def test_covariance_of_planted_linear_model():
+    """For a linear model y = X theta + N(0, s^2) the Fisher matrix is X'X / s^2 and the covariance of the estimate is
+    s^2 (X'X)^-1 -- the textbook least-squares result; the empirical scatter of repeated fits must agree with sigma
+    (a covariance taken from H instead of its inverse, or a missing square root, fails by orders of magnitude)."""
+    rng = np.random.default_rng(11)
+    X = rng.normal(size=(400, 4)); s = 0.3
+    H = X.T @ X / s ** 2
+    _, sig, info = oracle.covariance(H, 4)
+    th = np.array([np.linalg.lstsq(X, X @ np.ones(4) + s * rng.normal(size=400), rcond=None)[0] for _ in range(3000)])
+    np.testing.assert_allclose(th.std(axis=0), sig, rtol=0.06)
+    assert th.sum(axis=1).std() == pytest.approx(info[2], rel=0.06)
