@@ -444,11 +444,17 @@ def run_gpu(args):
                             "photometric_scale": [round(r.photometric_scale, 5) for r in res_f]}
         # Hessian at the fitted theta of epoch 0 (Eq. 15): np rows, max_epochs rows per launch
         h.hessian(dI[0], th_hat[0])
-        ms_h, _ = timed(lambda: h.hessian(dI[0], th_hat[0]), 1)
+        ms_h, H_hat = timed(lambda: h.hessian(dI[0], th_hat[0]), 1)
+        # covariance and uncertainties from it (Eq. 16-17): FP64 Cholesky factorisation and solves on the device
+        h.covariance(H_hat)
+        ms_c, (_, sig_hat, cov_info) = timed(lambda: h.covariance(H_hat), 1)
         if rank == 0:
             rows = M * M + 1
+            ci = cov_info.cpu().tolist()
             line["fits"]["hessian"] = {"ms": ms_h, "rows": rows, "launches": -(-rows // E),
                                        "tflops": useful_fma(epochs=rows) * 2 / (ms_h * 1e-3) / 1e12}
+            line["fits"]["covariance"] = {"ms": ms_c, "np": rows, "launches": rows + 3, "valid": ci[0],
+                                          "sigma_P": ci[2], "sigma_B0": float(sig_hat[M * M])}
 
     # ---- many small image pairs, one reference each (the paper's stamp workloads)
     if rank == 0 and not args.no_stamps:

@@ -138,6 +138,21 @@ int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs,
 int dia_hessian(dia_handle* h, const float* d_I, const unsigned char* d_mask, const float* d_var,
                 const float* d_theta, double* d_H);
 
+/* Covariance estimate of the fitted parameters from the Hessian of dia_hessian (Eq. 16-17):
+ * Sigma = H^-1, sigma_p = sqrt(Sigma_pp), with the validity test of PAPER.md:193 ("if either the determinant of Sigma
+ * is negative, or ... any eigenvalue is found to be negative or zero, then Sigma is not valid").  H is factorised as
+ * L L' in FP64 on the device; a symmetric matrix is positive definite -- all eigenvalues > 0, hence det > 0 -- exactly
+ * when every Cholesky pivot is positive, so one pivot test stands for both of the paper's (R20).
+ *   d_H     [np][np] float64 DEVICE, row-major, symmetric (only the lower triangle is read); not modified;
+ *   d_cov   [np][np] float64 DEVICE out, or NULL when only the uncertainties are wanted (skips the back-substitution);
+ *   d_sigma [np] float64 DEVICE out: sqrt(Sigma_pp), the Cramer-Rao bound of Eq. 17;
+ *   d_info  [5] float64 DEVICE out: { valid (1 = positive definite, 0 = the paper's warning flag), ln det H
+ *           (= -ln det Sigma), sigma_P = sqrt(u' Sigma u) for the photometric scale factor P = sum K (Eq. 3; u = 1 on
+ *           the m*m kernel pixels), smallest Cholesky pivot, index of the first non-positive pivot or -1 }.
+ * When valid == 0 the numbers in d_cov, d_sigma, ln det H and sigma_P are NaN or meaningless.  The first call
+ * allocates an np x np workspace (synchronises once); later calls are asynchronous on the handle's stream. */
+int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, double* d_sigma, double* d_info);
+
 /* Difference image and fit-quality metrics for n_epochs targets at the given theta (the science product,
  * PAPER.md:20; metrics of Eq. 29-30):
  *   D_ij = I_ij - M_ij on the valid region V (mask or not), 0 outside V;

@@ -9,7 +9,7 @@
  *   (2) eigenvalues of the symmetrised Sigma by the cyclic Jacobi rotation method (diagonalisation).
  * The photometric scale factor is P = sum of the kernel pixels (Eq. 3), a linear function u'theta with
  * u = 1 on the n_kernel kernel parameters and 0 on the background ones, so var P = u' Sigma u (linear error
- * propagation; reading R13).
+ * propagation; reading R20).
  * Pins (tests/test_oracle_pins.py): closed-form 2x2 and diagonal cases, numpy.linalg.inv / slogdet / eigvalsh on
  * random SPD and indefinite matrices, H Sigma = 1.
  */

@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     dia_destroy,
     dia_difference_image,
     dia_hessian,
+    dia_covariance,
     dia_eval_loss_grad,
     dia_fit,
     dia_measure_fp32_peak,

@@ -19,7 +19,7 @@ NOISE_MODEL, NOISE_FIXED = 0, 1
 FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
-                    "dia_measure_fp32_peak", "dia_difference_image", "dia_hessian")
+                    "dia_measure_fp32_peak", "dia_difference_image", "dia_hessian", "dia_covariance")
 
 
 class DiaError(RuntimeError):
@@ -89,6 +89,7 @@ def load_library(build_if_missing: bool = True):
     lib.dia_destroy.argtypes = [C.c_void_p]
     lib.dia_difference_image.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6
     lib.dia_hessian.argtypes = [C.c_void_p] * 6
+    lib.dia_covariance.argtypes = [C.c_void_p] * 5
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
     lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     _LIB = lib
@@ -162,6 +163,12 @@ def dia_hessian(handle: int, d_I, d_mask, d_var, d_theta, d_H) -> None:
                            _dptr(d_H, torch.float64, "d_H")), handle)
 
 
+def dia_covariance(handle: int, d_H, d_cov, d_sigma, d_info) -> None:
+    lib = load_library()
+    _check(lib.dia_covariance(handle, _dptr(d_H, torch.float64, "d_H"), _dptr(d_cov, torch.float64, "d_cov"),
+                              _dptr(d_sigma, torch.float64, "d_sigma"), _dptr(d_info, torch.float64, "d_info")), handle)
+
+
 def dia_destroy(handle: int) -> None:
     _check(load_library().dia_destroy(handle))
 
@@ -232,6 +239,15 @@ class Handle:
         H = torch.empty((self.np, self.np), dtype=torch.float64, device=I.device)
         dia_hessian(self._h, I, mask, var, theta, H)
         return H
+
+    def covariance(self, H, want_cov: bool = True):
+        """-> (cov float64 [np][np] or None, sigma float64 [np], info float64 [5]) CUDA tensors from the Hessian H
+        (Eq. 16-17); info = (valid, ln det H, sigma_P, smallest Cholesky pivot, first non-positive pivot or -1)."""
+        cov = torch.empty((self.np, self.np), dtype=torch.float64, device=H.device) if want_cov else None
+        sigma = torch.empty(self.np, dtype=torch.float64, device=H.device)
+        info = torch.empty(5, dtype=torch.float64, device=H.device)
+        dia_covariance(self._h, H, cov, sigma, info)
+        return cov, sigma, info
 
     def fit(self, I, theta0, opts: Optional[FitOpts] = None, mask=None, var=None):
         """Returns (theta_hat float32 [E][np] CUDA tensor, list[FitResult]); synchronises to read results."""

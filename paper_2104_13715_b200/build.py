@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libdia_b200.so")
 KERNEL_SIZES = list(range(1, 48, 2))
-HEADERS = ["dia_eval.cuh", "dia_fit.cuh", "dia_probe.cuh"]
+HEADERS = ["dia_eval.cuh", "dia_fit.cuh", "dia_hess.cuh", "dia_cov.cuh", "dia_probe.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 
@@ -30,6 +30,10 @@ def needs_build() -> bool:
         return True
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(d) > t for d in _deps())
+
+
+def _stale(obj: str, deps) -> bool:
+    return not os.path.exists(obj) or any(os.path.getmtime(d) > os.path.getmtime(obj) for d in deps)
 
 
 def _compile(job):
@@ -48,9 +52,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for m in KERNEL_SIZES:
         jobs.append((os.path.join(CSRC, "dia_eval_inst.cu"), os.path.join(OBJ, f"dia_eval_m{m}.o"),
                      [f"-DDIA_INST_M={m}"], verbose))
-    workers = max(1, min(len(jobs), os.cpu_count() or 1))
+    # the per-kernel-size units include dia_eval.cuh only; objects newer than their sources are kept
+    inst_deps = [os.path.join(CSRC, f) for f in ("dia_eval.cuh", "dia_eval_inst.cu")] + [os.path.join(HERE, "build.py")]
+    todo = [j for j in jobs if force or _stale(j[1], _deps() if j[1].endswith("dia_api.o") else inst_deps)]
+    workers = max(1, min(len(todo), os.cpu_count() or 1))
     with concurrent.futures.ThreadPoolExecutor(max_workers=workers) as pool:
-        results = list(pool.map(_compile, jobs))
+        results = list(pool.map(_compile, todo))
     for rc, cmd, out in results:
         if verbose and out:
             print(out)

@@ -15,6 +15,7 @@
 #include "dia_eval.cuh"
 #include "dia_fit.cuh"
 #include "dia_hess.cuh"
+#include "dia_cov.cuh"
 #include "dia_probe.cuh"
 
 struct dia_handle {
@@ -423,6 +424,38 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
   dia::hess_symmetrise_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(d_H, np);
   cudaError_t ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "hessian launch");
+  return DIA_OK;
+}
+
+extern "C" int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, double* d_sigma, double* d_info) {
+  if (!h) return DIA_ERR_INVALID_ARG;
+  if (!d_H || !d_sigma || !d_info) return fail(h, DIA_ERR_INVALID_ARG, "null Hessian, sigma or info");
+  if (d_cov == d_H) return fail(h, DIA_ERR_INVALID_ARG, "d_cov must not alias d_H");
+  const int np = h->np;
+  dia::HessWorkspace& w = h->hess;
+  if (!w.chol) {
+    cudaError_t ce = cudaMalloc(&w.chol, sizeof(double) * (size_t)np * np);
+    if (ce == cudaSuccess)
+      ce = cudaFuncSetAttribute(dia::cov_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(sizeof(double) * dia::kSolveWarps * np));
+    if (ce != cudaSuccess) {
+      cudaFree(w.chol);  w.chol = nullptr;
+      h->err = std::string("covariance workspace: ") + cudaGetErrorString(ce);
+      return DIA_ERR_ALLOC;
+    }
+  }
+  dia::cov_init_kernel<<<1, 1, 0, h->stream>>>(d_info);
+  for (int j = 0; j < np; ++j) {
+    const int rows = np - 1 - j;
+    const int grid = rows > 0 ? (rows + dia::kCholWarps - 1) / dia::kCholWarps : 1;
+    dia::chol_column_kernel<<<grid, dia::kCholWarps * 32, sizeof(double) * j, h->stream>>>(d_H, w.chol, np, j, d_info);
+  }
+  dia::cov_solve_kernel<<<(np + 1 + dia::kSolveWarps - 1) / dia::kSolveWarps, dia::kSolveWarps * 32,
+                          sizeof(double) * dia::kSolveWarps * np, h->stream>>>(w.chol, np, h->cfg.m * h->cfg.m, d_cov,
+                                                                                d_sigma, d_info);
+  if (d_cov) dia::hess_symmetrise_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(d_cov, np);
+  cudaError_t ce = cudaGetLastError();
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "covariance launch");
   return DIA_OK;
 }
 

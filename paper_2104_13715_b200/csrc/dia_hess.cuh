@@ -8,10 +8,11 @@ namespace dia {
 struct HessWorkspace {
   double* loss = nullptr;      // [np] scratch for the loss row of the partials (unused in Hessian mode)
   float* ident = nullptr;      // [np][np] identity: unit parameter vectors for the penalty's second derivative
+  double* chol = nullptr;      // [np][np] Cholesky factor of dia_covariance (L below, L' above the diagonal)
 };
 
 inline void hess_workspace_destroy(HessWorkspace* w) {
-  cudaFree(w->loss); cudaFree(w->ident);
+  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->chol);
   *w = HessWorkspace();
 }
 
