@@ -13,6 +13,7 @@
 #include <string>
 
 #include "dia_eval.cuh"
+#include "dia_eval_small.cuh"
 #include "dia_fit.cuh"
 #include "dia_hess.cuh"
 #include "dia_cov.cuh"
@@ -24,6 +25,8 @@ struct dia_handle {
   cudaStream_t stream;
   int grid, np, sms;       // grid: resident CTAs (SMs x occupancy), capped by max_epochs x tiles
   int tiles, n_refs;
+  int small_grid;          // > 0: the plain objective of this handle (m <= 5) runs eval_small_kernel on at most this many CTAs
+  int grid_limit;          // test hook DIA_GRID_LIMIT (0 = none)
   dia::ConstBlock* d_const_stage;   // staging copy of the constant block; non-null iff this handle may use the bank
   size_t smem;
   int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
@@ -173,9 +176,53 @@ static bool make_tensor_map(CUtensorMap* tm, const float* base, int n_cols, int 
 }
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
+static const void* small_kernel_for(int m) {
+  switch (m) {
+    case 1: return (const void*)dia::eval_small_kernel<1>;
+    case 3: return (const void*)dia::eval_small_kernel<3>;
+    case 5: return (const void*)dia::eval_small_kernel<5>;
+  }
+  return nullptr;
+}
+// Geometry of an eval_small_kernel launch (dia_eval_small.cuh): lanes side by side until they span the valid width,
+// and the largest number of rows per thread that still leaves three tiles per resident CTA.
+namespace dia { int eval_grid(const dia_handle* h, int n_epochs); int eval_part_cols(const dia_handle* h, int n_epochs); }
+struct SmallPlan { int rpt, lxlog, tiles, grid; };
+static SmallPlan small_plan(const dia_handle* h, int n_epochs) {
+  const int vc = h->cfg.n_cols - h->cfg.m + 1, vr = h->cfg.n_rows - h->cfg.m + 1;
+  SmallPlan sp;
+  sp.lxlog = 0;
+  while (sp.lxlog < 5 && (dia::kSmallPx << sp.lxlog) < vc) ++sp.lxlog;
+  const int tw = dia::kSmallPx << sp.lxlog, tx = (vc + tw - 1) / tw;
+  for (sp.rpt = 16; ; sp.rpt /= 2) {
+    const int th = (dia::kThreads / 32) * (32 >> sp.lxlog) * sp.rpt;
+    sp.tiles = tx * ((vr + th - 1) / th);
+    // (a full batch decides, so that every call on this handle cuts the image the same way: batched == singles)
+    if (sp.rpt == 2 || (long long)sp.tiles * h->cfg.max_epochs >= 3LL * h->small_grid) break;
+  }
+  const long long items = (long long)sp.tiles * n_epochs;
+  sp.grid = items < h->small_grid ? (int)items : h->small_grid;
+  return sp;
+}
+
 namespace dia {
 const void* eval_kernel_ptr(const dia_handle* h, bool aux) { return kernel_for(h->cfg.m, aux); }
 size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
+// the launch that evaluates p: kernel, grid, dynamic shared memory and the number of partial columns per epoch
+const void* eval_kernel_ptr_p(const dia_handle* h, const EvalParams& p) {
+  return p.small_rpt > 0 ? small_kernel_for(h->cfg.m) : kernel_for(h->cfg.m, eval_is_aux(p));
+}
+size_t eval_smem_bytes_p(const dia_handle* h, const EvalParams& p) { return p.small_rpt > 0 ? 0 : h->smem; }
+int eval_grid_p(const dia_handle* h, const EvalParams& p) {
+  return p.small_rpt > 0 ? small_plan(h, p.n_epochs).grid : eval_grid(h, p.n_epochs);
+}
+int eval_part_cols_p(const dia_handle* h, const EvalParams& p) {
+  if (p.small_rpt > 0) {
+    const SmallPlan sp = small_plan(h, p.n_epochs);
+    return sp.tiles < sp.grid ? sp.tiles : sp.grid;
+  }
+  return eval_part_cols(h, p.n_epochs);
+}
 // Many small images (at least one epoch per resident CTA): each CTA takes whole epochs, unless that balances the
 // CTAs more than 3 % worse than dealing the (epoch, tile) items out one by one.
 bool eval_by_epoch(const dia_handle* h, int n_epochs) {
@@ -200,7 +247,7 @@ bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff) {
   const int m = h->cfg.m, kp = (m + 3) / 4 * 4;
   const long long items = (long long)p.n_epochs * h->tiles;
   const long long waves = (items + h->grid - 1) / h->grid;
-  return h->d_const_stage && !diff && !eval_is_aux(p) && !eval_by_epoch(h, p.n_epochs) && waves * m * m >= 2 * 19 * 19 &&
+  return h->d_const_stage && !diff && p.small_rpt == 0 && !eval_is_aux(p) && !eval_by_epoch(h, p.n_epochs) && waves * m * m >= 2 * 19 * 19 &&
          p.n_epochs <= kConstEpochs &&
          (long long)p.n_epochs * m * kp <= kConstK;
 }
@@ -220,6 +267,10 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
     cudaError_t ce = cudaMemcpyToSymbolAsync(const_symbol_for(h->cfg.m), h->d_const_stage, const_block_bytes(h, p.n_epochs), 0,
                                              cudaMemcpyDeviceToDevice, h->stream);
     if (ce != cudaSuccess) return ce;
+  }
+  if (p.small_rpt > 0 && !diff) {
+    void* sargs[] = {(void*)&p};
+    return cudaLaunchKernel(small_kernel_for(h->cfg.m), dim3(eval_grid_p(h, p)), dim3(kThreads), sargs, 0, h->stream);
   }
   return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), diff, kc), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
                           h->smem, h->stream);
@@ -251,6 +302,13 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->inv_gain = c.noise == DIA_NOISE_MODEL ? 1.0f / c.gain : 0.f;
   p->use_tma = 0;
   p->epoch_per_cta = dia::eval_by_epoch(h, n_epochs) ? 1 : 0;
+  // plain objective with a small kernel: the register-resident kernel of dia_eval_small.cuh
+  p->small_rpt = 0;  p->small_lxlog = 0;  p->small_vec = 0;
+  if (h->small_grid > 0 && !d_mask && !d_var && hess_q0 < 0) {
+    const SmallPlan sp = small_plan(h, n_epochs);
+    p->small_rpt = sp.rpt;  p->small_lxlog = sp.lxlog;  p->epoch_per_cta = 0;
+    p->small_vec = (c.n_cols % 4 == 0 && aligned16(h->d_R) && aligned16(d_I)) ? 1 : 0;
+  }
   p->cp8 = (c.n_cols % 2 == 0) && (reinterpret_cast<uintptr_t>(h->d_R) & 7) == 0 && (reinterpret_cast<uintptr_t>(d_I) & 7) == 0;
   std::memset(tm, 0, sizeof(*tm));
   if (h->use_tma && aligned16(d_I) &&
@@ -312,11 +370,28 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   h->tiles = tiles;
   h->grid = sms * occ;                       // persistent grid: every CTA resident
   if ((long long)h->grid > (long long)tiles * cfg->max_epochs) h->grid = tiles * cfg->max_epochs;
+  h->grid_limit = 0;
   if (const char* lim = std::getenv("DIA_GRID_LIMIT")) {   // test hook: few CTAs => many tiles per CTA
     const int g = std::atoi(lim);
+    if (g >= 1) h->grid_limit = g;
     if (g >= 1 && g < h->grid) h->grid = g;
   }
-  ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * (tiles < h->grid ? tiles : h->grid) * (h->np + 1));
+  // m <= 5, no flat field, no background polynomial: eval_small_kernel evaluates the plain objective
+  h->small_grid = 0;
+  const char* no_small = std::getenv("DIA_DISABLE_SMALL");   // test hook: force the generic kernel
+  if (small_kernel_for(cfg->m) && !cfg->d_flat && cfg->bg_degree == 0 && cfg->noise == DIA_NOISE_MODEL &&
+      !(no_small && no_small[0] == '1')) {
+    int o = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, small_kernel_for(cfg->m), dia::kThreads, 0) == cudaSuccess && o >= 1) {
+      h->small_grid = sms * o;
+      if (h->grid_limit > 0 && h->grid_limit < h->small_grid) h->small_grid = h->grid_limit;
+    } else {
+      cudaGetLastError();
+    }
+  }
+  size_t part_cols = (size_t)(tiles < h->grid ? tiles : h->grid);
+  if ((size_t)h->small_grid > part_cols) part_cols = (size_t)h->small_grid;
+  ce = cudaMalloc(&h->d_partials, sizeof(double) * (size_t)cfg->max_epochs * part_cols * (h->np + 1));
   if (ce != cudaSuccess) { int rc = fail(nullptr, DIA_ERR_ALLOC, "workspace allocation failed"); cudaGetLastError(); delete h; return rc; }
   const char* no_const = std::getenv("DIA_DISABLE_CONST");   // test hook: force the shared-memory variant
   // a full batch would be a long enough launch (eval_uses_const): try to claim the constant block of this kernel size
@@ -375,7 +450,7 @@ static int eval_into(dia_handle* h, int n_epochs, const float* d_I, const unsign
   if (ce != cudaSuccess) return cuda_fail(h, ce, "eval launch");
   const int np1 = h->np + 1;
   dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, h->stream>>>(
-      h->d_partials, dia::eval_part_cols(h, n_epochs), np1, nullptr, d_loss, d_grad);
+      h->d_partials, dia::eval_part_cols_p(h, p), np1, nullptr, d_loss, d_grad);
   if (h->cfg.lambda_reg > 0.f && hess_q0 < 0)
     dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, h->stream>>>(d_theta, h->cfg.m, h->np, lambda_n(h), d_loss, d_grad);
   ce = cudaGetLastError();
@@ -472,6 +547,7 @@ extern "C" int dia_difference_image(dia_handle* h, int n_epochs, const float* d_
   fill_params(h, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm);
   p.part_rows = 3;
   p.diff = d_D;
+  if (p.small_rpt > 0) { p.small_rpt = 0;  p.epoch_per_cta = dia::eval_by_epoch(h, n_epochs) ? 1 : 0; }   // generic kernel
   ce = dia::launch_eval(h, p, tm, true);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "difference-image launch");
   dia::diff_metrics_kernel<<<n_epochs, 32, 0, h->stream>>>(h->d_partials, dia::eval_part_cols(h, n_epochs), d_metrics);
@@ -493,8 +569,8 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
   std::string err;
   const int unroll = 4;        // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
-  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid(h, n_epochs),
-                    dia::eval_part_cols(h, n_epochs), unroll, h->cfg.m, lambda_n(h), h->stream, &err);
+  rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid_p(h, p),
+                    dia::eval_part_cols_p(h, p), unroll, h->cfg.m, lambda_n(h), h->stream, &err);
   if (rc != DIA_OK) return fail(h, rc, err);
   return DIA_OK;
 }

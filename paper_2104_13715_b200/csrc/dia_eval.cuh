@@ -117,6 +117,9 @@ struct EvalParams {
                              // 1 = CTA b takes every tile of epochs b, b + grid, ... (many small images: one
                              // change of epoch per image instead of one per tile; partials have one column)
   int cp8;                   // cp.async staging path: 1 = rows are 8-byte aligned (even n_cols), copy pixel pairs
+  int small_rpt;             // > 0: eval_small_kernel (dia_eval_small.cuh) runs this evaluation, rows per thread and tile
+  int small_lxlog;           // ... log2 of the lanes of a warp that sit side by side in x (the rest stack in y)
+  int small_vec;             // ... rows of R and I are 16-byte aligned: 128-bit loads
 };
 
 struct TensorMaps {          // passed by value as a __grid_constant__ kernel parameter
