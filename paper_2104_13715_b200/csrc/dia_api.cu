@@ -176,14 +176,17 @@ static bool make_tensor_map(CUtensorMap* tm, const float* base, int n_cols, int 
 }
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
-static const void* small_kernel_for(int m) {
+static const void* small_kernel_for(int m, int loss = DIA_LOSS_GAUSSIAN) {
+  const bool hub = loss == DIA_LOSS_HUBER;
   switch (m) {
-    case 1: return (const void*)dia::eval_small_kernel<1>;
-    case 3: return (const void*)dia::eval_small_kernel<3>;
-    case 5: return (const void*)dia::eval_small_kernel<5>;
+    case 1: return hub ? (const void*)dia::eval_small_kernel<1, true> : (const void*)dia::eval_small_kernel<1, false>;
+    case 3: return hub ? (const void*)dia::eval_small_kernel<3, true> : (const void*)dia::eval_small_kernel<3, false>;
+    // m = 5 stays with the generic kernel: this design needs 180-230 registers per thread there (one CTA per SM) and
+    // was measured 12 % slower
   }
   return nullptr;
 }
+static size_t small_smem_for(int) { return 0; }   // static shared memory only
 // Geometry of an eval_small_kernel launch (dia_eval_small.cuh): lanes side by side until they span the valid width,
 // and the largest number of rows per thread that still leaves three tiles per resident CTA.
 namespace dia { int eval_grid(const dia_handle* h, int n_epochs); int eval_part_cols(const dia_handle* h, int n_epochs); }
@@ -210,9 +213,9 @@ const void* eval_kernel_ptr(const dia_handle* h, bool aux) { return kernel_for(h
 size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
 // the launch that evaluates p: kernel, grid, dynamic shared memory and the number of partial columns per epoch
 const void* eval_kernel_ptr_p(const dia_handle* h, const EvalParams& p) {
-  return p.small_rpt > 0 ? small_kernel_for(h->cfg.m) : kernel_for(h->cfg.m, eval_is_aux(p));
+  return p.small_rpt > 0 ? small_kernel_for(h->cfg.m, h->cfg.loss) : kernel_for(h->cfg.m, eval_is_aux(p));
 }
-size_t eval_smem_bytes_p(const dia_handle* h, const EvalParams& p) { return p.small_rpt > 0 ? 0 : h->smem; }
+size_t eval_smem_bytes_p(const dia_handle* h, const EvalParams& p) { return p.small_rpt > 0 ? small_smem_for(h->cfg.m) : h->smem; }
 int eval_grid_p(const dia_handle* h, const EvalParams& p) {
   return p.small_rpt > 0 ? small_plan(h, p.n_epochs).grid : eval_grid(h, p.n_epochs);
 }
@@ -270,7 +273,8 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
   }
   if (p.small_rpt > 0 && !diff) {
     void* sargs[] = {(void*)&p};
-    return cudaLaunchKernel(small_kernel_for(h->cfg.m), dim3(eval_grid_p(h, p)), dim3(kThreads), sargs, 0, h->stream);
+    return cudaLaunchKernel(small_kernel_for(h->cfg.m, h->cfg.loss), dim3(eval_grid_p(h, p)), dim3(kThreads), sargs,
+                            small_smem_for(h->cfg.m), h->stream);
   }
   return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), diff, kc), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
                           h->smem, h->stream);
@@ -382,7 +386,9 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   if (small_kernel_for(cfg->m) && !cfg->d_flat && cfg->bg_degree == 0 && cfg->noise == DIA_NOISE_MODEL &&
       !(no_small && no_small[0] == '1')) {
     int o = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, small_kernel_for(cfg->m), dia::kThreads, 0) == cudaSuccess && o >= 1) {
+    const void* ks = small_kernel_for(cfg->m, cfg->loss);
+    if (cudaFuncSetAttribute(ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem_for(cfg->m)) == cudaSuccess &&
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, ks, dia::kThreads, small_smem_for(cfg->m)) == cudaSuccess && o >= 1) {
       h->small_grid = sms * o;
       if (h->grid_limit > 0 && h->grid_limit < h->small_grid) h->small_grid = h->grid_limit;
     } else {

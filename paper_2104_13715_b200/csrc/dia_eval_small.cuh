@@ -1,4 +1,4 @@
-// dia_eval_small.cuh -- fused loss + gradient kernel for SMALL kernels (m = 1, 3, 5), plain objective only
+// dia_eval_small.cuh -- fused loss + gradient kernel for SMALL kernels (m = 1, 3; written for any odd m <= 5), plain objective only
 // (Eq. 2, 6, 8 / 12-13; no mask, flat field, variance map, background polynomial).
 //
 // For m <= 5 the evaluation has 4 m^2 <= 100 FLOP per 8 bytes of image: the roofline is HBM bandwidth (m <= 3) or
@@ -6,20 +6,24 @@
 // barriers per tile) cost more instructions per pixel than the arithmetic itself (87 per pixel at m = 3, ncu reading
 // in profiles/r01_sweeps.md).  Here everything stays in registers:
 //   * a thread owns an 8-pixel row strip and walks down `rpt` rows with a sliding window of the m reference rows it
-//     needs (one new row of 8 + m - 1 pixels per step, 128-bit loads straight from global memory -- neighbouring
-//     threads' halo re-reads hit L1), lanes of a warp sit side by side (coalesced 1 KB rows);
-//   * M, residual, variance, loss term and w = dL/dM per pixel as in the generic kernel (same pixel_terms);
+//     needs (one new row of 8 + m - 1 reference pixels and 8 target pixels per step, 128-bit loads straight from
+//     global memory, the rows four steps ahead requested from L2 by prefetch -- neighbouring threads' halo re-reads
+//     hit L1); lanes of a warp sit side by side (coalesced 1 KB rows);
+//   * M, residual, variance, loss term and w = dL/dM per pixel: the generic kernel's formulas, ln v from lg2.approx;
 //   * the m^2 gradient sums g[a][b] += w_q R[a][q + b] reuse the window registers: no w tile, no second pass;
 //   * per tile the m^2 FP32 sums are reduced across the warp by a transposing butterfly (lane k ends up with sum k)
 //     and added to a lane-held FP64 total; loss and g_B0 go to thread-private FP64 every row.
 // Work items, partial-column layout and the `done` flags are those of the generic kernel, so the second level
 // (reduce_partials_kernel / fit_step_kernel) is shared.  Fixed orders everywhere: bit-reproducible.
 #pragma once
+#include <type_traits>
+
 #include "dia_eval.cuh"
 
 namespace dia {
 
 constexpr int kSmallPx = 8;        // pixels per thread and row
+constexpr int kSmallAhead = 4;     // rows between the L2 prefetch of a row and its use
 
 __device__ __forceinline__ float4 ldg_hint_f4(const float* ptr, unsigned long long pol) {
   float4 v;
@@ -47,6 +51,11 @@ __device__ __forceinline__ void load_seg(const float* __restrict__ img, int n_ro
     for (int q = 0; q < SEG; ++q) r[q] = (row_ok && x + q < n_cols) ? __ldg(src + q) : 0.f;
   }
 }
+
+// Asks the L2 for the line that holds `ptr` (a row this thread reads kSmallAhead steps from now): the later load then
+// waits for an L2 hit instead of DRAM.  (Copying ahead into shared memory with per-thread cp.async was tried and was
+// 25 % slower: 16-byte copies with a 32-byte lane stride use the LSU poorly.)
+__device__ __forceinline__ void prefetch_l2(const float* ptr) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(ptr)); }
 
 // Transposing warp reduction of P = 1, 16 or 32 per-thread values: on return v[0] of lane l holds the sum over the
 // warp of value index l (P = 32), l >> 1 (P = 16), 0 (P = 1).  Fixed order.
@@ -83,8 +92,77 @@ struct SmallGeo {
   static constexpr int P = M == 1 ? 1 : (M == 3 ? 16 : 32);     // padded number of kernel-gradient sums
 };
 
-template <int M>
-__global__ void __launch_bounds__(kThreads, 2) eval_small_kernel(const EvalParams p) {
+// Per-pixel terms of the plain objective (D1; the formulas of pixel_terms<false, .> in
+// dia_eval.cuh) with the loss a template parameter and ln v from the MUFU unit (lg2.approx, absolute error 2^-22 in
+// log2 v: 1e-7 on a term of size 2-6).  hg = inv_gain / 2.
+template <bool HUBER>
+__device__ __forceinline__ void small_pixel_terms(float Mv, float Iv, float sigma0_sq, float inv_gain, float hg,
+                                                  float huber_c, float& li, float& wi) {
+  const float v = fmaf(inv_gain, fmaxf(Mv, 0.f), sigma0_sq);
+  const float hbp = Mv > 0.f ? hg : 0.f;
+  const float res = Iv - Mv;
+  const float inv_v = rcp_approx(v);
+  const float hb = hbp * inv_v;                    // b' / (2 v)
+  const float rv = res * inv_v;
+  const float z2 = res * rv;
+  const float hlv = 0.34657359028f * __log2f(v);   // ln(v) / 2
+  li = fmaf(0.5f, z2, hlv);
+  wi = fmaf(hb, 1.0f - z2, -rv);
+  if (HUBER) {                                     // Eq. 12
+    const float rsd = rsqrtf(v);
+    const float z = res * rsd;
+    if (fabsf(z) > huber_c) {
+      const float psi = copysignf(huber_c, z);
+      li = fmaf(huber_c, fabsf(z) - 0.5f * huber_c, hlv);
+      wi = fmaf(-psi, rsd, hb * (1.0f - psi * z));
+    }
+  }
+}
+
+// One row of a strip: model, per-pixel terms, gradient sums.  EDGE: the strip crosses the right edge of the valid
+// region, pixels beyond it contribute nothing (selects, not multiplications: zero-filled pixels may give NaN).
+template <int M, int U, bool HUBER, bool EDGE>
+__device__ __forceinline__ void small_row(const float (&win)[M][SmallGeo<M>::SEG], const float (&iv)[SmallGeo<M>::SEG],
+                                          const float* __restrict__ K, float B0, const EvalParams& p, float hg, int n_in,
+                                          float (&acc)[SmallGeo<M>::P], double& loss64, double& gb064) {
+  constexpr int H = SmallGeo<M>::H;
+  // window row a lives in win[(U + a) % M].  One FP32 chain per pixel, wings first, the centre pixel last (the
+  // largest terms of a peaked kernel come last; with m^2 <= 25 terms the order matters little)
+  float tot[kSmallPx];
+#pragma unroll
+  for (int q = 0; q < kSmallPx; ++q) tot[q] = B0;
+#pragma unroll
+  for (int ia = 0; ia < M; ++ia) {
+    const int a = (ia & 1) ? (M - 1 - (ia >> 1)) : (ia >> 1);       // 0, M-1, 1, M-2, ..., centre
+#pragma unroll
+    for (int ib = 0; ib < M; ++ib) {
+      const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
+      const float k = K[a * M + b];
+#pragma unroll
+      for (int q = 0; q < kSmallPx; ++q) tot[q] = fmaf(k, win[(U + a) % M][q + b], tot[q]);
+    }
+  }
+  float lsum = 0.f, wsum = 0.f;
+#pragma unroll
+  for (int q = 0; q < kSmallPx; ++q) {
+    float li, wi;
+    small_pixel_terms<HUBER>(tot[q], iv[q + H], p.sigma0_sq, p.inv_gain, hg, p.huber_c, li, wi);
+    if (EDGE) {
+      if (q >= n_in) { li = 0.f; wi = 0.f; }
+    }
+    lsum += li;
+    wsum += wi;
+#pragma unroll
+    for (int a = 0; a < M; ++a)
+#pragma unroll
+      for (int b = 0; b < M; ++b) acc[a * M + b] = fmaf(wi, win[(U + a) % M][q + b], acc[a * M + b]);
+  }
+  loss64 += (double)lsum;
+  gb064 += (double)wsum;
+}
+
+template <int M, bool HUBER>
+__global__ void __launch_bounds__(kThreads, M == 1 ? 3 : (M == 3 ? 2 : 1)) eval_small_kernel(const EvalParams p) {
   using G = SmallGeo<M>;
   constexpr int SEG = G::SEG, P = G::P, H = G::H;
   __shared__ double red[kThreads / 32][32];
@@ -100,6 +178,7 @@ __global__ void __launch_bounds__(kThreads, 2) eval_small_kernel(const EvalParam
   const int n_tiles = tiles_x * tiles_y;
   const size_t npix = (size_t)p.n_rows * p.n_cols;
   const bool vec = p.small_vec != 0;
+  const float hg = 0.5f * p.inv_gain;
   const unsigned long long pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
 
   const int grid = (int)gridDim.x;
@@ -159,62 +238,40 @@ __global__ void __launch_bounds__(kThreads, 2) eval_small_kernel(const EvalParam
     const int x0 = tile_x * tile_w + kSmallPx * lx;                       // first pixel of the strip (valid coords)
     const int y0 = tile_y * tile_h + (warp * (32 >> lxlog) + ly) * rpt;   // first row of this thread
     const int nrows = min(rpt, vr - y0);                                  // <= 0: nothing to do
+    const int n_in = vc - x0;                                             // pixels of the strip inside the valid region
     const float* __restrict__ Rimg = p.R + (p.n_refs > 1 ? (size_t)e * npix : (size_t)0);
     const float* __restrict__ Iimg = p.I + (size_t)e * npix;
 
     float acc[P];
 #pragma unroll
     for (int i = 0; i < P; ++i) acc[i] = 0.f;
-    if (x0 < vc && nrows > 0) {
+    if (n_in > 0 && nrows > 0) {
+      const float* __restrict__ Rrow = Rimg + (size_t)(y0 + M - 1) * p.n_cols + x0;   // new window row of step 0
+      const float* __restrict__ Irow = Iimg + (size_t)(y0 + H) * p.n_cols + x0;
       float win[M][SEG];
 #pragma unroll
       for (int a = 0; a < M - 1; ++a) load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + a, x0, vec, pol_keep, win[a]);
 #pragma unroll 1
       for (int r0 = 0; r0 < nrows; r0 += M) {
-#pragma unroll
-        for (int u = 0; u < M; ++u) {
-          const int r = r0 + u;
+        // M steps with compile-time window rotation: the new bottom row of step u goes to win[(u + M - 1) % M]
+        auto body = [&](auto uc) {
+          constexpr int U = decltype(uc)::value;
+          const int r = r0 + U;
           if (r < nrows) {
-            // window row a of this step lives in win[(u + a) % M]; the new bottom row goes to win[(u + M - 1) % M]
-            load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + r + M - 1, x0, vec, pol_keep, win[(u + M - 1) % M]);
+            if (r + kSmallAhead < nrows) {
+              prefetch_l2(Rrow + (size_t)(r + kSmallAhead) * p.n_cols);
+              prefetch_l2(Irow + (size_t)(r + kSmallAhead) * p.n_cols);
+            }
+            load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + r + M - 1, x0, vec, pol_keep, win[(U + M - 1) % M]);
             float iv[SEG];
             load_seg<SEG>(Iimg, p.n_rows, p.n_cols, y0 + r + H, x0, vec, pol_stream, iv);
-            // model: kernel rows in pairs (0, M-1), (1, M-2), ..., centre last; columns wings -> centre
-            float tot[kSmallPx];
-#pragma unroll
-            for (int q = 0; q < kSmallPx; ++q) tot[q] = B0;
-#pragma unroll
-            for (int ia = 0; ia < M; ++ia) {
-              const int a = (ia & 1) ? (M - 1 - (ia >> 1)) : (ia >> 1);
-              float rs[kSmallPx];
-#pragma unroll
-              for (int ib = 0; ib < M; ++ib) {
-                const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
-#pragma unroll
-                for (int q = 0; q < kSmallPx; ++q) {
-                  const float rv = win[(u + a) % M][q + b];
-                  rs[q] = ib == 0 ? K[a * M + b] * rv : fmaf(K[a * M + b], rv, rs[q]);
-                }
-              }
-#pragma unroll
-              for (int q = 0; q < kSmallPx; ++q) tot[q] += rs[q];
-            }
-            float lsum = 0.f, wsum = 0.f;
-#pragma unroll
-            for (int q = 0; q < kSmallPx; ++q) {
-              float li, wi;
-              pixel_terms<false, true>(p, e, npix, 0, x0 + q < vc, tot[q], iv[q + H], li, wi);
-              lsum += li;
-              wsum += wi;
-#pragma unroll
-              for (int a = 0; a < M; ++a)
-#pragma unroll
-                for (int b = 0; b < M; ++b) acc[a * M + b] = fmaf(wi, win[(u + a) % M][q + b], acc[a * M + b]);
-            }
-            loss64 += (double)lsum;
-            gb064 += (double)wsum;
+            if (n_in >= kSmallPx) small_row<M, U, HUBER, false>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
+            else small_row<M, U, HUBER, true>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
           }
-        }
+        };
+        body(std::integral_constant<int, 0>());
+        if constexpr (M >= 3) { body(std::integral_constant<int, 1>()); body(std::integral_constant<int, 2>()); }
+        if constexpr (M >= 5) { body(std::integral_constant<int, 3>()); body(std::integral_constant<int, 4>()); }
       }
     }
     warp_transpose_sum<P>(acc, lane);

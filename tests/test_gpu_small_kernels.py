@@ -1,5 +1,6 @@
-"""GPU-vs-oracle parity of the register-resident kernel for small kernels (m = 1, 3, 5; dia_eval_small.cuh), which
-evaluates the plain objective (no mask / flat / variance map / background polynomial) of handles with m <= 5.
+"""GPU-vs-oracle parity of the register-resident kernel for small kernels (m = 1, 3; dia_eval_small.cuh), which
+evaluates the plain objective (no mask / flat / variance map / background polynomial) of handles with m <= 3
+(m = 5 is listed too: it runs the generic kernel on the same shapes).
 
 Same protocol as tests/test_gpu_parity.py (loss to 1e-5 relative, gradient to 1e-5 of the cancellation-free scale S_p),
 on shapes chosen for this kernel's geometry: 8-pixel strips, lanes side by side up to 256 columns, 2-16 rows per thread,
@@ -73,7 +74,7 @@ def test_small_kernel_parity(dia, nr, nc, m, loss):
     h.close()
 
 
-@pytest.mark.parametrize("m", [1, 3, 5])
+@pytest.mark.parametrize("m", [1, 3])
 def test_small_kernel_is_the_one_that_runs_and_agrees_with_the_generic_kernel(dia, monkeypatch, m):
     """DIA_DISABLE_SMALL=1 forces the generic shared-memory kernel: both must agree with the oracle, and with each other
     far inside the tolerance; a mask (generic kernel on the same handle) of all ones gives the generic result."""
@@ -118,12 +119,12 @@ def test_small_kernel_many_tiles_per_cta_batched_and_singles(dia, monkeypatch, g
 
 def test_small_kernel_unpoisoned_by_border_and_minimum_size(dia):
     """NaN in the border of I (outside the valid set) must not reach a result; n == m leaves one valid pixel."""
-    w = make_workload(0, n=128, m=5)
-    h = dia.Handle(_dev(w.R), 5, sigma0=w.sigma0, gain=w.gain)
+    w = make_workload(0, n=128, m=3)
+    h = dia.Handle(_dev(w.R), 3, sigma0=w.sigma0, gain=w.gain)
     th = _dev(w.theta_true.astype(np.float32))
     L0, g0 = h.eval_loss_grad(_dev(w.I), th)
     Ip = w.I.copy()
-    Ip[:, :2, :] = np.nan; Ip[:, -2:, :] = np.nan; Ip[:, :, :2] = np.nan; Ip[:, :, -2:] = np.nan
+    Ip[:, :1, :] = np.nan; Ip[:, -1:, :] = np.nan; Ip[:, :, :1] = np.nan; Ip[:, :, -1:] = np.nan
     L1, g1 = h.eval_loss_grad(_dev(Ip), th)
     assert torch.equal(L0, L1) and torch.equal(g0, g1)
     h.close()
