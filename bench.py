@@ -233,10 +233,11 @@ def sweeps(dia, dev):
     from workloads import make_workload
     w = make_workload(4, n_epochs=1)
     peak = SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    hbm_peak = float(measured_peaks().get("hbm_gbs") or 6650.0)   # MEASURED_PEAKS.json, else B200_PROFILING.md's fallback
     cases = [(n, m, 1) for m in (19, 25) for n in (512, 1024, 2048, 4096)]
-    cases += [(1024, m, 1) for m in (3, 5, 7, 11, 15, 23, 31, 39, 47)] + [(4096, 47, 1)]
+    cases += [(1024, m, 1) for m in (1, 3, 5, 7, 11, 15, 23, 31, 39, 47)] + [(4096, 47, 1)]
     # small kernels on a batch larger than L2 (16 copies of the target: 1 GiB): the HBM-side regime of SURVEY.md 8(d)
-    cases += [(4096, m, 16) for m in (3, 5, 7)]
+    cases += [(4096, m, 16) for m in (1, 3, 5, 7)]
     out = []
     for n, m, E in cases:
         R = torch.from_numpy(np.ascontiguousarray(w.R[:n, :n])).to(dev)
@@ -260,7 +261,8 @@ def sweeps(dia, dev):
         out.append({"n": n, "m": m, "epochs": E, "us_per_eval": round(1e3 * ms / E, 2), "evals_per_s": round(1e3 * E / ms, 1),
                     "tflops": round(2.0 * useful_fma(n, m, E) / (ms * 1e-3) / 1e12, 3),
                     "frac_fp32_nominal": round(2.0 * useful_fma(n, m, E) / (ms * 1e-3) / 1e12 / peak, 4),
-                    "algorithmic_GBps": round(4.0 * n * n * (1 + E) / (ms * 1e-3) / 1e9, 1)})
+                    "algorithmic_GBps": round(4.0 * n * n * (1 + E) / (ms * 1e-3) / 1e9, 1),
+                    "frac_hbm_measured": round(4.0 * n * n * (1 + E) / (ms * 1e-3) / 1e9 / hbm_peak, 4)})
     return out
 
 

@@ -52,6 +52,16 @@ __device__ __forceinline__ void load_seg(const float* __restrict__ img, int n_ro
   }
 }
 
+// The same for a strip that lies inside the image with 16-byte aligned rows: no predicates, no zero fill.
+template <int SEG>
+__device__ __forceinline__ void load_fast(const float* __restrict__ src, unsigned long long pol, float (&r)[SEG]) {
+#pragma unroll
+  for (int q = 0; q < SEG / 4; ++q) {
+    const float4 v = ldg_hint_f4(src + 4 * q, pol);
+    r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
+  }
+}
+
 // Asks the L2 for the line that holds `ptr` (a row this thread reads kSmallAhead steps from now): the later load then
 // waits for an L2 hit instead of DRAM.  (Copying ahead into shared memory with per-thread cp.async was tried and was
 // 25 % slower: 16-byte copies with a 32-byte lane stride use the LSU poorly.)
@@ -161,6 +171,73 @@ __device__ __forceinline__ void small_row(const float (&win)[M][SmallGeo<M>::SEG
   gb064 += (double)wsum;
 }
 
+// All rows of one thread's strip in one tile.  FAST: the strip's segments lie inside the image and rows are 16-byte
+// aligned (every strip but the last of an image row): unpredicated 128-bit loads through running pointers; for
+// m = 1, where nothing but the loads stands between the kernel and the HBM roofline, the next row is loaded into a
+// second register set before the current one is used.
+template <int M, bool HUBER, bool FAST>
+__device__ __forceinline__ void small_strip(const EvalParams& p, const float* __restrict__ Rimg, const float* __restrict__ Iimg,
+                                            int y0, int x0, int nrows, int n_in, bool vec, unsigned long long pol_keep,
+                                            unsigned long long pol_stream, const float* __restrict__ K, float B0, float hg,
+                                            float (&acc)[SmallGeo<M>::P], double& loss64, double& gb064) {
+  using G = SmallGeo<M>;
+  constexpr int SEG = G::SEG, H = G::H;
+  const size_t pitch = (size_t)p.n_cols;
+  const float* __restrict__ Rp = Rimg + (size_t)(y0 + M - 1) * pitch + x0;   // new window row of the current step
+  const float* __restrict__ Ip = Iimg + (size_t)(y0 + H) * pitch + x0;      // target row of the current step
+  if constexpr (M == 1 && FAST) {
+    float rA[1][SEG], iA[SEG], rB[1][SEG], iB[SEG];
+    load_fast<SEG>(Rp, pol_keep, rA[0]);
+    load_fast<SEG>(Ip, pol_stream, iA);
+#pragma unroll 1
+    for (int r = 0; r < nrows; r += 2) {
+      if (r + kSmallAhead < nrows) { prefetch_l2(Rp + kSmallAhead * pitch); prefetch_l2(Ip + kSmallAhead * pitch); }
+      if (r + 1 < nrows) { load_fast<SEG>(Rp + pitch, pol_keep, rB[0]); load_fast<SEG>(Ip + pitch, pol_stream, iB); }
+      small_row<M, 0, HUBER, false>(rA, iA, K, B0, p, hg, n_in, acc, loss64, gb064);
+      if (r + 1 < nrows) {
+        if (r + 2 < nrows) { load_fast<SEG>(Rp + 2 * pitch, pol_keep, rA[0]); load_fast<SEG>(Ip + 2 * pitch, pol_stream, iA); }
+        small_row<M, 0, HUBER, false>(rB, iB, K, B0, p, hg, n_in, acc, loss64, gb064);
+      }
+      Rp += 2 * pitch;
+      Ip += 2 * pitch;
+    }
+  } else {
+    float win[M][SEG];
+#pragma unroll
+    for (int a = 0; a < M - 1; ++a) {
+      if constexpr (FAST) load_fast<SEG>(Rimg + (size_t)(y0 + a) * pitch + x0, pol_keep, win[a]);
+      else load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + a, x0, vec, pol_keep, win[a]);
+    }
+#pragma unroll 1
+    for (int r0 = 0; r0 < nrows; r0 += M) {
+      // M steps with compile-time window rotation: the new bottom row of step u goes to win[(u + M - 1) % M]
+      auto body = [&](auto uc) {
+        constexpr int U = decltype(uc)::value;
+        const int r = r0 + U;
+        if (r < nrows) {
+          if (r + kSmallAhead < nrows) { prefetch_l2(Rp + kSmallAhead * pitch); prefetch_l2(Ip + kSmallAhead * pitch); }
+          float iv[SEG];
+          if constexpr (FAST) {
+            load_fast<SEG>(Rp, pol_keep, win[(U + M - 1) % M]);
+            load_fast<SEG>(Ip, pol_stream, iv);
+            small_row<M, U, HUBER, false>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
+          } else {
+            load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + r + M - 1, x0, vec, pol_keep, win[(U + M - 1) % M]);
+            load_seg<SEG>(Iimg, p.n_rows, p.n_cols, y0 + r + H, x0, vec, pol_stream, iv);
+            if (n_in >= kSmallPx) small_row<M, U, HUBER, false>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
+            else small_row<M, U, HUBER, true>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
+          }
+          Rp += pitch;
+          Ip += pitch;
+        }
+      };
+      body(std::integral_constant<int, 0>());
+      if constexpr (M >= 3) { body(std::integral_constant<int, 1>()); body(std::integral_constant<int, 2>()); }
+      if constexpr (M >= 5) { body(std::integral_constant<int, 3>()); body(std::integral_constant<int, 4>()); }
+    }
+  }
+}
+
 template <int M, bool HUBER>
 __global__ void __launch_bounds__(kThreads, M == 1 ? 3 : (M == 3 ? 2 : 1)) eval_small_kernel(const EvalParams p) {
   using G = SmallGeo<M>;
@@ -246,33 +323,10 @@ __global__ void __launch_bounds__(kThreads, M == 1 ? 3 : (M == 3 ? 2 : 1)) eval_
 #pragma unroll
     for (int i = 0; i < P; ++i) acc[i] = 0.f;
     if (n_in > 0 && nrows > 0) {
-      const float* __restrict__ Rrow = Rimg + (size_t)(y0 + M - 1) * p.n_cols + x0;   // new window row of step 0
-      const float* __restrict__ Irow = Iimg + (size_t)(y0 + H) * p.n_cols + x0;
-      float win[M][SEG];
-#pragma unroll
-      for (int a = 0; a < M - 1; ++a) load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + a, x0, vec, pol_keep, win[a]);
-#pragma unroll 1
-      for (int r0 = 0; r0 < nrows; r0 += M) {
-        // M steps with compile-time window rotation: the new bottom row of step u goes to win[(u + M - 1) % M]
-        auto body = [&](auto uc) {
-          constexpr int U = decltype(uc)::value;
-          const int r = r0 + U;
-          if (r < nrows) {
-            if (r + kSmallAhead < nrows) {
-              prefetch_l2(Rrow + (size_t)(r + kSmallAhead) * p.n_cols);
-              prefetch_l2(Irow + (size_t)(r + kSmallAhead) * p.n_cols);
-            }
-            load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + r + M - 1, x0, vec, pol_keep, win[(U + M - 1) % M]);
-            float iv[SEG];
-            load_seg<SEG>(Iimg, p.n_rows, p.n_cols, y0 + r + H, x0, vec, pol_stream, iv);
-            if (n_in >= kSmallPx) small_row<M, U, HUBER, false>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
-            else small_row<M, U, HUBER, true>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
-          }
-        };
-        body(std::integral_constant<int, 0>());
-        if constexpr (M >= 3) { body(std::integral_constant<int, 1>()); body(std::integral_constant<int, 2>()); }
-        if constexpr (M >= 5) { body(std::integral_constant<int, 3>()); body(std::integral_constant<int, 4>()); }
-      }
+      if (vec && n_in >= kSmallPx && x0 + SEG <= p.n_cols)
+        small_strip<M, HUBER, true>(p, Rimg, Iimg, y0, x0, nrows, n_in, vec, pol_keep, pol_stream, K, B0, hg, acc, loss64, gb064);
+      else
+        small_strip<M, HUBER, false>(p, Rimg, Iimg, y0, x0, nrows, n_in, vec, pol_keep, pol_stream, K, B0, hg, acc, loss64, gb064);
     }
     warp_transpose_sum<P>(acc, lane);
     g64 += (double)acc[0];
