@@ -45,7 +45,7 @@ UNIT = "evals/s"
 SM_COUNT, FP32_LANES_PER_SM = 148, 128          # B200 (B200_PROFILING.md: 148 SMs; 128 FP32 lanes per SM)
 # dram__bytes_read.sum + dram__bytes_write.sum of one eval_kernel<19,false> launch over the 16-epoch batch,
 # from the ncu --set full capture summarised in profiles/ (None until captured)
-TRAFFIC_BYTES_PER_LAUNCH = 1.430e9     # profiles/r01_eval_kernel_full.md
+TRAFFIC_BYTES_PER_LAUNCH = 1.403e9     # profiles/r01_eval_kernel_full.md (last capture of r01: 1.388 GB read + 15.6 MB written)
 
 
 def useful_fma(n=N, m=M, epochs=1):
