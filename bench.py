@@ -460,6 +460,33 @@ def run_gpu(args):
             line["fits"]["covariance"] = {"ms": ms_c, "np": rows, "launches": rows + 3, "valid": ci[0],
                                           "sigma_P": ci[2], "sigma_B0": float(sig_hat[M * M])}
 
+    # ---- small kernels on the same resident batch: the HBM side of the roofline
+    if rank == 0 and not args.no_stamps:
+        hbm_peak = float(peaks.get("hbm_gbs") or 6650.0)
+        line["small_kernels"] = []
+        for ms_ in (1, 3):
+            hs = dia.Handle(dR, ms_, max_epochs=E, sigma0=cfg.sigma0, gain=cfg.gain)
+            ths = torch.full((E, ms_ * ms_ + 1), 1.0 / (ms_ * ms_), dtype=torch.float32, device=dev)
+            ths[:, -1] = 0.0
+            Ls = torch.empty(E, dtype=torch.float64, device=dev)
+            Gs = torch.empty((E, ms_ * ms_ + 1), dtype=torch.float64, device=dev)
+            for _ in range(3):
+                hs.eval_loss_grad(dI, ths, loss=Ls, grad=Gs)
+            ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)   # rank 0 only:
+            torch.cuda.synchronize()                                                                  # no barrier here
+            ev_a.record()
+            for _ in range(20):
+                hs.eval_loss_grad(dI, ths, loss=Ls, grad=Gs)
+            ev_b.record()
+            torch.cuda.synchronize()
+            ms_s = ev_a.elapsed_time(ev_b)
+            hs.close()
+            gbs = 4.0 * N * N * (1 + E) / (ms_s / 20 * 1e-3) / 1e9
+            line["small_kernels"].append({"m": ms_, "epochs": E, "us_per_epoch": 1e3 * ms_s / 20 / E,
+                                          "evals_per_s": E * 20 / (ms_s * 1e-3), "bound": "hbm",
+                                          "algorithmic_GBps": gbs, "hbm_peak_gbs": hbm_peak, "frac": gbs / hbm_peak,
+                                          "kernel": f"dia::eval_small_kernel<{ms_}, false>"})
+
     # ---- many small image pairs, one reference each (the paper's stamp workloads)
     if rank == 0 and not args.no_stamps:
         line["stamps"] = stamp_batch_rate(dia, dev)

@@ -187,6 +187,7 @@ static const void* small_kernel_for(int m, int loss = DIA_LOSS_GAUSSIAN) {
   return nullptr;
 }
 static size_t small_smem_for(int) { return 0; }   // static shared memory only
+static int small_threads_for(int m) { return m == 1 ? dia::SmallGeo<1>::THREADS : dia::SmallGeo<3>::THREADS; }
 // Geometry of an eval_small_kernel launch (dia_eval_small.cuh): lanes side by side until they span the valid width,
 // and the largest number of rows per thread that still leaves three tiles per resident CTA.
 namespace dia { int eval_grid(const dia_handle* h, int n_epochs); int eval_part_cols(const dia_handle* h, int n_epochs); }
@@ -198,7 +199,7 @@ static SmallPlan small_plan(const dia_handle* h, int n_epochs) {
   while (sp.lxlog < 5 && (dia::kSmallPx << sp.lxlog) < vc) ++sp.lxlog;
   const int tw = dia::kSmallPx << sp.lxlog, tx = (vc + tw - 1) / tw;
   for (sp.rpt = 16; ; sp.rpt /= 2) {
-    const int th = (dia::kThreads / 32) * (32 >> sp.lxlog) * sp.rpt;
+    const int th = (small_threads_for(h->cfg.m) / 32) * (32 >> sp.lxlog) * sp.rpt;
     sp.tiles = tx * ((vr + th - 1) / th);
     // (a full batch decides, so that every call on this handle cuts the image the same way: batched == singles)
     if (sp.rpt == 2 || (long long)sp.tiles * h->cfg.max_epochs >= 3LL * h->small_grid) break;
@@ -215,6 +216,7 @@ size_t eval_smem_bytes(const dia_handle* h) { return h->smem; }
 const void* eval_kernel_ptr_p(const dia_handle* h, const EvalParams& p) {
   return p.small_rpt > 0 ? small_kernel_for(h->cfg.m, h->cfg.loss) : kernel_for(h->cfg.m, eval_is_aux(p));
 }
+int eval_threads_p(const dia_handle* h, const EvalParams& p) { return p.small_rpt > 0 ? small_threads_for(h->cfg.m) : kThreads; }
 size_t eval_smem_bytes_p(const dia_handle* h, const EvalParams& p) { return p.small_rpt > 0 ? small_smem_for(h->cfg.m) : h->smem; }
 int eval_grid_p(const dia_handle* h, const EvalParams& p) {
   return p.small_rpt > 0 ? small_plan(h, p.n_epochs).grid : eval_grid(h, p.n_epochs);
@@ -273,7 +275,7 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
   }
   if (p.small_rpt > 0 && !diff) {
     void* sargs[] = {(void*)&p};
-    return cudaLaunchKernel(small_kernel_for(h->cfg.m, h->cfg.loss), dim3(eval_grid_p(h, p)), dim3(kThreads), sargs,
+    return cudaLaunchKernel(small_kernel_for(h->cfg.m, h->cfg.loss), dim3(eval_grid_p(h, p)), dim3(small_threads_for(h->cfg.m)), sargs,
                             small_smem_for(h->cfg.m), h->stream);
   }
   return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), diff, kc), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
@@ -388,7 +390,7 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
     int o = 0;
     const void* ks = small_kernel_for(cfg->m, cfg->loss);
     if (cudaFuncSetAttribute(ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)small_smem_for(cfg->m)) == cudaSuccess &&
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, ks, dia::kThreads, small_smem_for(cfg->m)) == cudaSuccess && o >= 1) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, ks, small_threads_for(cfg->m), small_smem_for(cfg->m)) == cudaSuccess && o >= 1) {
       h->small_grid = sms * o;
       if (h->grid_limit > 0 && h->grid_limit < h->small_grid) h->small_grid = h->grid_limit;
     } else {

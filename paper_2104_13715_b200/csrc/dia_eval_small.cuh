@@ -101,6 +101,10 @@ struct SmallGeo {
   static constexpr int H = (M - 1) / 2;
   static constexpr int SEG = round_up(kSmallPx + M - 1, 4);     // 8 (m = 1) or 12 floats per window row
   static constexpr int P = M == 1 ? 1 : (M == 3 ? 16 : 32);     // padded number of kernel-gradient sums
+  // m = 1: 3 CTAs of 8 warps at 80 registers; m = 3: 2 CTAs at 128 registers (3 CTAs of 7 warps at 96 registers, or
+  // of 8 warps at 80, spill and were measured 19 % and 13 % slower); m = 5: one CTA
+  static constexpr int THREADS = 256;
+  static constexpr int MAXREG = M == 1 ? 80 : (M == 3 ? 128 : 255);
 };
 
 __device__ __forceinline__ float lg2_approx(float x) {      // v is a variance: never subnormal, so no rescaling step
@@ -145,25 +149,21 @@ __device__ __forceinline__ void small_row(const float (&win)[M][SmallGeo<M>::SEG
   constexpr int H = SmallGeo<M>::H;
   // window row a lives in win[(U + a) % M].  One FP32 chain per pixel, wings first, the centre pixel last (the
   // largest terms of a peaked kernel come last; with m^2 <= 25 terms the order matters little)
-  float tot[kSmallPx];
-#pragma unroll
-  for (int q = 0; q < kSmallPx; ++q) tot[q] = B0;
-#pragma unroll
-  for (int ia = 0; ia < M; ++ia) {
-    const int a = (ia & 1) ? (M - 1 - (ia >> 1)) : (ia >> 1);       // 0, M-1, 1, M-2, ..., centre
-#pragma unroll
-    for (int ib = 0; ib < M; ++ib) {
-      const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
-      const float k = K[a * M + b];
-#pragma unroll
-      for (int q = 0; q < kSmallPx; ++q) tot[q] = fmaf(k, win[(U + a) % M][q + b], tot[q]);
-    }
-  }
   float lsum = 0.f, wsum = 0.f;
 #pragma unroll
   for (int q = 0; q < kSmallPx; ++q) {
+    float tot = B0;
+#pragma unroll
+    for (int ia = 0; ia < M; ++ia) {
+      const int a = (ia & 1) ? (M - 1 - (ia >> 1)) : (ia >> 1);       // 0, M-1, 1, M-2, ..., centre
+#pragma unroll
+      for (int ib = 0; ib < M; ++ib) {
+        const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
+        tot = fmaf(K[a * M + b], win[(U + a) % M][q + b], tot);
+      }
+    }
     float li, wi;
-    small_pixel_terms<HUBER>(tot[q], iv[q + H], p.sigma0_sq, p.inv_gain, hg, p.huber_c, li, wi);
+    small_pixel_terms<HUBER>(tot, iv[q + H], p.sigma0_sq, p.inv_gain, hg, p.huber_c, li, wi);
     if (EDGE) {
       if (q >= n_in) { li = 0.f; wi = 0.f; }
     }
@@ -246,17 +246,17 @@ __device__ __forceinline__ void small_strip(const EvalParams& p, const float* __
 }
 
 template <int M, bool HUBER>
-__global__ void __launch_bounds__(kThreads, M == 1 ? 3 : (M == 3 ? 2 : 1)) eval_small_kernel(const EvalParams p) {
+__global__ void __maxnreg__(SmallGeo<M>::MAXREG) eval_small_kernel(const EvalParams p) {
   using G = SmallGeo<M>;
   constexpr int SEG = G::SEG, P = G::P, H = G::H;
-  __shared__ double red[kThreads / 32][32];
-  __shared__ double red2[2][kThreads / 32];
+  __shared__ double red[(G::THREADS / 32)][32];
+  __shared__ double red2[2][(G::THREADS / 32)];
   __shared__ float K[M * M];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int lxlog = p.small_lxlog, rpt = p.small_rpt;
   const int lx = lane & ((1 << lxlog) - 1), ly = lane >> lxlog;
   const int rows_per_warp = (32 >> lxlog) * rpt;
-  const int tile_w = kSmallPx << lxlog, tile_h = (kThreads / 32) * rows_per_warp;
+  const int tile_w = kSmallPx << lxlog, tile_h = ((G::THREADS / 32)) * rows_per_warp;
   const int vr = p.n_rows - M + 1, vc = p.n_cols - M + 1;
   const int tiles_x = (vc + tile_w - 1) / tile_w, tiles_y = (vr + tile_h - 1) / tile_h;
   const int n_tiles = tiles_x * tiles_y;
@@ -289,13 +289,13 @@ __global__ void __launch_bounds__(kThreads, M == 1 ? 3 : (M == 3 ? 2 : 1)) eval_
       const int src = P == 32 ? tid : (P == 16 ? 2 * tid : 0);
       double s = 0.0;
 #pragma unroll
-      for (int w = 0; w < kThreads / 32; ++w) s += red[w][src];
+      for (int w = 0; w < (G::THREADS / 32); ++w) s += red[w][src];
       out[(size_t)tid * ncols] = s;
     }
     if (tid == 32) {
       double ls = 0.0, gs = 0.0;
 #pragma unroll
-      for (int w = 0; w < kThreads / 32; ++w) { ls += red2[0][w]; gs += red2[1][w]; }
+      for (int w = 0; w < (G::THREADS / 32); ++w) { ls += red2[0][w]; gs += red2[1][w]; }
       out[(size_t)(M * M) * ncols] = gs;
       out[(size_t)p.np * ncols] = ls;
     }

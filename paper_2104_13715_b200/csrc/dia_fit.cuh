@@ -34,6 +34,7 @@ const void* const_symbol(const dia_handle* h);
 size_t eval_smem_bytes(const dia_handle* h);
 const void* eval_kernel_ptr_p(const dia_handle* h, const EvalParams& p);
 size_t eval_smem_bytes_p(const dia_handle* h, const EvalParams& p);
+int eval_threads_p(const dia_handle* h, const EvalParams& p);
 
 enum { PH_ADAM = 0, PH_LBFGS = 1, PH_DONE = 2 };
 
@@ -507,7 +508,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     cudaKernelNodeParams ke = {};
     const bool kc = eval_uses_const(h, p, false);
     ke.func = kc ? (void*)eval_kernel_ptr_kc(h) : (void*)eval_kernel_ptr_p(h, p);
-    ke.gridDim = dim3(grid); ke.blockDim = dim3(kThreads);
+    ke.gridDim = dim3(grid); ke.blockDim = dim3(eval_threads_p(h, p));
     ke.sharedMemBytes = (unsigned)eval_smem_bytes_p(h, p); ke.kernelParams = eval_args; ke.extra = nullptr;
     StepArgs sa;
     sa.b = w->b; sa.partials = p.partials; sa.n_blocks = part_cols; sa.np = w->np; sa.hist_cap = w->hist_cap;
