@@ -174,3 +174,18 @@ def test_small_kernel_one_reference_per_epoch_and_fit(dia):
         th1, r1 = h.fit(_dev(w.I[e:e + 1]), _dev(w.theta0[e:e + 1]), dia.FitOpts.default())
         assert r1[0].n_evals == rb[e].n_evals and torch.equal(th1[0], thb[e])
     h.close()
+
+
+@pytest.mark.parametrize("m", [1, 3])
+def test_small_kernel_full_size_c4(dia, m):
+    """The 4096^2 field of BASELINE config 4, two epochs, in the launch configuration bench.py's small-kernel leg and
+    sweep time (16 rows per thread, 444 or 296 CTAs, 128-bit loads): every output against the oracle over all pixels."""
+    w = make_workload(4, m=m, n_epochs=2)
+    cfg = oracle.RefConfig(w.n, w.n, m, sigma0=w.sigma0, gain=w.gain)
+    h = dia.Handle(_dev(w.R), m, max_epochs=16, sigma0=w.sigma0, gain=w.gain)     # a 16-epoch handle cuts 16-row strips
+    I = _dev(w.I)
+    for th, kind in ((w.theta0, "norm"), (w.theta_true.astype(np.float32), "S")):
+        Lo, go, So = oracle.eval_loss_grad(cfg, w.R, w.I, th, want_scale=True)
+        Lg, gg = h.eval_loss_grad(I, _dev(th))
+        _compare(Lg, gg, Lo, go, So, kind, f"small m={m} c4 full size")
+    h.close()
