@@ -166,3 +166,23 @@ def test_covariance_argument_errors(dia):
     with pytest.raises(dia.DiaError):
         dia.dia_covariance(h._h, H, None, None, info)
     h.close()
+
+
+def test_covariance_maximum_size_properties(dia):
+    """m = 47 (DIA_MAX_KERNEL_SIZE): np = 2210, beyond what the oracle's Jacobi diagonalisation finishes in seconds, so
+    the properties that define the result are checked instead: H Sigma = 1, exact symmetry, ln det H equal to the sum of
+    the planted log-eigenvalues, and sigma / sigma_P against LAPACK's inverse."""
+    m = 47
+    h = _handle(dia, m, n=64)
+    n = m * m + 1
+    H, ev = _spd(n, 12, 1e4)
+    cov, sig, info = (t.cpu().numpy() for t in h.covariance(_dev(H)))
+    assert info[0] == 1.0 and info[4] == -1.0
+    assert abs(info[1] - np.log(ev).sum()) <= 1e-10 * abs(np.log(ev).sum())
+    assert np.array_equal(cov, cov.T)
+    assert np.abs(H @ cov - np.eye(n)).max() <= 1e-8
+    ref = np.linalg.inv(H)
+    np.testing.assert_allclose(sig, np.sqrt(np.diag(ref)), rtol=1e-9)
+    u = np.zeros(n); u[:m * m] = 1.0
+    assert info[2] == pytest.approx(np.sqrt(u @ ref @ u), rel=1e-9)
+    h.close()
