@@ -118,10 +118,40 @@ def build_workload(first_epoch: int, n_epochs: int, n: int = N, m: int = M):
     R = make_reference(cfg, n)
     I = np.empty((n_epochs, n, n), np.float32)
     th0 = np.empty((n_epochs, m * m + 1), np.float32)
+    global TRUE_WIDTHS                      # sigma of each planted kernel (second moment), for the Gaussian-init series
+    TRUE_WIDTHS = []
+    h = (m - 1) // 2
+    r2 = (np.arange(m)[:, None] - h) ** 2 + (np.arange(m)[None, :] - h) ** 2
     for e in range(n_epochs):
-        I[e], _, _, _ = make_target(cfg, first_epoch + e, R, m)
+        I[e], th_true, _, _ = make_target(cfg, first_epoch + e, R, m)
         th0[e] = theta_init(R, I[e], m)
+        K = np.asarray(th_true[:m * m], np.float64).reshape(m, m)
+        TRUE_WIDTHS.append(float(np.sqrt((K * r2).sum() / (2.0 * K.sum()))))
     return cfg, R, I, th0
+
+
+TRUE_WIDTHS = []
+
+
+def oracle_fit_and_b08_times():
+    """the oracle's own fit (dia_ref_fit, paper settings) and the classical B08 normal-equation solve
+    (3 iterations) timed on the host cores, on the configs they finish in seconds (c0, c1)."""
+    import oracle
+    from workloads import make_workload
+    out = {}
+    for c in (0, 1):
+        w = make_workload(c)
+        rc = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+        t0 = time.perf_counter()
+        th_b = oracle.b08_solve(rc, w.R, w.I[0], n_iters=3)
+        t_b08 = time.perf_counter() - t0
+        entry = {"n": w.n, "m": w.m, "b08_solve_3_iterations_s": t_b08, "b08_photometric_scale": float(th_b[:-1].sum())}
+        if c == 0:
+            t0 = time.perf_counter()
+            _, res = oracle.fit(rc, w.R, w.I, w.theta0, oracle.RefFitOpts.default())
+            entry.update({"oracle_fit_s": time.perf_counter() - t0, "oracle_fit_evals": int(res[0].n_evals)})
+        out[f"c{c}"] = entry
+    return {"classical_and_fit": out}
 
 
 def oracle_eval_rate(cfg, R, I0, th0, crop: int, repeats: int = 1):
@@ -446,6 +476,18 @@ def run_gpu(args):
                             "n_adam": [r.n_adam for r in res_f], "n_lbfgs": [r.n_lbfgs for r in res_f],
                             "n_evals": [r.n_evals for r in res_f], "status": [r.status for r in res_f],
                             "photometric_scale": [round(r.photometric_scale, 5) for r in res_f]}
+        # second series (the paper's other panel): Gaussian initial kernel of the true width
+        from workloads import gaussian_kernel_init
+        thg = np.stack([gaussian_kernel_init(M, TRUE_WIDTHS[e], float(th0[e][-1])) for e in range(E)])
+        dthg = torch.from_numpy(thg).to(dev)
+        ms_fit_g, (_, res_g) = timed(lambda: h.fit(dI, dthg, fit_opts), 1)
+        if rank == 0:
+            line["fits"]["gaussian_init"] = {"value": E * world / (ms_fit_g * 1e-3), "unit": "fits/s", "ms_per_batch": ms_fit_g,
+                                             "init": "symmetric Gaussian of each epoch's planted width, sum 1; B0 as in the "
+                                                     "flat-kernel series",
+                                             "n_adam": [r.n_adam for r in res_g], "n_lbfgs": [r.n_lbfgs for r in res_g],
+                                             "n_evals": [r.n_evals for r in res_g], "status": [r.status for r in res_g],
+                                             "photometric_scale": [round(r.photometric_scale, 5) for r in res_g]}
         # Hessian at the fitted theta of epoch 0 (Eq. 15): np rows, max_epochs rows per launch
         h.hessian(dI[0], th_hat[0])
         ms_h, H_hat = timed(lambda: h.hessian(dI[0], th_hat[0]), 1)
@@ -500,6 +542,7 @@ def run_gpu(args):
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"FP64 oracle loss+gradient evaluation of epoch 0 at the full {crop}x{crop} size, "
                                           f"best of 3 calls ({sec:.2f} s per call, OpenMP over all host cores)"}
+        line["cpu_baseline"].update(oracle_fit_and_b08_times())
     h.close()
     if rank == 0:
         print(json.dumps(line), flush=True)
