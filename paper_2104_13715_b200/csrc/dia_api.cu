@@ -130,6 +130,14 @@ static const void* kernel_for(int m, bool aux, bool diff = false, bool kc = fals
   }
   return nullptr;
 }
+static const void* hess_kernel_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::eval_kernel_ptr_m##MM(4);
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return nullptr;
+}
 static const void* const_symbol_for(int m) {
   switch (m) {
 #define X(MM) case MM: return dia::const_symbol_m##MM();
@@ -483,7 +491,8 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
   const int np = h->np;
   dia::HessWorkspace& w = h->hess;
   if (!w.loss) {
-    cudaError_t ce = cudaMalloc(&w.loss, sizeof(double) * (size_t)np);
+    cudaError_t ce = cudaFuncSetAttribute(hess_kernel_for(h->cfg.m), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
+    if (ce == cudaSuccess) ce = cudaMalloc(&w.loss, sizeof(double) * (size_t)np);
     if (ce == cudaSuccess && h->cfg.lambda_reg > 0.f) {
       ce = cudaMalloc(&w.ident, sizeof(float) * (size_t)np * np);
       if (ce == cudaSuccess) dia::hess_identity_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(w.ident, np);
@@ -494,12 +503,31 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
       return DIA_ERR_ALLOC;
     }
   }
-  // rows q0 .. q0 + n - 1 of H per launch: the fused kernel with the weight h X_q in place of w (D3)
-  for (int q0 = 0; q0 < np; q0 += h->cfg.max_epochs) {
+  // Kernel-pixel rows (q < m^2), max_epochs rows per launch: hess_block_kernel computes h once per tile and then one
+  // gradient pass per row; it delivers the kernel-kernel block, the remaining entries of these rows
+  // come from the background rows below by symmetry.
+  const int nk = h->cfg.m * h->cfg.m;
+  const void* kblock = hess_kernel_for(h->cfg.m);
+  const int bgrid = h->grid < h->tiles ? h->grid : h->tiles;
+  for (int q0 = 0; q0 < nk; q0 += h->cfg.max_epochs) {
+    const int n = nk - q0 < h->cfg.max_epochs ? nk - q0 : h->cfg.max_epochs;
+    dia::EvalParams p;
+    dia::TensorMaps tm;
+    fill_params(h, n, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, q0);
+    void* args[] = {(void*)&p};
+    cudaError_t ce = cudaLaunchKernel(kblock, dim3(bgrid), dim3(dia::kThreads), args, h->smem, h->stream);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "hessian block launch");
+    const int np1 = np + 1, warps = 8;
+    dia::reduce_partials_kernel<<<dim3((np1 + warps - 1) / warps, n), warps * 32, 0, h->stream>>>(
+        h->d_partials, bgrid, np1, nullptr, w.loss + q0, d_H + (size_t)q0 * np);
+  }
+  // Background rows (B0 and the polynomial terms): the fused kernel with the weight h X_q in place of w (D3)
+  for (int q0 = nk; q0 < np; q0 += h->cfg.max_epochs) {
     const int n = np - q0 < h->cfg.max_epochs ? np - q0 : h->cfg.max_epochs;
     rc = eval_into(h, n, d_I, d_mask, d_var, d_theta, w.loss + q0, d_H + (size_t)q0 * np, q0);
     if (rc != DIA_OK) return rc;
   }
+  dia::hess_fill_columns_kernel<<<(nk * (np - nk) + 255) / 256, 256, 0, h->stream>>>(d_H, np, nk);
   // Eq. 20: the penalty lambda N |L theta|^2 adds 2 lambda N L'L; its gradient is linear in theta, so the
   // gradient at the unit vector e_q is row q
   if (h->cfg.lambda_reg > 0.f)

@@ -792,6 +792,131 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) eval_kernel(const Eval
   if (cur_j >= 0) finish_epoch();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Hessian block kernel (dia_hessian): rows hess_q0 .. hess_q0 + n_epochs - 1 (all of them
+// kernel-pixel rows, q < M*M) of the kernel-kernel block of H for one target, H[q][o] = sum_V h X_q X_o.
+// Per tile the model and h = d^2 l / dM^2 are computed ONCE (forward stencil + epilogue, as in eval_kernel's
+// Hessian mode with X_q = 1); then for every row q the weight tile h X_q -- X_q is the reference pixel shifted by
+// row q's kernel position, read from the staged R tile -- is correlated against the R tile exactly as in the gradient
+// phase of eval_kernel, and the FP32 strips are folded into this CTA's FP64 partial column of row q.  A launch of 16
+// rows therefore costs 1 forward + 16 gradient passes per tile instead of 16 + 16.  Tiles are staged by cp.async
+// (single buffer: staging is < 1 % of 17 passes).  Columns M*M.. of the partials (background terms, loss) are written
+// as zeros; the host fills those entries of H from the background rows by symmetry.
+// ------------------------------------------------------------------------------------------------
+template <int M>
+__global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) hess_block_kernel(const EvalParams p) {
+  using G = Geo<M>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  unsigned char* sm = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  float* const Rs = reinterpret_cast<float*>(sm + G::OFF_R);
+  float* const Is = reinterpret_cast<float*>(sm + G::OFF_I);      // I tile during the forward phase, then h X_q
+  float* const Hs = reinterpret_cast<float*>(sm + G::OFF_W);      // h tile
+  float* const accS = reinterpret_cast<float*>(sm + G::OFF_ACC);
+  float* const Ks = reinterpret_cast<float*>(sm + G::OFF_K);
+  float* const Bs = reinterpret_cast<float*>(sm + G::OFF_BG);
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n_tiles = p.tiles_x * p.tiles_y;
+  const int vr = p.n_rows - M + 1, vc = p.n_cols - M + 1;
+  const size_t npix = (size_t)p.n_rows * p.n_cols;
+  const int f_col = (warp & 1) * 32 + (lane & 1) * kP;
+  const int f_row = (warp >> 1) * 16 + (lane >> 1);
+  const int g_a = tid % M, g_s = tid / M;
+  const bool g_active = g_s < G::S;
+  float4* const myacc = reinterpret_cast<float4*>(accS + tid * G::KP);
+  const int grid = (int)gridDim.x, ncols = grid;      // the host launches min(resident CTAs, tiles) CTAs
+
+  for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
+    const int a = idx / G::KP, b = idx - a * G::KP;
+    Ks[idx] = (b < M) ? p.theta[a * M + b] : 0.f;
+  }
+  const float B0 = p.theta[M * M];
+  if (tid < kMaxBg) Bs[tid] = (tid < p.np - M * M) ? p.theta[M * M + tid] : 0.f;
+  __syncthreads();
+
+  bool first = true;
+  for (int t = (int)blockIdx.x; t < n_tiles; t += grid) {
+    const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
+    stage_tile_cp_async<G::RH, G::RPITCH>(p.R, p.n_rows, p.n_cols, p.cp8, tile_y * kTH, tile_x * kTW, smem_u32(Rs));
+    stage_tile_cp_async<kTH, kIPitch>(p.I, p.n_rows, p.n_cols, p.cp8, tile_y * kTH + G::H, tile_x * kTW + G::H - G::IOFF,
+                                      smem_u32(Is));
+    asm volatile("cp.async.wait_all;\n" ::: "memory");
+    __syncthreads();
+    {                                        // forward: h tile
+      float tot[kP];
+      forward_strip<M, false>(Ks, 0, Rs + f_row * G::RPITCH + f_col, B0, tot);
+      const int iy = tile_y * kTH + f_row, ix0 = tile_x * kTW + f_col;
+      const float* irow = Is + f_row * kIPitch + f_col;
+      float* hrow = Hs + f_row * kIPitch + f_col;
+      float lsum, wsum, Sp[4];
+      const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
+      if (edge) strip_epilogue<M, true, true>(p, 0, npix, iy, ix0, vr, vc, tot, irow, hrow, Bs, lsum, wsum, Sp, nullptr, 0, 0);
+      else strip_epilogue<M, true, false>(p, 0, npix, iy, ix0, vr, vc, tot, irow, hrow, Bs, lsum, wsum, Sp, nullptr, 0, 0);
+    }
+    __syncthreads();                         // h tile complete, I tile consumed
+    const int rows_here = min(kTH, vr - tile_y * kTH);
+    const int n_items = rows_here * (kTW / kP);
+#pragma unroll 1
+    for (int jq = 0; jq < p.n_epochs; ++jq) {
+      const int q = p.hess_q0 + jq;
+      const int aq = q / M, bq = q - aq * M;
+      {                                      // weight tile of row q: h X_q, this thread's forward strip
+        const float* xr = Rs + (f_row + aq) * G::RPITCH + f_col + bq;
+        const float4* h4 = reinterpret_cast<const float4*>(Hs + f_row * kIPitch + f_col);
+        float4* w4 = reinterpret_cast<float4*>(Is + f_row * kIPitch + f_col);
+#pragma unroll
+        for (int c = 0; c < kP / 4; ++c) {
+          float4 v = h4[c];
+          v.x *= xr[4 * c]; v.y *= xr[4 * c + 1]; v.z *= xr[4 * c + 2]; v.w *= xr[4 * c + 3];
+          w4[c] = v;
+        }
+      }
+      __syncthreads();
+      if (g_active) {                        // the gradient phase of eval_kernel on this weight tile
+        float acc[G::KP];
+#pragma unroll
+        for (int c = 0; c < G::KP; ++c) acc[c] = 0.f;
+#pragma unroll 1
+        for (int item = g_s; item < n_items; item += G::S) {
+          const int i = item / (kTW / kP), c = item - i * (kTW / kP);
+          float w[kP], r[G::RSEG];
+          const float4* w4 = reinterpret_cast<const float4*>(Is + i * kIPitch + c * kP);
+#pragma unroll
+          for (int k = 0; k < kP / 4; ++k) {
+            const float4 v = w4[k];
+            w[4 * k] = v.x; w[4 * k + 1] = v.y; w[4 * k + 2] = v.z; w[4 * k + 3] = v.w;
+          }
+          const float4* r4 = reinterpret_cast<const float4*>(Rs + (i + g_a) * G::RPITCH + c * kP);
+#pragma unroll
+          for (int k = 0; k < G::RSEG / 4; ++k) {
+            const float4 v = r4[k];
+            r[4 * k] = v.x; r[4 * k + 1] = v.y; r[4 * k + 2] = v.z; r[4 * k + 3] = v.w;
+          }
+#pragma unroll
+          for (int k = 0; k < kP; ++k)
+#pragma unroll
+            for (int b = 0; b < M; ++b) acc[b] = fmaf(w[k], r[k + b], acc[b]);
+        }
+#pragma unroll
+        for (int k = 0; k < G::KP / 4; ++k)
+          myacc[k] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
+      }
+      __syncthreads();
+      double* outp = p.partials + ((size_t)jq * p.part_rows) * ncols + blockIdx.x;
+      for (int o = tid; o < M * M; o += kThreads) {
+        const int a = o / M, b = o - a * M;
+        double sacc = 0.0;
+#pragma unroll 1
+        for (int ss = 0; ss < G::S; ++ss) sacc += (double)accS[(ss * M + a) * G::KP + b];
+        outp[(size_t)o * ncols] = first ? sacc : outp[(size_t)o * ncols] + sacc;
+      }
+      if (first && tid < p.part_rows - M * M) outp[(size_t)(M * M + tid) * ncols] = 0.0;
+      __syncthreads();                       // strips and weight tile free for the next row
+    }
+    first = false;
+  }
+}
+
 #ifndef DIA_INST_M      // the small stand-alone kernels belong to the API translation unit only
 // Fixed-order sum of one row of block partials by one warp: lane l adds columns l, l+32, ... in order,
 // then the 32 lane sums are combined by a fixed butterfly -- deterministic for a given n_blocks.

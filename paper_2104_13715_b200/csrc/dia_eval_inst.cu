@@ -14,13 +14,14 @@
 namespace dia {
 
 // variant: 0 = plain objective, 1 = generic (mask / flat / variance map), 2 = difference image,
-//          3 = plain objective with the kernel pixels in the constant bank
+//          3 = plain objective with the kernel pixels in the constant bank, 4 = kernel-kernel block of the Hessian
 const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
   switch (variant) {
     case 0: return (const void*)eval_kernel<DIA_INST_M, false, false, false>;
     case 1: return (const void*)eval_kernel<DIA_INST_M, true, false, false>;
     case 2: return (const void*)eval_kernel<DIA_INST_M, true, true, false>;
     case 3: return (const void*)eval_kernel<DIA_INST_M, false, false, true>;
+    case 4: return (const void*)hess_block_kernel<DIA_INST_M>;
   }
   return nullptr;
 }

@@ -22,6 +22,16 @@ __global__ void hess_identity_kernel(float* __restrict__ A, int np) {
     A[idx] = (idx / np == idx % np) ? 1.f : 0.f;
 }
 
+// Entries H[q][nk + t] of the kernel-pixel rows q < nk, which hess_block_kernel leaves at zero: by symmetry the
+// entries H[nk + t][q] of the background rows.
+__global__ void hess_fill_columns_kernel(double* __restrict__ H, int np, int nk) {
+  const int nb = np - nk, total = nk * nb;
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+    const int q = idx / nb, t = idx - q * nb;
+    H[(size_t)q * np + nk + t] = H[(size_t)(nk + t) * np + q];
+  }
+}
+
 // H <- (H + H') / 2: rows p and q were accumulated in different FP32 orders
 __global__ void hess_symmetrise_kernel(double* __restrict__ H, int np) {
   const int total = np * np;
