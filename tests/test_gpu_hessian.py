@@ -121,3 +121,23 @@ def test_hessian_argument_errors(dia):
     with pytest.raises(dia.DiaError):
         h.hessian(_dev(w.I[0]), _dev(w.theta_true[0].astype(np.float32)))
     h.close()
+
+
+@pytest.mark.parametrize("grid_limit", [1, 5])
+def test_hessian_many_tiles_per_cta(dia, monkeypatch, grid_limit):
+    """Test hook DIA_GRID_LIMIT: one or five CTAs walk through all 36 tiles of a 400^2 image, so every CTA of
+    hess_block_kernel accumulates its FP64 partial column over many tiles (the launch shape of a 4096^2 image: 4096
+    tiles on 296 CTAs) and restages its single R / I buffer between them; 23 rows per launch leave a ragged last one."""
+    monkeypatch.setenv("DIA_GRID_LIMIT", str(grid_limit))
+    w = make_workload(4, n=400, m=9, n_epochs=1)
+    cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+    h = dia.Handle(_dev(w.R), w.m, max_epochs=23, sigma0=w.sigma0, gain=w.gain)
+    assert h.info()["grid_blocks"] == grid_limit
+    th = w.theta_true[0].astype(np.float32)
+    Ho = oracle.hessian(cfg, w.R, w.I[0], th)
+    Hg = h.hessian(_dev(w.I[0]), _dev(th)).cpu().numpy()
+    e = _e_H(Hg, Ho)
+    print(f"hessian grid={grid_limit}: e_H={e:.2e}")
+    assert e <= TOL_H
+    assert np.array_equal(Hg, h.hessian(_dev(w.I[0]), _dev(th)).cpu().numpy())
+    h.close()
