@@ -41,3 +41,31 @@ def max_over_ranks(value: float, device=None, group=None) -> float:
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+# ---- row bands of ONE image pair ------------------------------------------------------------
+# The objective is a sum over valid pixels, so the valid rows split into bands: rank g evaluates the sub-image
+# rows [r0, r1 + m - 1) of R and I -- whose own valid region is exactly the band -- with an ordinary handle, and the
+# full loss and gradient are the sums of the per-rank results.  R is constant, so there is no halo exchange per
+# evaluation; the only collective is one (m^2 + 2)-double all-gather, summed in rank order on every rank (deterministic,
+# identical on all ranks).  Evaluation only: dia_fit's on-device loop has no place for a collective.
+def row_band(n_rows: int, m: int, world_size: int, rank: int) -> Tuple[int, int, int, int]:
+    """-> (v0, v1, i0, i1): valid rows [v0, v1) owned by `rank` (indices into the valid region, n_rows - m + 1 rows in
+    all, split like epoch_shard) and the image rows [i0, i1) = [v0, v1 + m - 1) to hand to dia_create / the targets."""
+    n_valid = n_rows - m + 1
+    if m < 1 or m % 2 == 0 or n_valid < 1:
+        raise ValueError("bad image or kernel size")
+    v0, v1 = epoch_shard(n_valid, world_size, rank)
+    return v0, v1, v0, (v1 + m - 1 if v1 > v0 else v0)
+
+
+def sum_over_ranks_in_order(local: torch.Tensor, group=None) -> torch.Tensor:
+    """All-gathers a small per-rank tensor (loss and gradient of a band, float64) and adds the parts in rank order on
+    every rank: the same bits everywhere, whatever order the collective completes in."""
+    world = dist.get_world_size(group)
+    parts: List[torch.Tensor] = [torch.empty_like(local) for _ in range(world)]
+    dist.all_gather(parts, local.contiguous(), group=group)
+    total = torch.zeros_like(local)
+    for r in range(world):
+        total += parts[r]
+    return total

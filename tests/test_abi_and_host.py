@@ -157,6 +157,51 @@ def test_epoch_sharding_two_ranks_gloo(tmp_path):
     assert "rank0-ok" in out.stdout and "rank1-ok" in out.stdout, out.stdout
 
 
+_BAND_WORKER = textwrap.dedent("""
+    import os, sys
+    sys.path.insert(0, {root!r})
+    import numpy as np, torch, torch.distributed as dist
+    import oracle
+    from workloads import make_workload
+    from paper_2104_13715_b200.sharding import row_band, sum_over_ranks_in_order
+    dist.init_process_group("gloo")
+    rank, world = dist.get_rank(), dist.get_world_size()
+    w = make_workload(0, n=61, m=5)                      # 57 valid rows: bands of 29 and 28
+    th = w.theta_true[0].astype(np.float32)
+    v0, v1, i0, i1 = row_band(w.n, w.m, world, rank)
+    assert i1 - i0 == (v1 - v0) + w.m - 1
+    cfg = oracle.RefConfig(i1 - i0, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+    L, g = oracle.eval_loss_grad(cfg, w.R[i0:i1], w.I[:, i0:i1], th)        # the band as an ordinary sub-image
+    local = torch.from_numpy(np.concatenate([L, g[0]]))
+    total = sum_over_ranks_in_order(local).numpy()
+    full = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+    Lf, gf = oracle.eval_loss_grad(full, w.R, w.I, th)
+    assert abs(total[0] - Lf[0]) <= 1e-12 * abs(Lf[0]), (total[0], Lf[0])
+    assert np.abs(total[1:] - gf[0]).max() <= 1e-10 * np.abs(gf[0]).max()
+    dist.destroy_process_group()
+    print("band%d-ok" % rank, flush=True)
+""")
+
+
+def test_row_band_sharding_two_ranks_gloo(tmp_path):
+    """SURVEY.md 8(e)(2) on CPU: two ranks evaluate row bands of one image pair as ordinary sub-images (the oracle
+    stands in for the device call), one small all-gather summed in rank order gives the full loss and gradient."""
+    from paper_2104_13715_b200.sharding import row_band
+    assert row_band(100, 7, 3, 0) == (0, 32, 0, 38) and row_band(100, 7, 3, 2) == (63, 94, 63, 100)
+    with pytest.raises(ValueError):
+        row_band(5, 7, 1, 0)
+    script = tmp_path / "band_worker.py"
+    script.write_text(_BAND_WORKER.format(root=ROOT))
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=240)
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert "band0-ok" in out.stdout and "band1-ok" in out.stdout, out.stdout
+
+
 def test_bench_accounting():
     sys.path.insert(0, ROOT)
     import bench

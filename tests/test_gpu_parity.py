@@ -518,3 +518,23 @@ def test_full_size_direct(dia, c, E):
         Lg, gg = h.eval_loss_grad(I, _dev(th), mask=mask)
         _compare(Lg, gg, Lo, go, So, kind, f"c{c} full size {name}")
     h.close()
+
+
+def test_row_bands_sum_to_the_full_image(dia):
+    """the valid rows split into bands, each evaluated as an ordinary sub-image (its own handle, as a
+    rank would); the band results add up to the full-image loss and gradient, and to the oracle's."""
+    from paper_2104_13715_b200.sharding import row_band
+    w = make_workload(4, n=300, n_epochs=1, m=19)
+    th = w.theta_true.astype(np.float32)
+    Lo, go, So = oracle.eval_loss_grad(_ref_cfg(w), w.R, w.I, th, want_scale=True)
+    world = 3
+    L = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g = torch.zeros((1, w.m * w.m + 1), dtype=torch.float64, device="cuda")
+    for rank in range(world):
+        v0, v1, i0, i1 = row_band(w.n, w.m, world, rank)
+        h = dia.Handle(_dev(w.R[i0:i1]), w.m, sigma0=w.sigma0, gain=w.gain)
+        Lb, gb = h.eval_loss_grad(_dev(w.I[:, i0:i1]), _dev(th))
+        L += Lb
+        g += gb
+        h.close()
+    _compare(L, g, Lo, go, So, "S", "row bands")
