@@ -497,13 +497,13 @@ def run_gpu(args):
         if rank == 0:
             rows = M * M + 1
             ci = cov_info.cpu().tolist()
-            # work model of dia_hessian: per launch of E kernel-pixel rows one forward pass and E gradient passes
-            # (m^2 FMA per valid pixel each); the B0 row is one ordinary evaluation (2 m^2)
-            n_launch = -(-(M * M) // E)
+            # work model of dia_hessian: per launch of 32 kernel-pixel rows (kHessRows) one forward pass and 32 gradient
+            # passes (m^2 FMA per valid pixel each); the B0 row is one ordinary evaluation (2 m^2)
+            n_launch = -(-(M * M) // 32)
             fma_h = (n_launch + M * M + 2 * (rows - M * M)) * 0.5 * useful_fma()
             line["fits"]["hessian"] = {"ms": ms_h, "rows": rows, "launches": n_launch + 1,
                                        "tflops": 2.0 * fma_h / (ms_h * 1e-3) / 1e12,
-                                       "work_model": "1 forward + 16 gradient passes per 16-row launch"}
+                                       "work_model": "1 forward + 32 gradient passes per 32-row launch"}
             line["fits"]["covariance"] = {"ms": ms_c, "np": rows, "launches": rows + 3, "valid": ci[0],
                                           "sigma_P": ci[2], "sigma_B0": float(sig_hat[M * M])}
 

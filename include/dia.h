@@ -129,8 +129,8 @@ int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs,
  * with X the design vector of a pixel (the m*m shifted reference pixels, then the background basis) and
  * h_ij = d^2 l_ij / dM^2 (D3), row q of H is sum_V (h_ij X_q) X -- the gradient sum of
  * dia_eval_loss_grad with the per-pixel weight h_ij X_q in place of w_ij -- so the stencil code of the fused kernel
- * computes the rows, max_epochs rows per launch with h_ij evaluated once per launch (create the handle with
- * max_epochs >= 16 to batch them); the penalty of Eq. 20 adds 2 lambda N L'L, and H is symmetrised.
+ * computes the rows, 32 kernel-pixel rows per launch with h_ij evaluated once per launch (whatever the handle's
+ * max_epochs); the penalty of Eq. 20 adds 2 lambda N L'L, and H is symmetrised.
  *   d_I [n_rows][n_cols], d_mask / d_var as in dia_eval_loss_grad for one epoch; d_theta [np] float32;
  *   d_H [np][np] float64 DEVICE, row-major, out.
  * The first call allocates a small workspace (synchronises once); later calls are asynchronous.  Handles created

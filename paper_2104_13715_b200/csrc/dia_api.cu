@@ -493,6 +493,8 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
   if (!w.loss) {
     cudaError_t ce = cudaFuncSetAttribute(hess_kernel_for(h->cfg.m), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
     if (ce == cudaSuccess) ce = cudaMalloc(&w.loss, sizeof(double) * (size_t)np);
+    if (ce == cudaSuccess)
+      ce = cudaMalloc(&w.partials, sizeof(double) * (size_t)dia::kHessRows * (np + 1) * (h->grid < h->tiles ? h->grid : h->tiles));
     if (ce == cudaSuccess && h->cfg.lambda_reg > 0.f) {
       ce = cudaMalloc(&w.ident, sizeof(float) * (size_t)np * np);
       if (ce == cudaSuccess) dia::hess_identity_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(w.ident, np);
@@ -503,23 +505,24 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
       return DIA_ERR_ALLOC;
     }
   }
-  // Kernel-pixel rows (q < m^2), max_epochs rows per launch: hess_block_kernel computes h once per tile and then one
+  // Kernel-pixel rows (q < m^2), kHessRows rows per launch: hess_block_kernel computes h once per tile and then one
   // gradient pass per row; it delivers the kernel-kernel block, the remaining entries of these rows
   // come from the background rows below by symmetry.
   const int nk = h->cfg.m * h->cfg.m;
   const void* kblock = hess_kernel_for(h->cfg.m);
   const int bgrid = h->grid < h->tiles ? h->grid : h->tiles;
-  for (int q0 = 0; q0 < nk; q0 += h->cfg.max_epochs) {
-    const int n = nk - q0 < h->cfg.max_epochs ? nk - q0 : h->cfg.max_epochs;
+  for (int q0 = 0; q0 < nk; q0 += dia::kHessRows) {
+    const int n = nk - q0 < dia::kHessRows ? nk - q0 : dia::kHessRows;
     dia::EvalParams p;
     dia::TensorMaps tm;
-    fill_params(h, n, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, q0);
+    fill_params(h, 1, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, q0);
+    p.n_epochs = n;  p.partials = w.partials;      // rows of this launch, the Hessian's own partial columns
     void* args[] = {(void*)&p};
     cudaError_t ce = cudaLaunchKernel(kblock, dim3(bgrid), dim3(dia::kThreads), args, h->smem, h->stream);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "hessian block launch");
     const int np1 = np + 1, warps = 8;
     dia::reduce_partials_kernel<<<dim3((np1 + warps - 1) / warps, n), warps * 32, 0, h->stream>>>(
-        h->d_partials, bgrid, np1, nullptr, w.loss + q0, d_H + (size_t)q0 * np);
+        w.partials, bgrid, np1, nullptr, w.loss + q0, d_H + (size_t)q0 * np);
   }
   // Background rows (B0 and the polynomial terms): the fused kernel with the weight h X_q in place of w (D3)
   for (int q0 = nk; q0 < np; q0 += h->cfg.max_epochs) {

@@ -798,9 +798,9 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) eval_kernel(const Eval
 // Per tile the model and h = d^2 l / dM^2 are computed ONCE (forward stencil + epilogue, as in eval_kernel's
 // Hessian mode with X_q = 1); then for every row q the weight tile h X_q -- X_q is the reference pixel shifted by
 // row q's kernel position, read from the staged R tile -- is correlated against the R tile exactly as in the gradient
-// phase of eval_kernel, and the FP32 strips are folded into this CTA's FP64 partial column of row q.  A launch of 16
-// rows therefore costs 1 forward + 16 gradient passes per tile instead of 16 + 16.  Tiles are staged by cp.async
-// (single buffer: staging is < 1 % of 17 passes).  Columns M*M.. of the partials (background terms, loss) are written
+// phase of eval_kernel, and the FP32 strips are folded into this CTA's FP64 partial column of row q.  A launch of 32
+// rows therefore costs 1 forward + 32 gradient passes per tile instead of 32 + 32.  Tiles are staged by cp.async
+// (single buffer: staging is < 1 % of 33 passes).  Columns M*M.. of the partials (background terms, loss) are written
 // as zeros; the host fills those entries of H from the background rows by symmetry.
 // ------------------------------------------------------------------------------------------------
 template <int M>

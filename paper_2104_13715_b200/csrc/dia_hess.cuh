@@ -5,14 +5,18 @@
 
 namespace dia {
 
+constexpr int kHessRows = 32;   // kernel-pixel rows of H per hess_block_kernel launch: 1 forward + 32 gradient passes
+
 struct HessWorkspace {
   double* loss = nullptr;      // [np] scratch for the loss row of the partials (unused in Hessian mode)
   float* ident = nullptr;      // [np][np] identity: unit parameter vectors for the penalty's second derivative
+  double* partials = nullptr;  // [kHessRows][np+1][CTAs] block partials of hess_block_kernel (its own: the row count
+                               // per launch does not depend on the handle's max_epochs)
   double* chol = nullptr;      // [np][np] Cholesky factor of dia_covariance (L below, L' above the diagonal)
 };
 
 inline void hess_workspace_destroy(HessWorkspace* w) {
-  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->chol);
+  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->partials); cudaFree(w->chol);
   *w = HessWorkspace();
 }
 

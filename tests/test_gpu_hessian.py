@@ -127,7 +127,8 @@ def test_hessian_argument_errors(dia):
 def test_hessian_many_tiles_per_cta(dia, monkeypatch, grid_limit):
     """Test hook DIA_GRID_LIMIT: one or five CTAs walk through all 36 tiles of a 400^2 image, so every CTA of
     hess_block_kernel accumulates its FP64 partial column over many tiles (the launch shape of a 4096^2 image: 4096
-    tiles on 296 CTAs) and restages its single R / I buffer between them; 23 rows per launch leave a ragged last one."""
+    tiles on 296 CTAs) and restages its single R / I buffer between them; 81 kernel-pixel rows in launches of 32 leave a
+    ragged last one."""
     monkeypatch.setenv("DIA_GRID_LIMIT", str(grid_limit))
     w = make_workload(4, n=400, m=9, n_epochs=1)
     cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
