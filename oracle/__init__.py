@@ -9,6 +9,7 @@ from .dia_ref import (  # noqa: F401
     RefFitResult,
     eval_loss_grad,
     fit,
+    fit_trace,
     b08_solve,
     difference_image,
     hessian,

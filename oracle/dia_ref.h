@@ -12,10 +12,12 @@
  *   (PAPER.md:60); theta = [K (m*m values), B0]; the valid set is
  *   h <= i < n_rows-h, h <= j < n_cols-h intersected with mask != 0.
  *
- * Pin status (tests/test_oracle_*.py): model, noise, both losses, gradient, B08 solve,
- * fixed-weight fit and planted recovery are pinned.  The free-running Adam->L-BFGS fit on
- * NOISY data is "parity unpinned" beyond its fixed-weight / planted special cases
- * (no external value exists).
+ * Pin status (tests/test_oracle_*.py): model, noise, both losses, gradient, Hessian, covariance, B08 solve,
+ * fixed-weight fit and planted recovery are pinned; the optimiser's arithmetic is pinned step by step
+ * (tests/test_oracle_optimiser_pins.py: the Adam trajectory against torch.optim.Adam in float64, every L-BFGS
+ * direction against the dense BFGS recursion with and without eviction, the switch rule on crafted tolerances).
+ * What stays "parity unpinned" is the ITERATE AT WHICH a free-running fit on noisy data stops under the paper's
+ * loss-change rule: no external value exists for it.
  */
 #ifndef DIA_REF_H
 #define DIA_REF_H
@@ -97,6 +99,14 @@ int dia_ref_covariance(int n, int n_kernel, const double* H, double* cov, double
 int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
                 int n_epochs, const float* I, const unsigned char* mask, const float* var,
                 float* theta, dia_ref_fit_result* result);
+
+/* dia_ref_fit for ONE epoch, recording the FP64 iterates: trace_theta [trace_cap][np] = theta after every Adam /
+ * L-BFGS update in order, trace_loss [trace_cap] (nullable) = the loss the Adam update was computed from / the
+ * L-BFGS update reached, *trace_n = rows written.  Same arithmetic (same routine) as dia_ref_fit. */
+int dia_ref_fit_trace(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
+                      const float* I, const unsigned char* mask, const float* var,
+                      float* theta, dia_ref_fit_result* result,
+                      double* trace_theta, double* trace_loss, int trace_cap, int* trace_n);
 
 /* B08 iterated normal-equation solve (DESIGN c.3).  One epoch.
  * var_fixed (nullable): if given, every iteration uses this variance map instead of Eq. 6.

@@ -152,6 +152,25 @@ def fit(cfg: RefConfig, R, I, theta0, opts: Optional[RefFitOpts] = None, mask=No
     return theta, list(res)
 
 
+def fit_trace(cfg: RefConfig, R, I, theta0, opts: Optional[RefFitOpts] = None, mask=None, var=None, cap=4096):
+    """One epoch.  -> (theta_hat float32 [np], RefFitResult, trace_theta float64 [n_updates][np], trace_loss [n_updates]):
+    the FP64 iterate after every Adam / L-BFGS update, in order."""
+    c, keep = cfg._c()
+    R = _f32(R)
+    E, I, mask, var, theta = _epochs(cfg, I, mask, var, theta0)
+    assert E == 1
+    theta = theta.copy()
+    opts = opts or RefFitOpts.default()
+    res = RefFitResult()
+    tr = np.zeros((cap, cfg.n_params), dtype=np.float64)
+    trL = np.zeros(cap, dtype=np.float64)
+    n = C.c_int(0)
+    _check(_lib().dia_ref_fit_trace(C.byref(c), _ptr(R), C.byref(opts), _ptr(I), _ptr(mask), _ptr(var),
+                                    _ptr(theta), C.byref(res), _ptr(tr), _ptr(trL), int(cap), C.byref(n)),
+           "dia_ref_fit_trace")
+    return theta[0], res, tr[:n.value].copy(), trL[:n.value].copy()
+
+
 def b08_solve(cfg: RefConfig, R, I, mask=None, var_fixed=None, n_iters=3, clip_last=False,
               want_H=False):
     c, keep = cfg._c()

@@ -28,7 +28,17 @@ typedef struct {
   int np;
   float* th32;
   int n_evals;
+  /* optional FP64 record of the iterates (dia_ref_fit_trace): row r = theta after update r, its loss column the
+     loss that update was computed from (Adam: at the pre-update iterate) or reached (L-BFGS: at the new iterate) */
+  double* tr_theta; double* tr_loss; int tr_cap, tr_n;
 } objective;
+
+static void record(objective* ob, const double* th, double L) {
+  if (!ob->tr_theta || ob->tr_n >= ob->tr_cap) return;
+  memcpy(ob->tr_theta + (size_t)ob->tr_n * ob->np, th, sizeof(double) * ob->np);
+  if (ob->tr_loss) ob->tr_loss[ob->tr_n] = L;
+  ob->tr_n++;
+}
 
 /* Evaluate the objective at the float32 rounding of theta (R9). */
 static void eval_at(objective* ob, const double* theta, double* L, double* g) {
@@ -90,6 +100,7 @@ static int fit_one(objective* ob, const dia_ref_fit_opts* o, float* theta_io, di
     }
     n_adam++;
     Lprev = L;
+    record(ob, th, L);
   }
 
   /* ---------------- L-BFGS PHASE ---------------- */
@@ -162,6 +173,7 @@ static int fit_one(objective* ob, const dia_ref_fit_opts* o, float* theta_io, di
       for (int q = 0; q < np; ++q) { th[q] = thn[q]; g[q] = gn[q]; }
       L = Ln;
       n_lbfgs++;
+      record(ob, th, L);
       if (o->force_lbfgs_iters < 0) {
         if (dL <= o->tol_change_rel * fabs(L)) { status = DIA_REF_FIT_CONVERGED_CHANGE; break; }   /* R8 */
         if (k >= o->max_lbfgs_iters) { status = DIA_REF_FIT_MAX_ITERS; break; }
@@ -192,9 +204,34 @@ int dia_ref_fit(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opt
   if (!th32) return DIA_REF_ERR_ALLOC;
   int rc = DIA_REF_OK;
   for (int e = 0; e < n_epochs && rc == DIA_REF_OK; ++e) {
-    objective ob = { cfg, R, I + e * npix, mask ? mask + e * npix : NULL, var ? var + e * npix : NULL, np, th32, 0 };
+    objective ob = { cfg, R, I + e * npix, mask ? mask + e * npix : NULL, var ? var + e * npix : NULL, np, th32, 0,
+                     NULL, NULL, 0, 0 };
     rc = fit_one(&ob, opts, theta + (size_t)e * np, result + e);
   }
+  free(th32);
+  return rc;
+}
+
+
+/* dia_ref_fit for one epoch that also records the FP64 iterates (the float32 theta of dia_ref_fit hides 1e-8 of
+ * them): trace_theta [trace_cap][np] receives theta after every Adam / L-BFGS update in order, trace_loss
+ * [trace_cap] the loss belonging to it, *trace_n the number of rows written.  Same arithmetic as dia_ref_fit --
+ * it is the same fit_one -- so that the optimiser can be pinned against library / textbook recursions
+ * (tests/test_oracle_optimiser_pins.py). */
+int dia_ref_fit_trace(const dia_ref_config* cfg, const float* R, const dia_ref_fit_opts* opts,
+                      const float* I, const unsigned char* mask, const float* var,
+                      float* theta, dia_ref_fit_result* result,
+                      double* trace_theta, double* trace_loss, int trace_cap, int* trace_n) {
+  if (!cfg || !R || !opts || !I || !theta || !result || !trace_theta || !trace_n || trace_cap < 0)
+    return DIA_REF_ERR_INVALID_ARG;
+  if (cfg->m < 1 || cfg->m % 2 == 0) return DIA_REF_ERR_INVALID_ARG;
+  if (cfg->noise == DIA_REF_NOISE_FIXED && !var) return DIA_REF_ERR_INVALID_ARG;
+  const int np = dia_ref_num_params(cfg);
+  float* th32 = (float*)malloc(sizeof(float) * np);
+  if (!th32) return DIA_REF_ERR_ALLOC;
+  objective ob = { cfg, R, I, mask, var, np, th32, 0, trace_theta, trace_loss, trace_cap, 0 };
+  const int rc = fit_one(&ob, opts, theta, result);
+  *trace_n = ob.tr_n;
   free(th32);
   return rc;
 }
