@@ -24,6 +24,10 @@
  *    reported per epoch in dia_fit_result.status, not by return code.
  *  - Same inputs => bit-identical outputs on repeated calls (fixed tile->block map, fixed-order
  *    FP64 reductions, no floating-point atomics).
+ *  - Threads: different handles may be driven from different host threads at the same time, on the same or on
+ *    different streams (handles of one kernel size that share a stream also share a constant-memory block; the
+ *    library serialises the enqueues that refresh and use it).  ONE handle must not be used by two threads at once:
+ *    it owns a single workspace, and its calls are ordered by its stream only.
  *  - There is no CPU fallback: without a CUDA device every entry point fails with DIA_ERR_CUDA.
  */
 #ifndef DIA_H

@@ -219,44 +219,56 @@ class Handle:
         return 1 if I.dim() == 2 else I.shape[0]
 
     def eval_loss_grad(self, I, theta, mask=None, var=None, loss=None, grad=None):
+        """The outputs are allocated on, and written in the order of, the HANDLE's stream (`with` block below): a
+        handle created with its own stream gives tensors that are safe to use on that stream; on any other
+        stream synchronise first (Handle.synchronize())."""
         E = self._epochs(I)
         dev = I.device
-        loss = torch.empty(E, dtype=torch.float64, device=dev) if loss is None else loss
-        grad = torch.empty((E, self.np), dtype=torch.float64, device=dev) if grad is None else grad
-        dia_eval_loss_grad(self._h, E, I, mask, var, theta, loss, grad)
+        with self._stream_ctx():
+            loss = torch.empty(E, dtype=torch.float64, device=dev) if loss is None else loss
+            grad = torch.empty((E, self.np), dtype=torch.float64, device=dev) if grad is None else grad
+            dia_eval_loss_grad(self._h, E, I, mask, var, theta, loss, grad)
         return loss, grad
+
+    def synchronize(self):
+        """Waits for everything enqueued on the handle's stream."""
+        (self.stream if self.stream is not None else torch.cuda.current_stream(self.R.device)).synchronize()
 
     def difference_image(self, I, theta, mask=None, var=None):
         """-> (D float32 [E][n_rows][n_cols], metrics float64 [E][4] = N_used, MFB, MFV, chi^2), CUDA tensors."""
         E = self._epochs(I)
-        D = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.float32, device=I.device)
-        metrics = torch.empty((E, 4), dtype=torch.float64, device=I.device)
-        dia_difference_image(self._h, E, I, mask, var, theta, D, metrics)
+        with self._stream_ctx():
+            D = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.float32, device=I.device)
+            metrics = torch.empty((E, 4), dtype=torch.float64, device=I.device)
+            dia_difference_image(self._h, E, I, mask, var, theta, D, metrics)
         return D, metrics
 
     def hessian(self, I, theta, mask=None, var=None):
         """-> H float64 [np][np] CUDA tensor: Hessian of the objective at theta for the single target I."""
-        H = torch.empty((self.np, self.np), dtype=torch.float64, device=I.device)
-        dia_hessian(self._h, I, mask, var, theta, H)
+        with self._stream_ctx():
+            H = torch.empty((self.np, self.np), dtype=torch.float64, device=I.device)
+            dia_hessian(self._h, I, mask, var, theta, H)
         return H
 
     def covariance(self, H, want_cov: bool = True):
         """-> (cov float64 [np][np] or None, sigma float64 [np], info float64 [5]) CUDA tensors from the Hessian H
         (Eq. 16-17); info = (valid, ln det H, sigma_P, smallest Cholesky pivot, first non-positive pivot or -1)."""
-        cov = torch.empty((self.np, self.np), dtype=torch.float64, device=H.device) if want_cov else None
-        sigma = torch.empty(self.np, dtype=torch.float64, device=H.device)
-        info = torch.empty(5, dtype=torch.float64, device=H.device)
-        dia_covariance(self._h, H, cov, sigma, info)
+        with self._stream_ctx():
+            cov = torch.empty((self.np, self.np), dtype=torch.float64, device=H.device) if want_cov else None
+            sigma = torch.empty(self.np, dtype=torch.float64, device=H.device)
+            info = torch.empty(5, dtype=torch.float64, device=H.device)
+            dia_covariance(self._h, H, cov, sigma, info)
         return cov, sigma, info
 
     def fit(self, I, theta0, opts: Optional[FitOpts] = None, mask=None, var=None):
         """Returns (theta_hat float32 [E][np] CUDA tensor, list[FitResult]); synchronises to read results."""
         E = self._epochs(I)
-        theta = theta0.clone().reshape(E, self.np).contiguous()
-        res = torch.zeros(E * C.sizeof(FitResult), dtype=torch.uint8, device=I.device)
         opts = opts or FitOpts.default()
-        dia_fit(self._h, opts, E, I, mask, var, theta, res)
-        host = res.cpu().numpy().tobytes()          # synchronises
+        with self._stream_ctx():                    # allocate, fit and read back in the order of the handle's stream
+            theta = theta0.clone().reshape(E, self.np).contiguous()
+            res = torch.zeros(E * C.sizeof(FitResult), dtype=torch.uint8, device=I.device)
+            dia_fit(self._h, opts, E, I, mask, var, theta, res)
+            host = res.cpu().numpy().tobytes()      # synchronises that stream
         out = [FitResult.from_buffer_copy(host[i * C.sizeof(FitResult):(i + 1) * C.sizeof(FitResult)])
                for i in range(E)]
         return theta, out
@@ -278,7 +290,13 @@ class Handle:
             self._hgrad = torch.empty((E, self.np), dtype=torch.float64).pin_memory()
 
     def _stream_ctx(self):
-        return torch.cuda.stream(self.stream) if self.stream is not None else torch.cuda.stream(torch.cuda.current_stream())
+        """Context in which torch's current stream is the handle's stream.  A handle with its own stream first makes
+        that stream wait for the caller's current stream, so inputs produced there are complete."""
+        cur = torch.cuda.current_stream(self.R.device)
+        if self.stream is None or self.stream == cur:
+            return torch.cuda.stream(cur)
+        self.stream.wait_stream(cur)
+        return torch.cuda.stream(self.stream)
 
     def fit_host(self, I_host: torch.Tensor, theta0_host: torch.Tensor, opts: Optional[FitOpts] = None,
                  mask_host: Optional[torch.Tensor] = None, chunks: Optional[int] = None):
@@ -286,7 +304,8 @@ class Handle:
         (and the mask) to the device, fits, copies theta-hat and the result structs back and synchronises.
         The batch is cut into `chunks` groups of epochs (default 4 when there are at least 8 epochs): the copy of
         group k+1 runs on a second stream while group k is being fitted, so only the first copy is exposed.
-        Returns (theta_hat [E][np] float32 host tensor, list[FitResult], bytes host->device, bytes device->host)."""
+        Returns (theta_hat [E][np] float32 host tensor, list[FitResult], bytes host->device, bytes device->host);
+        theta_hat is a copy (the pinned staging buffers are reused by the next call)."""
         E = 1 if I_host.dim() == 2 else I_host.shape[0]
         dev = self.R.device
         self._staging(E, dev, mask_host is not None)
@@ -327,10 +346,11 @@ class Handle:
         res = [FitResult.from_buffer_copy(raw[i * nres:(i + 1) * nres]) for i in range(E)]
         h2d = self._dI.numel() * 4 + self._dth.numel() * 4 + (self._dmask.numel() if mask_host is not None else 0)
         d2h = self._hth.numel() * 4 + self._hres.numel()
-        return self._hth, res, h2d, d2h
+        return self._hth.clone(), res, h2d, d2h
 
     def eval_loss_grad_host(self, I_host: torch.Tensor, theta_host: torch.Tensor):
-        """dia_eval_loss_grad with HOST inputs and outputs; returns (loss, grad, bytes h2d, bytes d2h)."""
+        """dia_eval_loss_grad with HOST inputs and outputs; returns (loss, grad, bytes h2d, bytes d2h); loss and grad
+        are copies (the pinned staging buffers are reused by the next call)."""
         E = 1 if I_host.dim() == 2 else I_host.shape[0]
         self._staging(E, self.R.device, False)
         with self._stream_ctx():
@@ -340,7 +360,7 @@ class Handle:
             self._hloss.copy_(self._dloss, non_blocking=True)
             self._hgrad.copy_(self._dgrad, non_blocking=True)
             torch.cuda.current_stream().synchronize()
-        return (self._hloss, self._hgrad, self._dI.numel() * 4 + self._dth.numel() * 4,
+        return (self._hloss.clone(), self._hgrad.clone(), self._dI.numel() * 4 + self._dth.numel() * 4,
                 self._hloss.numel() * 8 + self._hgrad.numel() * 8)
 
     def close(self):

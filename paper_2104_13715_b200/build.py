@@ -1,7 +1,7 @@
 """Builds paper_2104_13715_b200/libdia_b200.so with nvcc for sm_100a (in-tree).
 
 The fused kernel is instantiated for every odd kernel size m <= 47 in four variants; each m is its own
-translation unit (csrc/dia_eval_inst.cu compiled with -DDIA_INST_M=<m>), so the 17 compilations run in parallel.
+translation unit (csrc/dia_eval_inst.cu compiled with -DDIA_INST_M=<m>), so the 24 + 1 compilations run in parallel.
 """
 from __future__ import annotations
 

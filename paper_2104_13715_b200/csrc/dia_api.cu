@@ -27,6 +27,7 @@ struct dia_handle {
   int tiles, n_refs;
   int small_grid;          // > 0: the plain objective of this handle (m <= 5) runs eval_small_kernel on at most this many CTAs
   int grid_limit;          // test hook DIA_GRID_LIMIT (0 = none)
+  int flush_tiles;         // tiles between two FP64 folds of the FP32 gradient strips (kFlushTiles; test hook DIA_FLUSH_TILES)
   dia::ConstBlock* d_const_stage;   // staging copy of the constant block; non-null iff this handle may use the bank
   size_t smem;
   int use_tma;             // rows 16-byte aligned: R / I tiles are staged with TMA tensor copies
@@ -45,6 +46,7 @@ static thread_local std::string g_create_err;
 struct ConstSlot { void* stream = nullptr; int device = -1; int refs = 0; };
 static std::mutex g_const_mutex;
 static ConstSlot g_const_slot[DIA_MAX_KERNEL_SIZE + 1];
+static std::mutex g_const_launch_mutex[DIA_MAX_KERNEL_SIZE + 1];   // (pack, copy, launch) of one evaluation is atomic per kernel size
 static bool const_slot_acquire(int m, void* stream, int device) {
   std::lock_guard<std::mutex> lock(g_const_mutex);
   ConstSlot& sl = g_const_slot[m];
@@ -275,11 +277,17 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
   void* args[] = {(void*)&p, (void*)&tm};
   const bool kc = eval_uses_const(h, p, diff);
   if (kc) {      // refresh the constant block from theta (and the done flags) first, stream-ordered
+    // The block is shared by every handle of this kernel size on this stream: the three enqueues (pack, copy, launch)
+    // must not interleave with those of another host thread driving such a handle, or the other handle's kernel
+    // pixels would be in the bank when this launch runs.  (A dia_fit graph launch is one enqueue and needs no lock.)
+    std::lock_guard<std::mutex> lock(g_const_launch_mutex[h->cfg.m]);
     const int kp = (h->cfg.m + 3) / 4 * 4;
     pack_const_kernel<<<1, 256, 0, h->stream>>>(p.theta, p.done, p.n_epochs, p.np, h->cfg.m, kp, h->d_const_stage);
     cudaError_t ce = cudaMemcpyToSymbolAsync(const_symbol_for(h->cfg.m), h->d_const_stage, const_block_bytes(h, p.n_epochs), 0,
                                              cudaMemcpyDeviceToDevice, h->stream);
     if (ce != cudaSuccess) return ce;
+    return cudaLaunchKernel(kernel_for(h->cfg.m, false, false, true), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
+                            h->smem, h->stream);
   }
   if (p.small_rpt > 0 && !diff) {
     void* sargs[] = {(void*)&p};
@@ -315,6 +323,7 @@ static void fill_params(const dia_handle* h, int n_epochs, const float* d_I, con
   p->huber_c = c.huber_c;  p->sigma0_sq = c.sigma0 * c.sigma0;
   p->inv_gain = c.noise == DIA_NOISE_MODEL ? 1.0f / c.gain : 0.f;
   p->use_tma = 0;
+  p->flush_tiles = h->flush_tiles;
   p->epoch_per_cta = dia::eval_by_epoch(h, n_epochs) ? 1 : 0;
   // plain objective with a small kernel: the register-resident kernel of dia_eval_small.cuh
   p->small_rpt = 0;  p->small_lxlog = 0;  p->small_vec = 0;
@@ -370,7 +379,8 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
     if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
     int o = 0;
     ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, dia::kThreads, h->smem);
-    if (ce != cudaSuccess || o < 1) { int rc = cuda_fail(nullptr, ce, "occupancy query"); delete h; return rc; }
+    if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "occupancy query"); delete h; return rc; }
+    if (o < 1) { int rc = fail(nullptr, DIA_ERR_UNSUPPORTED, "the evaluation kernel of this kernel size does not fit on an SM of this device"); delete h; return rc; }
     occ = (aux == 0 || o < occ) ? o : occ;   // one grid size for all variants
   }
   h->use_tma = 0;
@@ -389,6 +399,11 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
     const int g = std::atoi(lim);
     if (g >= 1) h->grid_limit = g;
     if (g >= 1 && g < h->grid) h->grid = g;
+  }
+  h->flush_tiles = dia::kFlushTiles;
+  if (const char* ft = std::getenv("DIA_FLUSH_TILES")) {   // test hook: how often the FP32 strips are folded
+    const int f = std::atoi(ft);
+    if (f >= 1) h->flush_tiles = f;
   }
   // m <= 5, no flat field, no background polynomial: eval_small_kernel evaluates the plain objective
   h->small_grid = 0;
@@ -633,6 +648,7 @@ extern "C" int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_
   if (launches_per_eval) {
     dia::EvalParams p = {};               // a full batch of the plain objective
     p.n_epochs = h->cfg.max_epochs;  p.flat = h->cfg.d_flat;  p.noise_kind = h->cfg.noise;  p.hess_q0 = -1;
+    if (h->small_grid > 0) p.small_rpt = small_plan(h, p.n_epochs).rpt;     // such handles run eval_small_kernel: no bank
     const bool kc = dia::eval_uses_const(h, p, false);
     *launches_per_eval = 2 + (kc ? 1 : 0) + (h->cfg.lambda_reg > 0.f ? 1 : 0);
   }

@@ -26,7 +26,7 @@ constexpr int kThreads = 256;
 constexpr int kTW = 64, kTH = 64;     // output tile
 constexpr int kP = 16;                // forward strip / gradient chunk length (pixels)
 constexpr int kIPitch = 68;           // I/w tile pitch (floats); 68/4 = 17 is odd => conflict-free rows
-constexpr int kFlushTiles = 32;       // FP32 gradient strips are folded into FP64 at least this often
+constexpr int kFlushTiles = 32;       // FP32 gradient strips are folded into FP64 at least this often (EvalParams::flush_tiles)
 constexpr int kSmemBudget = 113 * 1024;   // per CTA, two CTAs per SM
 constexpr int kSmemBudget1 = 226 * 1024;  // per CTA when only one fits (m >= 33)
 constexpr int kMaxBg = 16;            // background coefficients held per epoch (degree <= 3 uses 10)
@@ -120,6 +120,7 @@ struct EvalParams {
   int small_rpt;             // > 0: eval_small_kernel (dia_eval_small.cuh) runs this evaluation, rows per thread and tile
   int small_lxlog;           // ... log2 of the lanes of a warp that sit side by side in x (the rest stack in y)
   int small_vec;             // ... rows of R and I are 16-byte aligned: 128-bit loads
+  int flush_tiles;           // the FP32 gradient strips are folded into FP64 every flush_tiles tiles (kFlushTiles)
 };
 
 struct TensorMaps {          // passed by value as a __grid_constant__ kernel parameter
@@ -183,6 +184,36 @@ __device__ __forceinline__ float rcp_approx(float x) {
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+
+// Packed FP32 pairs (sm_100 fma.rn.f32x2 / FFMA2): one issue slot carries two fused multiply-adds, which halves the
+// issue slots the stencil and the correlation need and leaves the FMA pipe -- not instruction issue -- as the bound.
+// A pair lives in an aligned 64-bit register; {lo, hi} <-> pair moves are register renamings, not instructions.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ float pk_lo(f32x2 v) {
+  float lo, hi;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  return lo;
+}
+__device__ __forceinline__ float pk_hi(f32x2 v) {
+  float lo, hi;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  return hi;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {      // {a.lo b.lo + c.lo, a.hi b.hi + c.hi}
+  f32x2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
 }
 
 __device__ __forceinline__ double warp_sum_f64(double v) {
@@ -324,11 +355,21 @@ __device__ __forceinline__ void pixel_terms(const EvalParams& p, int e, size_t n
 // Each pair is one FP32 chain that is then added to the running total, so the large centre terms
 // come last ("accumulation order").
 // ------------------------------------------------------------------------------------------------
+// Row chain state of one 16-pixel strip in packed form.  Kernel columns b of even index meet the pixel pairs
+// (0,1), (2,3), ... with an aligned pair of reference pixels, those of odd index the pixel pairs (1,2), (3,4), ...
+// (and pixels 0 and 15 singly): two chains per pixel, one per column parity, both in the order wings -> centre.
+struct RowChain {
+  f32x2 e[kP / 2];         // even columns: pixels (2p, 2p+1)
+  f32x2 o[kP / 2 - 1];     // odd columns: pixels (2p+1, 2p+2)
+  float o0, o15;           // odd columns: pixels 0 and 15
+};
+
 template <int M, bool KC>
 __device__ __forceinline__ void row_chain(const float* __restrict__ Ks, int koff, const float* __restrict__ Rrow, int a,
-                                          float (&rs)[kP], bool first) {
+                                          RowChain& c, bool first) {
   using G = Geo<M>;
-  float k[G::KP], r[G::RSEG];
+  float k[G::KP];
+  f32x2 rp[G::RSEG / 2];                               // rp[t] = (r[2t], r[2t+1])
   if (KC) {                                          // warp-uniform loads from the constant bank
     const float4* k4 = reinterpret_cast<const float4*>(c_blk.K + koff + a * G::KP);
 #pragma unroll
@@ -344,24 +385,55 @@ __device__ __forceinline__ void row_chain(const float* __restrict__ Ks, int koff
       k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
     }
   }
-  const float4* r4 = reinterpret_cast<const float4*>(Rrow + a * G::RPITCH);
+  const ulonglong2* r2 = reinterpret_cast<const ulonglong2*>(Rrow + a * G::RPITCH);
 #pragma unroll
   for (int q = 0; q < G::RSEG / 4; ++q) {
-    const float4 v = r4[q];
-    r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
+    const ulonglong2 v = r2[q];
+    rp[2 * q] = v.x; rp[2 * q + 1] = v.y;
   }
-  if (first) {
+  bool first_e = first, first_o = first;
 #pragma unroll
-    for (int q = 0; q < kP; ++q) rs[q] = k[0] * r[q];
-  } else {
+  for (int ib = 0; ib < M; ++ib) {
+    const int b = (ib == 0) ? 0 : ((ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1));     // 0, M-1, 1, M-2, ..., centre
+    const f32x2 kk = pk2(k[b], k[b]);
+    if ((b & 1) == 0) {
+      if (first_e) {
 #pragma unroll
-    for (int q = 0; q < kP; ++q) rs[q] = fmaf(k[0], r[q], rs[q]);
+        for (int p = 0; p < kP / 2; ++p) c.e[p] = mul2(kk, rp[p + b / 2]);
+      } else {
+#pragma unroll
+        for (int p = 0; p < kP / 2; ++p) c.e[p] = fma2(kk, rp[p + b / 2], c.e[p]);
+      }
+      first_e = false;
+    } else {
+      const float r_first = pk_hi(rp[(b - 1) / 2]);            // r[b]
+      const float r_last = pk_lo(rp[(kP - 1 + b) / 2]);        // r[15 + b]
+      if (first_o) {
+#pragma unroll
+        for (int p = 0; p < kP / 2 - 1; ++p) c.o[p] = mul2(kk, rp[p + (b + 1) / 2]);
+        c.o0 = k[b] * r_first;  c.o15 = k[b] * r_last;
+      } else {
+#pragma unroll
+        for (int p = 0; p < kP / 2 - 1; ++p) c.o[p] = fma2(kk, rp[p + (b + 1) / 2], c.o[p]);
+        c.o0 = fmaf(k[b], r_first, c.o0);  c.o15 = fmaf(k[b], r_last, c.o15);
+      }
+      first_o = false;
+    }
   }
+}
+
+// adds the two chains of a row pair to the running model values
+template <int M>
+__device__ __forceinline__ void chain_to_total(const RowChain& c, float (&tot)[kP]) {
 #pragma unroll
-  for (int ib = 1; ib < M; ++ib) {
-    const int b = (ib & 1) ? (M - 1 - (ib >> 1)) : (ib >> 1);
-#pragma unroll
-    for (int q = 0; q < kP; ++q) rs[q] = fmaf(k[b], r[q + b], rs[q]);
+  for (int p = 0; p < kP / 2; ++p) {
+    float lo = pk_lo(c.e[p]), hi = pk_hi(c.e[p]);
+    if (M > 1) {
+      lo += (p == 0) ? c.o0 : pk_hi(c.o[p > 0 ? p - 1 : 0]);
+      hi += (p == kP / 2 - 1) ? c.o15 : pk_lo(c.o[p < kP / 2 - 1 ? p : 0]);
+    }
+    tot[2 * p] += lo;
+    tot[2 * p + 1] += hi;
   }
 }
 
@@ -371,17 +443,15 @@ __device__ __forceinline__ void forward_strip(const float* __restrict__ Ks, int 
   using G = Geo<M>;
 #pragma unroll
   for (int q = 0; q < kP; ++q) tot[q] = B0;
-  float rs[kP];
+  RowChain c;
 #pragma unroll 1
   for (int ip = 0; ip < G::H; ++ip) {
-    row_chain<M, KC>(Ks, koff, Rrow, ip, rs, true);
-    row_chain<M, KC>(Ks, koff, Rrow, M - 1 - ip, rs, false);
-#pragma unroll
-    for (int q = 0; q < kP; ++q) tot[q] += rs[q];
+    row_chain<M, KC>(Ks, koff, Rrow, ip, c, true);
+    row_chain<M, KC>(Ks, koff, Rrow, M - 1 - ip, c, false);
+    chain_to_total<M>(c, tot);
   }
-  row_chain<M, KC>(Ks, koff, Rrow, G::H, rs, true);
-#pragma unroll
-  for (int q = 0; q < kP; ++q) tot[q] += rs[q];
+  row_chain<M, KC>(Ks, koff, Rrow, G::H, c, true);
+  chain_to_total<M>(c, tot);
 }
 
 // Adds the background terms beyond b_00 (Eq. 18-19) to the model strip.
@@ -512,6 +582,103 @@ __device__ __forceinline__ void strip_epilogue(const EvalParams& p, int e, size_
 #pragma unroll
   for (int q = 0; q < kP / 4; ++q)
     reinterpret_cast<float4*>(wrow)[q] = make_float4(iv[4 * q], iv[4 * q + 1], iv[4 * q + 2], iv[4 * q + 3]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// gradient: thread (a, s) owns g[a][0..M-1] and correlates 16-pixel chunks of the weight tile against row i + a of
+// the staged R tile: g[a][b] += w[q] r[q + b].  Packed form: for even q the kernel columns pair up as (0,1), (2,3), ...
+// (+ column M-1 singly) against aligned pairs of reference pixels, for odd q as (1,2), (3,4), ... (+ column 0 singly);
+// the two pairings are two accumulator sets, added when the strip is stored.  Kernel sizes whose 2 M accumulators
+// do not fit the register budget of two CTAs per SM keep one set and take the odd pixels with scalar FMAs.
+// ------------------------------------------------------------------------------------------------
+template <int M>
+struct GradAcc {
+  static constexpr int NP = (M - 1) / 2 > 0 ? (M - 1) / 2 : 1;
+  static constexpr bool TWO = Geo<M>::CTAS == 1 || (2 * M + kP + Geo<M>::RSEG <= 108);
+  f32x2 e[NP];    // columns (2t, 2t+1)
+  float el;       // column M-1
+  f32x2 o[NP];    // columns (2t+1, 2t+2)        (TWO only)
+  float of;       // column 0                    (TWO only)
+};
+
+template <int M>
+__device__ __forceinline__ void grad_acc_load(GradAcc<M>& A, const float4* __restrict__ myacc) {
+  using G = Geo<M>;
+  float acc[G::KP];
+#pragma unroll
+  for (int q = 0; q < G::KP / 4; ++q) {
+    const float4 v = myacc[q];
+    acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
+  }
+#pragma unroll
+  for (int t = 0; t < (M - 1) / 2; ++t) { A.e[t] = pk2(acc[2 * t], acc[2 * t + 1]); A.o[t] = pk2(0.f, 0.f); }
+  A.el = acc[M - 1];
+  A.of = 0.f;
+}
+template <int M>
+__device__ __forceinline__ void grad_acc_zero(GradAcc<M>& A) {
+#pragma unroll
+  for (int t = 0; t < (M - 1) / 2; ++t) { A.e[t] = pk2(0.f, 0.f); A.o[t] = pk2(0.f, 0.f); }
+  A.el = 0.f;
+  A.of = 0.f;
+}
+template <int M>
+__device__ __forceinline__ void grad_acc_store(const GradAcc<M>& A, float4* __restrict__ myacc) {
+  using G = Geo<M>;
+  float acc[G::KP];
+#pragma unroll
+  for (int b = 0; b < G::KP; ++b) acc[b] = 0.f;
+#pragma unroll
+  for (int t = 0; t < (M - 1) / 2; ++t) { acc[2 * t] = pk_lo(A.e[t]); acc[2 * t + 1] = pk_hi(A.e[t]); }
+  acc[M - 1] = A.el;
+  if (GradAcc<M>::TWO) {
+    acc[0] += A.of;
+#pragma unroll
+    for (int t = 0; t < (M - 1) / 2; ++t) { acc[2 * t + 1] += pk_lo(A.o[t]); acc[2 * t + 2] += pk_hi(A.o[t]); }
+  }
+#pragma unroll
+  for (int q = 0; q < G::KP / 4; ++q)
+    myacc[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+}
+// one 16-pixel chunk: wrow = the chunk of the weight tile, rrow = row i + a of the R tile at the chunk's first column
+template <int M>
+__device__ __forceinline__ void grad_chunk(GradAcc<M>& A, const float* __restrict__ wrow, const float* __restrict__ rrow) {
+  using G = Geo<M>;
+  float w[kP];
+  f32x2 rp[G::RSEG / 2];
+  const float4* w4 = reinterpret_cast<const float4*>(wrow);
+#pragma unroll
+  for (int q = 0; q < kP / 4; ++q) {
+    const float4 v = w4[q];
+    w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
+  }
+  const ulonglong2* r2 = reinterpret_cast<const ulonglong2*>(rrow);
+#pragma unroll
+  for (int q = 0; q < G::RSEG / 4; ++q) {
+    const ulonglong2 v = r2[q];
+    rp[2 * q] = v.x; rp[2 * q + 1] = v.y;
+  }
+#pragma unroll
+  for (int q = 0; q < kP; ++q) {
+    const f32x2 ww = pk2(w[q], w[q]);
+    if ((q & 1) == 0) {
+#pragma unroll
+      for (int t = 0; t < (M - 1) / 2; ++t) A.e[t] = fma2(ww, rp[q / 2 + t], A.e[t]);
+      A.el = fmaf(w[q], pk_lo(rp[(q + M - 1) / 2]), A.el);
+    } else if (GradAcc<M>::TWO) {
+      A.of = fmaf(w[q], pk_hi(rp[(q - 1) / 2]), A.of);
+#pragma unroll
+      for (int t = 0; t < (M - 1) / 2; ++t) A.o[t] = fma2(ww, rp[(q + 1) / 2 + t], A.o[t]);
+    } else {
+#pragma unroll
+      for (int t = 0; t < (M - 1) / 2; ++t) {       // r[q + 2t] = hi of pair (q + 2t - 1) / 2, r[q + 2t + 1] = lo of the next
+        const float lo = fmaf(w[q], pk_hi(rp[(q - 1) / 2 + t]), pk_lo(A.e[t]));
+        const float hi = fmaf(w[q], pk_lo(rp[(q + 1) / 2 + t]), pk_hi(A.e[t]));
+        A.e[t] = pk2(lo, hi);
+      }
+      A.el = fmaf(w[q], pk_hi(rp[(q + M - 2) / 2]), A.el);
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -749,42 +916,20 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) eval_kernel(const Eval
 
     // ------------------------------------------------------------------ gradient
     if (!DIFF && g_active) {
-      float acc[G::KP];
-#pragma unroll
-      for (int q = 0; q < G::KP / 4; ++q) {
-        const float4 v = myacc[q];
-        acc[4 * q] = v.x; acc[4 * q + 1] = v.y; acc[4 * q + 2] = v.z; acc[4 * q + 3] = v.w;
-      }
+      GradAcc<M> A;
+      grad_acc_load<M>(A, myacc);
       const int rows_here = min(kTH, vr - tile_y * kTH);
       const int n_items = rows_here * (kTW / kP);
 #pragma unroll 1
       for (int item = g_s; item < n_items; item += G::S) {
         const int i = item / (kTW / kP), c = item - i * (kTW / kP);
-        float w[kP], r[G::RSEG];
-        const float4* w4 = reinterpret_cast<const float4*>(Ws + i * kIPitch + c * kP);
-#pragma unroll
-        for (int q = 0; q < kP / 4; ++q) {
-          const float4 v = w4[q];
-          w[4 * q] = v.x; w[4 * q + 1] = v.y; w[4 * q + 2] = v.z; w[4 * q + 3] = v.w;
-        }
-        const float4* r4 = reinterpret_cast<const float4*>(Rs + (i + g_a) * G::RPITCH + c * kP);
-#pragma unroll
-        for (int q = 0; q < G::RSEG / 4; ++q) {
-          const float4 v = r4[q];
-          r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
-        }
-#pragma unroll
-        for (int q = 0; q < kP; ++q)
-#pragma unroll
-          for (int b = 0; b < M; ++b) acc[b] = fmaf(w[q], r[q + b], acc[b]);
+        grad_chunk<M>(A, Ws + i * kIPitch + c * kP, Rs + (i + g_a) * G::RPITCH + c * kP);
       }
-#pragma unroll
-      for (int q = 0; q < G::KP / 4; ++q)
-        myacc[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+      grad_acc_store<M>(A, myacc);
     }
     __syncthreads();                       // (B) everyone is done reading this w tile and R buffer
     if (G::NRBUF == 1 && more) stage_R<M>(p, tm, en, tn, smem_u32(Rbuf(it + 1)), barR(it + 1));
-    if (!DIFF && ++since_flush == kFlushTiles && more && jn == j) flush();
+    if (!DIFF && ++since_flush == p.flush_tiles && more && jn == j) flush();
     j = jn;
     t = tn;
     ++it;
@@ -873,33 +1018,14 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) hess_block_kernel(cons
       }
       __syncthreads();
       if (g_active) {                        // the gradient phase of eval_kernel on this weight tile
-        float acc[G::KP];
-#pragma unroll
-        for (int c = 0; c < G::KP; ++c) acc[c] = 0.f;
+        GradAcc<M> A;
+        grad_acc_zero<M>(A);
 #pragma unroll 1
         for (int item = g_s; item < n_items; item += G::S) {
           const int i = item / (kTW / kP), c = item - i * (kTW / kP);
-          float w[kP], r[G::RSEG];
-          const float4* w4 = reinterpret_cast<const float4*>(Is + i * kIPitch + c * kP);
-#pragma unroll
-          for (int k = 0; k < kP / 4; ++k) {
-            const float4 v = w4[k];
-            w[4 * k] = v.x; w[4 * k + 1] = v.y; w[4 * k + 2] = v.z; w[4 * k + 3] = v.w;
-          }
-          const float4* r4 = reinterpret_cast<const float4*>(Rs + (i + g_a) * G::RPITCH + c * kP);
-#pragma unroll
-          for (int k = 0; k < G::RSEG / 4; ++k) {
-            const float4 v = r4[k];
-            r[4 * k] = v.x; r[4 * k + 1] = v.y; r[4 * k + 2] = v.z; r[4 * k + 3] = v.w;
-          }
-#pragma unroll
-          for (int k = 0; k < kP; ++k)
-#pragma unroll
-            for (int b = 0; b < M; ++b) acc[b] = fmaf(w[k], r[k + b], acc[b]);
+          grad_chunk<M>(A, Is + i * kIPitch + c * kP, Rs + (i + g_a) * G::RPITCH + c * kP);
         }
-#pragma unroll
-        for (int k = 0; k < G::KP / 4; ++k)
-          myacc[k] = make_float4(acc[4 * k], acc[4 * k + 1], acc[4 * k + 2], acc[4 * k + 3]);
+        grad_acc_store<M>(A, myacc);
       }
       __syncthreads();
       double* outp = p.partials + ((size_t)jq * p.part_rows) * ncols + blockIdx.x;

@@ -49,6 +49,11 @@ def max_over_ranks(value: float, device=None, group=None) -> float:
 # full loss and gradient are the sums of the per-rank results.  R is constant, so there is no halo exchange per
 # evaluation; the only collective is one (m^2 + 2)-double all-gather, summed in rank order on every rank (deterministic,
 # identical on all ranks).  Evaluation only: dia_fit's on-device loop has no place for a collective.
+# Limits: (1) plain scalar background only -- with bg_degree > 0 every band's handle would centre and normalise the
+# coordinates of Eq. 19 on its own sub-image, so the band sums would not add up to the full-image objective;
+# (2) a flat field, mask or variance map must be sliced to the band's image rows by the caller, like R and I;
+# (3) a rank whose band is empty (more ranks than valid rows) creates no handle and contributes zeros
+# (`band_is_empty`; dia_create rejects an image smaller than the kernel).
 def row_band(n_rows: int, m: int, world_size: int, rank: int) -> Tuple[int, int, int, int]:
     """-> (v0, v1, i0, i1): valid rows [v0, v1) owned by `rank` (indices into the valid region, n_rows - m + 1 rows in
     all, split like epoch_shard) and the image rows [i0, i1) = [v0, v1 + m - 1) to hand to dia_create / the targets."""
@@ -57,6 +62,12 @@ def row_band(n_rows: int, m: int, world_size: int, rank: int) -> Tuple[int, int,
         raise ValueError("bad image or kernel size")
     v0, v1 = epoch_shard(n_valid, world_size, rank)
     return v0, v1, v0, (v1 + m - 1 if v1 > v0 else v0)
+
+
+def band_is_empty(band: Tuple[int, int, int, int]) -> bool:
+    """True when row_band gave this rank no valid row: it must not call dia_create and contributes
+    torch.zeros(m*m + 2, dtype=float64) to sum_over_ranks_in_order."""
+    return band[1] <= band[0]
 
 
 def sum_over_ranks_in_order(local: torch.Tensor, group=None) -> torch.Tensor:

@@ -112,10 +112,17 @@ def test_covariance_of_fitted_model_end_to_end(dia, c, n, m):
     e_sig = np.abs(sigg / sigo - 1.0).max()
     print(f"   single-pixel uncertainties: max |sigma_gpu / sigma_or - 1| = {e_sig:.2e}, first-order bound {bound:.2e}")
     assert e_sig <= max(bound, 1e-6)
-    # ln det H moves by tr(H^-1 dH) to first order: the float32 Hessian's error, not the factorisation's
+    # ln det H: the device factorises ITS Hessian, so the reference value is numpy's FP64 log-determinant of that same
+    # matrix (the factorisation's accuracy), and the difference to the oracle's ln det is the float32 Hessian's doing:
+    # tr(H^-1 dH) to first order, reported -- with cond(H) ~ 1e9 the relative perturbation |H^-1 dH| of the weakest
+    # directions is O(1) (see the bound above) and the higher orders are as large as the first, so no linearised
+    # value is asserted
+    sign, lndet_np = np.linalg.slogdet(Hg.cpu().numpy())
     d_lndet = float(np.sum(covo * (Hg.cpu().numpy() - Ho)))
-    print(f"   ln det H {infog[1]:.6f} ({infoo[1]:.6f}), first-order prediction of the difference {d_lndet:.3e}")
-    assert abs(infog[1] - infoo[1] - d_lndet) <= 0.2 * abs(d_lndet) + 1e-8 * abs(infoo[1])
+    print(f"   ln det H {infog[1]:.6f} (numpy on the same matrix {lndet_np:.6f}; oracle's H {infoo[1]:.6f}, first-order "
+          f"prediction of the difference {d_lndet:.3e})")
+    assert sign > 0 and abs(infog[1] - lndet_np) <= 1e-9 * abs(lndet_np)
+    assert abs(infog[1] - infoo[1]) <= 1e-4 * abs(infoo[1])
     # the linear algebra alone, both sides on the oracle's Hessian
     cov2, sig2, info2 = (t.cpu().numpy() for t in h.covariance(_dev(Ho)))
     _compare(cov2, sig2, info2, covo, sigo, infoo, 1e-9 * max(1.0, cond / 1e5))

@@ -374,6 +374,42 @@ def test_constant_bank_variant_matches_shared_memory_variant(dia, monkeypatch):
     h3.close()
 
 
+def test_constant_bank_two_host_threads_two_handles(dia):
+    """Threading contract of include/dia.h: different handles may be driven from different host threads, also when they
+    share a stream and therefore the constant block of their kernel size.  Each evaluation is three enqueues (pack,
+    copy to the bank, launch); the library makes the triple atomic, so no evaluation may run with the other handle's
+    kernel pixels.  Two threads, 40 evaluations each at different theta, every result bit-identical to the one
+    computed alone."""
+    import threading
+    w = make_workload(4, n=640, n_epochs=3, m=19)
+    I = _dev(w.I)
+    ths = [_dev(w.theta_true.astype(np.float32)), _dev(w.theta0)]
+    hs = [_handle(dia, w), _handle(dia, w)]
+    assert all(h.info()["launches_per_eval"] == 3 for h in hs)
+    want = [h.eval_loss_grad(I, th) for h, th in zip(hs, ths)]
+    torch.cuda.synchronize()
+    assert not torch.equal(want[0][0], want[1][0])
+    bad, errs = [0, 0], []
+    go_flag = threading.Barrier(2)
+
+    def work(k):
+        try:
+            torch.cuda.set_device(0)
+            go_flag.wait()
+            outs = [hs[k].eval_loss_grad(I, ths[k]) for _ in range(40)]
+            torch.cuda.synchronize()
+            bad[k] = sum(1 for L, g in outs if not (torch.equal(L, want[k][0]) and torch.equal(g, want[k][1])))
+        except Exception as exc:      # noqa: BLE001 -- reported below
+            errs.append(exc)
+
+    ts = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert not errs, errs
+    assert bad == [0, 0], f"evaluations that saw the other handle's kernel: {bad}"
+    [h.close() for h in hs]
+
+
 def test_constant_bank_variant_on_a_batch_of_medium_images(dia, monkeypatch):
     """The constant-bank variant is chosen by launch length, not image size: 24 epochs of 300^2 (25 tiles each,
     three waves of the 296 resident CTAs) use it; same bits as the shared-memory variant, and the oracle's values."""

@@ -17,7 +17,7 @@ from __future__ import annotations
 
 import dataclasses
 import math
-from typing import Optional
+from typing import Optional, Sequence
 
 import numpy as np
 from scipy import signal, special
@@ -121,6 +121,20 @@ def render_stars(n: int, xs, ys, fluxes, fwhm: float, sky: float) -> np.ndarray:
         img += np.bincount(flat_idx, weights=stamp[ok], minlength=n * n)
         del stamp, ex, ey, gx, gy
     return img.reshape(n, n) + sky
+
+
+REF_NOISE_VARIANCE_RATIO = 0.1     # "10 times less variance than the target"
+
+
+def add_reference_noise(cfg: Config, R_noiseless: np.ndarray) -> np.ndarray:
+    """The paper's S10 reference noise: sigma_R = 10^-1/2 sqrt(sigma0^2 + R_noiseless / G) (Eq. 22, PAPER.md:280,
+    with the config's sigma0 and gain in place of the paper's 5 and 1) and R_noisy = R_noiseless + W sigma_R,
+    W ~ N(0, 1) (Eq. 23).  Own RNG stream `default_rng(777000 + c)`, so that the streams of the
+    noiseless recipe are untouched.  float64 in, float32 out."""
+    rng = np.random.default_rng(777000 + cfg.index)
+    R64 = np.asarray(R_noiseless, dtype=np.float64)
+    sig = np.sqrt(REF_NOISE_VARIANCE_RATIO * (cfg.sigma0 ** 2 + np.maximum(R64, 0.0) / cfg.gain))
+    return (R64 + rng.standard_normal(R64.shape) * sig).astype(np.float32)
 
 
 def make_reference(cfg: Config, n: Optional[int] = None) -> np.ndarray:
@@ -251,18 +265,23 @@ def gaussian_kernel_init(m: int, phi_k: float, b0: float) -> np.ndarray:
 
 
 def make_workload(c: int, n: Optional[int] = None, n_epochs: Optional[int] = None,
-                  m: Optional[int] = None, noise: bool = True) -> Workload:
+                  m: Optional[int] = None, noise: bool = True, ref_noise: bool = False,
+                  epochs: Optional[Sequence[int]] = None) -> Workload:
     """Config `c` of BASELINE.json; n / n_epochs / m may be reduced for tests
-    (same recipe, same stellar density, same RNG streams)."""
+    (same recipe, same stellar density, same RNG streams).  `epochs` selects target epochs by index (default
+    0 .. n_epochs-1).  `ref_noise`: the targets are simulated from the noiseless reference as
+    always, and the reference handed to the fit carries the paper's S10 noise (Eq. 22-23) -- the situation of
+    every image pair of the paper; BASELINE.json's configs are the ref_noise = False case."""
     cfg = CONFIGS[c]
     n = cfg.n if n is None else n
     m = cfg.m if m is None else m
     E = cfg.n_epochs if n_epochs is None else n_epochs
-    R = make_reference(cfg, n)
+    R_true = make_reference(cfg, n)
+    R = add_reference_noise(cfg, R_true) if ref_noise else R_true
     Is, thetas, masks, theta0s = [], [], [], []
     flat = None
-    for e in range(E):
-        I, th, fl, mk = make_target(cfg, e, R, m, noise)
+    for e in (range(E) if epochs is None else epochs):
+        I, th, fl, mk = make_target(cfg, e, R_true, m, noise)
         Is.append(I)
         thetas.append(th)
         theta0s.append(theta_init(R, I, m))
