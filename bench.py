@@ -43,9 +43,20 @@ STEP_ADAM, STEP_LBFGS = 8, 3
 METRIC = "loss+grad evaluations per second (4096^2 image, 19x19 kernel + B0, per epoch)"
 UNIT = "evals/s"
 SM_COUNT, FP32_LANES_PER_SM = 148, 128          # B200 (B200_PROFILING.md: 148 SMs; 128 FP32 lanes per SM)
-# dram__bytes_read.sum + dram__bytes_write.sum of one eval_kernel<19,false> launch over the 16-epoch batch,
-# from the ncu --set full capture summarised in profiles/ (None until captured)
-TRAFFIC_BYTES_PER_LAUNCH = 1.403e9     # profiles/r01_eval_kernel_full.md (last capture of r01: 1.388 GB read + 15.6 MB written)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+
+
+def measured_traffic(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` over the 16-epoch batch, from the last
+    matching row of profiles/dram_traffic.csv (one row per committed `ncu --set full` capture: kernel, capture file,
+    commit, bytes read, bytes written); None when no capture is recorded."""
+    try:
+        import csv
+        rows = list(csv.reader(l for l in open(TRAFFIC_CSV) if l.strip() and not l.startswith("#")))
+        rows = [r for r in rows[1:] if r[0] == kernel]
+        return (float(rows[-1][3]) + float(rows[-1][4]), rows[-1][1], rows[-1][2]) if rows else (None, None, None)
+    except Exception:
+        return None, None, None
 
 
 def useful_fma(n=N, m=M, epochs=1):
@@ -169,6 +180,20 @@ def oracle_eval_rate(cfg, R, I0, th0, crop: int, repeats: int = 1):
     return frac / best, best, oracle.num_threads()
 
 
+def oracle_single_thread_rate():
+    """the oracle timed single-threaded beside the OpenMP figure.  The thread count of the oracle is
+    fixed when its library loads, so this runs `bench.py --impl reference` once more in a child process with
+    OMP_NUM_THREADS=1 (two steps of a 1024^2 evaluation, scaled to full-size evaluations per second)."""
+    try:
+        env = dict(os.environ, OMP_NUM_THREADS="1", RANK="0", WORLD_SIZE="1")
+        out = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "reference", "--steps", "2", "--warmup", "1"],
+                             env=env, capture_output=True, text=True, timeout=600)
+        d = json.loads(out.stdout.strip().splitlines()[-1])
+        return {"value": d["value"], "unit": UNIT, "cores": d["cpu_baseline"]["cores"], "sample": d["cpu_baseline"]["sample"]}
+    except Exception as exc:      # noqa: BLE001 -- a reported baseline, never fatal
+        return {"error": repr(exc)}
+
+
 def stamp_batch_rate(dia, dev, n_stamps=296, n=142, m=19):
     """Throughput of the one-reference-per-epoch mode on synthetic stamps of the paper's stamp shape
     (142^2 images, 19x19 kernel): batched evaluations and a lock-step fit."""
@@ -250,7 +275,9 @@ def other_configs(dia, dev):
         out.append({"config": c, "n": w.n, "m": w.m, "loss": w.loss, "evals_per_s": 1e3 / ms_eval,
                     "us_per_eval": 1e3 * ms_eval, "frac_fp32_nominal": 2.0 * useful_fma(w.n, w.m) / (ms_eval * 1e-3) / 1e12 /
                     (SM_COUNT * FP32_LANES_PER_SM * 2 * 1.965e9 / 1e12),
-                    "fits_per_s": 1e3 / ms_fit, "ms_per_fit": ms_fit, "n_adam": res[0].n_adam, "n_lbfgs": res[0].n_lbfgs,
+                    "fits_per_s": 1e3 / ms_fit, "ms_per_fit": ms_fit, "lr_b0": float(opts.lr_b0),
+                    "adam_met_switch_rule": bool(res[0].n_adam < opts.max_adam_iters),
+                    "n_adam": res[0].n_adam, "n_lbfgs": res[0].n_lbfgs,
                     "status": res[0].status, "photometric_scale": round(res[0].photometric_scale, 5)})
     return out
 
@@ -421,11 +448,12 @@ def run_gpu(args):
     # ---- the dominant kernel alone: back-to-back batched evaluations (eval_kernel + the small reduce kernel)
     loss = torch.empty(E, dtype=torch.float64, device=dev)
     grad = torch.empty((E, M * M + 1), dtype=torch.float64, device=dev)
-    n_eval_launch = 10
+    n_eval_launch, n_series = 50, 5            # back-to-back launches between two events, median of 5 series
     for _ in range(3):
         h.eval_loss_grad(dI, dth0, loss=loss, grad=grad)
-    ms_k, _ = timed(lambda: h.eval_loss_grad(dI, dth0, loss=loss, grad=grad), n_eval_launch)
-    ms_kernel = ms_k / n_eval_launch
+    series = sorted(timed(lambda: h.eval_loss_grad(dI, dth0, loss=loss, grad=grad), n_eval_launch)[0] / n_eval_launch
+                    for _ in range(n_series))
+    ms_kernel = series[n_series // 2]
     flop_per_launch = 2.0 * useful_fma(epochs=E)
     achieved_tflops = flop_per_launch / (ms_kernel * 1e-3) / 1e12
     info = h.info()
@@ -436,17 +464,26 @@ def run_gpu(args):
         sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
         nominal_tflops = SM_COUNT * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
         measured_fma = dia.dia_measure_fp32_peak()
+        patterns = {name: 2.0 * dia.dia_measure_fp32_pattern(k) / 1e12 for k, name in
+                    enumerate(("pipe_peak_one_vector_register", "forward_ffma2_uniform_multiplicand",
+                               "gradient_ffma2_vector_operands", "scalar_ffma_three_vector_registers"))}
+        kernel_name = f"dia::eval_kernel<{M}, false, false, true>"
+        traffic, traffic_file, traffic_commit = measured_traffic(kernel_name)
         roof = {"bound": "alu", "achieved": achieved_tflops, "peak": nominal_tflops, "unit": "TFLOP/s",
-                "frac": achieved_tflops / nominal_tflops, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                "frac": achieved_tflops / nominal_tflops, "traffic": traffic,
+                "traffic_source": f"profiles/dram_traffic.csv: {traffic_file} at commit {traffic_commit}",
+                "ms_per_launch_series": series, "pattern_peaks_tflops": patterns,
                 "peak_kind": f"nominal FP32 FMA pipe: {SM_COUNT} SMs x {FP32_LANES_PER_SM} lanes x 2 FLOP x "
                              f"{sm_max_mhz:.0f} MHz (DESIGN.md section 8)",
                 "peak_measured": 2.0 * measured_fma / 1e12,
                 "frac_of_measured": achieved_tflops / (2.0 * measured_fma / 1e12),
-                "peak_measured_kind": "register-only FFMA microbenchmark run in this process (dia_measure_fp32_peak)",
-                "kernel": f"dia::eval_kernel<{M}, false>", "ms_per_launch": ms_kernel,
+                "peak_measured_kind": "register-only FFMA microbenchmark run in this process (dia_measure_fp32_peak: FFMAs "
+                                      "reading one vector register; the kernel's own operand patterns are in pattern_peaks_tflops)",
+                "kernel": kernel_name, "ms_per_launch": ms_kernel,
                 "flop_per_launch": flop_per_launch,
                 "how": f"CUDA events around {n_eval_launch} back-to-back dia_eval_loss_grad launches of the "
-                       f"{E}-epoch batch (eval_kernel + reduce_partials_kernel), useful FLOP = 4 m^2 per valid pixel",
+                       f"{E}-epoch batch (pack_const + eval_kernel + reduce_partials_kernel), median of {n_series} series, "
+                       f"useful FLOP = 4 m^2 per valid pixel",
                 "hbm_gbs_algorithmic": (4.0 * N * N * (1 + E)) / (ms_kernel * 1e-3) / 1e9,
                 "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -547,6 +584,8 @@ def run_gpu(args):
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"FP64 oracle loss+gradient evaluation of epoch 0 at the full {crop}x{crop} size, "
                                           f"best of 3 calls ({sec:.2f} s per call, OpenMP over all host cores)"}
+        line["cpu_baseline"]["host_cores_available"] = len(os.sched_getaffinity(0))
+        line["cpu_baseline"]["single_thread"] = oracle_single_thread_rate()
         line["cpu_baseline"].update(oracle_fit_and_b08_times())
     h.close()
     if rank == 0:

@@ -179,11 +179,17 @@ const char* dia_last_error(const dia_handle* h);
 int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_per_block,
                  int* smem_bytes, int* launches_per_eval);
 
-/* Register-only FFMA microbenchmark on the current device (the operand pattern of the stencil's inner
- * loop, no memory traffic): writes the measured FP32 peak in fused multiply-adds per second to
- * *fma_per_second (HOST pointer).  Synchronises.  This is the "measured" denominator of the FP32
- * roofline fraction; the nominal one is SMs x 128 lanes x SM clock. */
+/* Register-only FMA microbenchmarks on the current device (no memory traffic; SURVEY.md section 7 hard part 2 asks for
+ * the measured FP32 peak that MEASURED_PEAKS.json lacks).  Each writes thread-level fused multiply-adds per second to
+ * *fma_per_second (HOST pointer) and synchronises.
+ *   dia_measure_fp32_peak: the FMA pipe's peak, FFMAs that read one vector register (pattern 0) -- 97 % of the
+ *     nominal SMs x 128 lanes x SM clock on B200, i.e. the nominal peak is attainable and is what the roofline uses;
+ *   dia_measure_fp32_pattern: 0 = that; 1 = the forward stencil's packed FFMA2 with the kernel pixel in a uniform
+ *     register; 2 = the gradient correlation's packed FFMA2 with all operands in vector registers; 3 = scalar FFMA with
+ *     three vector registers (the loops before packing).  1-3 show what the register file's operand bandwidth allows
+ *     the kernel's own inner loops (profiles/r02_fp32_peak_sass.md). */
 int dia_measure_fp32_peak(void* stream, double* fma_per_second);
+int dia_measure_fp32_pattern(void* stream, int pattern, double* fma_per_second);
 
 #ifdef __cplusplus
 }

@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     dia_eval_loss_grad,
     dia_fit,
     dia_measure_fp32_peak,
+    dia_measure_fp32_pattern,
     load_library,
     LOSS_GAUSSIAN,
     LOSS_HUBER,

@@ -19,7 +19,7 @@ NOISE_MODEL, NOISE_FIXED = 0, 1
 FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
-                    "dia_measure_fp32_peak", "dia_difference_image", "dia_hessian", "dia_covariance")
+                    "dia_measure_fp32_peak", "dia_measure_fp32_pattern", "dia_difference_image", "dia_hessian", "dia_covariance")
 
 
 class DiaError(RuntimeError):
@@ -92,6 +92,7 @@ def load_library(build_if_missing: bool = True):
     lib.dia_covariance.argtypes = [C.c_void_p] * 5
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
     lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+    lib.dia_measure_fp32_pattern.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
     _LIB = lib
     return lib
 
@@ -177,6 +178,14 @@ def dia_measure_fp32_peak(stream: Optional[torch.cuda.Stream] = None) -> float:
     """Measured FP32 peak of the current device in FMA/s (register-only FFMA microbenchmark)."""
     out = C.c_double()
     _check(load_library().dia_measure_fp32_peak(None if stream is None else stream.cuda_stream, C.byref(out)))
+    return out.value
+
+
+def dia_measure_fp32_pattern(pattern: int, stream: Optional[torch.cuda.Stream] = None) -> float:
+    """FMA/s of one operand pattern of the register-only microbenchmark (include/dia.h): 0 pipe peak, 1 forward
+    stencil (FFMA2, uniform multiplicand), 2 gradient (FFMA2, vector operands), 3 scalar three-register FFMA."""
+    out = C.c_double()
+    _check(load_library().dia_measure_fp32_pattern(None if stream is None else stream.cuda_stream, int(pattern), C.byref(out)))
     return out.value
 
 

@@ -124,7 +124,7 @@ DIA_FOR_EACH_M(X)
 // aux = true: mask / flat field / caller variance map present (read from global memory per pixel);
 // diff = true: difference-image instantiation; kc = true: kernel pixels in the constant bank
 static const void* kernel_for(int m, bool aux, bool diff = false, bool kc = false) {
-  const int variant = diff ? 2 : aux ? 1 : kc ? 3 : 0;
+  const int variant = diff ? 2 : aux ? (kc ? 5 : 1) : kc ? 3 : 0;
   switch (m) {
 #define X(MM) case MM: return dia::eval_kernel_ptr_m##MM(variant);
     DIA_FOR_EACH_M(X)
@@ -255,14 +255,15 @@ int eval_part_cols(const dia_handle* h, int n_epochs) {
   const int g = eval_grid(h, n_epochs);
   return h->tiles < g ? h->tiles : g;
 }
-// Constant-bank variant: plain objective (no mask / flat / variance map), few enough epochs, and enough work per
+// Constant-bank variant: loss and gradient (plain or with mask / flat / variance map; not the Hessian rows, whose
+// "epochs" share one theta), few enough epochs, and enough work per
 // launch: refreshing the bank costs ~5.5 us (pack kernel + copy to the symbol) and buys ~9 % of the kernel time,
 // which pays from about 60 us on -- two or more tiles per resident CTA at m = 19 (bench.py --sweep).
 bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff) {
   const int m = h->cfg.m, kp = (m + 3) / 4 * 4;
   const long long items = (long long)p.n_epochs * h->tiles;
   const long long waves = (items + h->grid - 1) / h->grid;
-  return h->d_const_stage && !diff && p.small_rpt == 0 && !eval_is_aux(p) && !eval_by_epoch(h, p.n_epochs) && waves * m * m >= 2 * 19 * 19 &&
+  return h->d_const_stage && !diff && p.small_rpt == 0 && p.hess_q0 < 0 && !eval_by_epoch(h, p.n_epochs) && waves * m * m >= 2 * 19 * 19 &&
          p.n_epochs <= kConstEpochs &&
          (long long)p.n_epochs * m * kp <= kConstK;
 }
@@ -270,7 +271,7 @@ size_t const_block_bytes(const dia_handle* h, int n_epochs) {
   const int kp = (h->cfg.m + 3) / 4 * 4;
   return offsetof(ConstBlock, K) + sizeof(float) * (size_t)n_epochs * h->cfg.m * kp;
 }
-const void* eval_kernel_ptr_kc(const dia_handle* h) { return kernel_for(h->cfg.m, false, false, true); }
+const void* eval_kernel_ptr_kc(const dia_handle* h, const EvalParams& p) { return kernel_for(h->cfg.m, eval_is_aux(p), false, true); }
 ConstBlock* const_stage(const dia_handle* h) { return h->d_const_stage; }
 const void* const_symbol(const dia_handle* h) { return const_symbol_for(h->cfg.m); }
 cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMaps& tm, bool diff) {
@@ -286,7 +287,7 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
     cudaError_t ce = cudaMemcpyToSymbolAsync(const_symbol_for(h->cfg.m), h->d_const_stage, const_block_bytes(h, p.n_epochs), 0,
                                              cudaMemcpyDeviceToDevice, h->stream);
     if (ce != cudaSuccess) return ce;
-    return cudaLaunchKernel(kernel_for(h->cfg.m, false, false, true), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
+    return cudaLaunchKernel(kernel_for(h->cfg.m, eval_is_aux(p), false, true), dim3(eval_grid(h, p.n_epochs)), dim3(kThreads), args,
                             h->smem, h->stream);
   }
   if (p.small_rpt > 0 && !diff) {
@@ -373,8 +374,8 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   h->d_const_stage = nullptr;
 
   int occ = 0;
-  for (int aux = 0; aux < 4; ++aux) {        // evaluation (plain, generic), difference image, constant-bank variant
-    const void* k = kernel_for(cfg->m, aux == 1 || aux == 2, aux == 2, aux == 3);
+  for (int aux = 0; aux < 5; ++aux) {        // evaluation (plain, generic), difference image, constant-bank variants
+    const void* k = kernel_for(cfg->m, aux == 1 || aux == 2 || aux == 4, aux == 2, aux >= 3);
     ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem);
     if (ce != cudaSuccess) { int rc = cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)"); delete h; return rc; }
     int o = 0;
@@ -633,6 +634,14 @@ extern "C" int dia_measure_fp32_peak(void* stream, double* fma_per_second) {
   if (!fma_per_second) return DIA_ERR_INVALID_ARG;
   const double v = dia::measure_fp32_peak((cudaStream_t)stream, 5);
   if (v <= 0.0) { cudaGetLastError(); return fail(nullptr, DIA_ERR_CUDA, "FP32 peak probe failed (no CUDA device?)"); }
+  *fma_per_second = v;
+  return DIA_OK;
+}
+
+extern "C" int dia_measure_fp32_pattern(void* stream, int pattern, double* fma_per_second) {
+  if (!fma_per_second || pattern < 0 || pattern >= dia::kProbePatterns) return DIA_ERR_INVALID_ARG;
+  const double v = dia::measure_fp32_pattern((cudaStream_t)stream, pattern, 5);
+  if (v <= 0.0) { cudaGetLastError(); return fail(nullptr, DIA_ERR_CUDA, "FP32 probe failed (no CUDA device?)"); }
   *fma_per_second = v;
   return DIA_OK;
 }

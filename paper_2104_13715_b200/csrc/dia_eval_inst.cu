@@ -1,6 +1,6 @@
 // dia_eval_inst.cu -- one translation unit per kernel size: compiled once for every odd m with
 // -DDIA_INST_M=<m> (paper_2104_13715_b200/build.py runs these compilations in parallel).  Each unit holds the
-// four instantiations of the fused kernel for its m and its own copy of the constant block, and exports two
+// five instantiations of the fused kernel for its m and its own copy of the constant block, and exports two
 // accessors that dia_api.cu uses to launch the kernels and to address the constant symbol.
 #include "dia_eval.cuh"
 
@@ -14,7 +14,8 @@
 namespace dia {
 
 // variant: 0 = plain objective, 1 = generic (mask / flat / variance map), 2 = difference image,
-//          3 = plain objective with the kernel pixels in the constant bank, 4 = kernel-kernel block of the Hessian
+//          3 = plain objective with the kernel pixels in the constant bank, 4 = kernel-kernel block of the Hessian,
+//          5 = generic with the kernel pixels in the constant bank
 const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
   switch (variant) {
     case 0: return (const void*)eval_kernel<DIA_INST_M, false, false, false>;
@@ -22,6 +23,7 @@ const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
     case 2: return (const void*)eval_kernel<DIA_INST_M, true, true, false>;
     case 3: return (const void*)eval_kernel<DIA_INST_M, false, false, true>;
     case 4: return (const void*)hess_block_kernel<DIA_INST_M>;
+    case 5: return (const void*)eval_kernel<DIA_INST_M, true, false, true>;
   }
   return nullptr;
 }

@@ -28,7 +28,7 @@ cudaError_t launch_eval(const dia_handle* h, const EvalParams& p, const TensorMa
 const void* eval_kernel_ptr(const dia_handle* h, bool aux);
 bool eval_uses_const(const dia_handle* h, const EvalParams& p, bool diff);
 size_t const_block_bytes(const dia_handle* h, int n_epochs);
-const void* eval_kernel_ptr_kc(const dia_handle* h);
+const void* eval_kernel_ptr_kc(const dia_handle* h, const EvalParams& p);
 ConstBlock* const_stage(const dia_handle* h);
 const void* const_symbol(const dia_handle* h);
 size_t eval_smem_bytes(const dia_handle* h);
@@ -507,7 +507,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     void* eval_args[] = {(void*)&pe, (void*)&tme};
     cudaKernelNodeParams ke = {};
     const bool kc = eval_uses_const(h, p, false);
-    ke.func = kc ? (void*)eval_kernel_ptr_kc(h) : (void*)eval_kernel_ptr_p(h, p);
+    ke.func = kc ? (void*)eval_kernel_ptr_kc(h, p) : (void*)eval_kernel_ptr_p(h, p);
     ke.gridDim = dim3(grid); ke.blockDim = dim3(eval_threads_p(h, p));
     ke.sharedMemBytes = (unsigned)eval_smem_bytes_p(h, p); ke.kernelParams = eval_args; ke.extra = nullptr;
     StepArgs sa;

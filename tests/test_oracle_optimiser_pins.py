@@ -207,3 +207,49 @@ def test_switch_rule_strict_less_and_previous_loss_denominator():
     # the recorded relative changes do fall through the paper's 1e-6 on this problem only much later: the tests above
     # are about the comparison, not about that value
     assert min(rel) < max(rel)
+
+
+# ------------------------------------------------------------------------------------------ what is NOT pinned, and why
+_SELF_CHECK = """
+import json, sys
+import numpy as np
+import oracle
+from workloads import make_workload
+w = make_workload(1, n=160, m=9)
+cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
+th, r = oracle.fit(cfg, w.R, w.I, w.theta0)
+print(json.dumps(dict(threads=oracle.num_threads(), n_adam=r[0].n_adam, n_lbfgs=r[0].n_lbfgs, status=r[0].status,
+                      P=r[0].photometric_scale, loss=r[0].loss, theta=th[0].astype(float).tolist())))
+"""
+
+
+def test_stopped_iterate_depends_on_summation_order():
+    """Why the stopped iterate of a free-running fit is "parity unpinned": the oracle itself does
+    not reproduce it.  The same fit (config 1 at 160^2, 9x9 kernel, paper settings) with 3 and with 4 OpenMP threads --
+    two orders of the same FP64 sums, 1e-16 apart -- stops after different numbers of L-BFGS iterations and its
+    kernels differ by far more than north_star's 1e-4, while the photometric scale and the loss (what the data
+    determine) agree.  No implementation, in any precision, can match such an iterate to 1e-4; the fit-parity
+    protocol therefore asserts lock-step and well-conditioned (converged / regularised) fits strictly and the
+    stopped iterate through the model image."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    runs = []
+    for threads in (3, 4):
+        env = dict(os.environ, OMP_NUM_THREADS=str(threads), PYTHONPATH=root)
+        out = subprocess.run([sys.executable, "-c", _SELF_CHECK], env=env, cwd=root, capture_output=True, text=True, check=True)
+        runs.append(json.loads(out.stdout.strip().splitlines()[-1]))
+    a, b = runs
+    assert (a["threads"], b["threads"]) == (3, 4)
+    assert a["status"] in (0, 1) and b["status"] in (0, 1)
+    assert a["n_adam"] == b["n_adam"]                       # the Adam phase is robust at this horizon ...
+    Ka, Kb = np.array(a["theta"][:-1]), np.array(b["theta"][:-1])
+    dK = np.abs(Ka - Kb).max() / np.abs(Ka).max()
+    dP = abs(a["P"] - b["P"]) / abs(a["P"])
+    dL = abs(a["loss"] - b["loss"]) / abs(a["loss"])
+    print(f"oracle vs oracle (3 / 4 threads): lbfgs {a['n_lbfgs']} / {b['n_lbfgs']}, dK={dK:.2e} dP={dP:.2e} dL={dL:.2e}")
+    assert a["n_lbfgs"] != b["n_lbfgs"]                     # ... the stop rule fires at different L-BFGS iterations
+    assert dK > 10 * 1e-4                                   # the kernels differ by far more than the parity tolerance
+    assert dP <= 1e-4 and dL <= 1e-4                        # the scale factor and the loss do not

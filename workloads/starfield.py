@@ -266,22 +266,30 @@ def gaussian_kernel_init(m: int, phi_k: float, b0: float) -> np.ndarray:
 
 def make_workload(c: int, n: Optional[int] = None, n_epochs: Optional[int] = None,
                   m: Optional[int] = None, noise: bool = True, ref_noise: bool = False,
-                  epochs: Optional[Sequence[int]] = None) -> Workload:
+                  epochs: Optional[Sequence[int]] = None, sky_subtract: bool = False) -> Workload:
     """Config `c` of BASELINE.json; n / n_epochs / m may be reduced for tests
     (same recipe, same stellar density, same RNG streams).  `epochs` selects target epochs by index (default
     0 .. n_epochs-1).  `ref_noise`: the targets are simulated from the noiseless reference as
     always, and the reference handed to the fit carries the paper's S10 noise (Eq. 22-23) -- the situation of
-    every image pair of the paper; BASELINE.json's configs are the ref_noise = False case."""
+    every image pair of the paper; BASELINE.json's configs are the ref_noise = False case.  `sky_subtract`: the
+    reference handed to the fit has its sky level removed ("we always background subtract the reference image",
+    PAPER.md:240) -- the targets are unchanged, so the planted B0 becomes B0 + P sky in theta_true; BASELINE.json's
+    configs leave the sky in (sky_subtract = False)."""
     cfg = CONFIGS[c]
     n = cfg.n if n is None else n
     m = cfg.m if m is None else m
     E = cfg.n_epochs if n_epochs is None else n_epochs
     R_true = make_reference(cfg, n)
     R = add_reference_noise(cfg, R_true) if ref_noise else R_true
+    if sky_subtract:
+        R = (R.astype(np.float64) - cfg.sky).astype(np.float32)
     Is, thetas, masks, theta0s = [], [], [], []
     flat = None
     for e in (range(E) if epochs is None else epochs):
         I, th, fl, mk = make_target(cfg, e, R_true, m, noise)
+        if sky_subtract:
+            th = th.copy()
+            th[-1] += th[:-1].sum() * cfg.sky
         Is.append(I)
         thetas.append(th)
         theta0s.append(theta_init(R, I, m))
