@@ -6,6 +6,7 @@ CUDA tensors.  PyTorch is used for device memory and streams only.
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 import os
 from typing import Optional
@@ -24,6 +25,9 @@ EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", 
 
 class DiaError(RuntimeError):
     pass
+
+
+_NO_CTX = contextlib.nullcontext()
 
 
 class _Config(C.Structure):
@@ -299,11 +303,15 @@ class Handle:
             self._hgrad = torch.empty((E, self.np), dtype=torch.float64).pin_memory()
 
     def _stream_ctx(self):
-        """Context in which torch's current stream is the handle's stream.  A handle with its own stream first makes
-        that stream wait for the caller's current stream, so inputs produced there are complete."""
+        """Context in which torch's current stream is the handle's stream.  A handle without a stream of its own
+        runs on the legacy default stream like torch's default: nothing to switch (and no per-call cost -- a stream
+        context costs several microseconds of host time, as much as a small evaluation).  A handle with its own
+        stream first makes that stream wait for the caller's current stream, so inputs produced there are complete."""
+        if self.stream is None:
+            return _NO_CTX
         cur = torch.cuda.current_stream(self.R.device)
-        if self.stream is None or self.stream == cur:
-            return torch.cuda.stream(cur)
+        if self.stream == cur:
+            return _NO_CTX
         self.stream.wait_stream(cur)
         return torch.cuda.stream(self.stream)
 

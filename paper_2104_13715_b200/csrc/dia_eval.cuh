@@ -196,13 +196,13 @@ __device__ __forceinline__ f32x2 pk2(float lo, float hi) {
   return r;
 }
 __device__ __forceinline__ float pk_lo(f32x2 v) {
-  float lo, hi;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  float lo;
+  asm("{\n.reg .b32 t;\nmov.b64 {%0, t}, %1;\n}" : "=f"(lo) : "l"(v));
   return lo;
 }
 __device__ __forceinline__ float pk_hi(f32x2 v) {
-  float lo, hi;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  float hi;
+  asm("{\n.reg .b32 t;\nmov.b64 {t, %0}, %1;\n}" : "=f"(hi) : "l"(v));
   return hi;
 }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {      // {a.lo b.lo + c.lo, a.hi b.hi + c.hi}
