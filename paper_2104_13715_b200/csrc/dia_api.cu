@@ -15,6 +15,7 @@
 #include "dia_eval.cuh"
 #include "dia_eval_small.cuh"
 #include "dia_fit.cuh"
+#include "dia_fit_cluster.cuh"
 #include "dia_hess.cuh"
 #include "dia_cov.cuh"
 #include "dia_probe.cuh"
@@ -27,6 +28,8 @@ struct dia_handle {
   int tiles, n_refs;
   int small_grid;          // > 0: the plain objective of this handle (m <= 5) runs eval_small_kernel on at most this many CTAs
   int grid_limit;          // test hook DIA_GRID_LIMIT (0 = none)
+  int cluster_fit;         // 1: dia_fit may run small image pairs in fit_cluster_kernel (0: test hook DIA_DISABLE_CLUSTER, or
+                           // the kernel does not fit); -1: not decided yet
   int flush_tiles;         // tiles between two FP64 folds of the FP32 gradient strips (kFlushTiles; test hook DIA_FLUSH_TILES)
   dia::ConstBlock* d_const_stage;   // staging copy of the constant block; non-null iff this handle may use the bank
   size_t smem;
@@ -116,7 +119,7 @@ static void geometry_for(int m, int* rpitch, int* rh) {
 // The kernel instantiations live in one translation unit per m (dia_eval_inst.cu); each exports its kernels and
 // the host shadow of its own constant block.
 namespace dia {
-#define X(MM) const void* eval_kernel_ptr_m##MM(int variant); const void* const_symbol_m##MM();
+#define X(MM) const void* eval_kernel_ptr_m##MM(int variant); const void* const_symbol_m##MM(); size_t cluster_smem_m##MM();
 DIA_FOR_EACH_M(X)
 #undef X
 }  // namespace dia
@@ -139,6 +142,22 @@ static const void* hess_kernel_for(int m) {
 #undef X
   }
   return nullptr;
+}
+static const void* cluster_kernel_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::eval_kernel_ptr_m##MM(6);
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return nullptr;
+}
+static size_t cluster_smem_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::cluster_smem_m##MM();
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return 0;
 }
 static const void* const_symbol_for(int m) {
   switch (m) {
@@ -401,6 +420,8 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
     if (g >= 1) h->grid_limit = g;
     if (g >= 1 && g < h->grid) h->grid = g;
   }
+  h->cluster_fit = -1;
+  if (const char* nc = std::getenv("DIA_DISABLE_CLUSTER")) { if (nc[0] == '1') h->cluster_fit = 0; }   // test hook: graph loop
   h->flush_tiles = dia::kFlushTiles;
   if (const char* ft = std::getenv("DIA_FLUSH_TILES")) {   // test hook: how often the FP32 strips are folded
     const int f = std::atoi(ft);
@@ -622,6 +643,44 @@ extern "C" int dia_fit(dia_handle* h, const dia_fit_opts* opts, int n_epochs, co
   dia::EvalParams p;
   dia::TensorMaps tm;
   fill_params(h, n_epochs, d_I, d_mask, d_var, h->fit.d_theta32, h->fit.d_done, &p, &tm);
+  // Small image pairs, plain objective: the whole fit inside one kernel, one cluster of `tiles` CTAs per epoch
+  // (dia_fit_cluster.cuh).  Chosen when every cluster is resident at once, or for free-running fits of larger
+  // batches: there each cluster leaves when its own fit has stopped and the next pair starts (measured, 296 stamps
+  // of 142^2, m = 19: 2.1 s against 4.0 s for the graph loop, which iterates until the slowest pair is done), while
+  // in lock-step -- every pair takes the same number of steps -- the graph loop's batched evaluations are faster
+  // (19 ms against 29 ms for 121 iterations).  Otherwise the graph loop below.
+  const bool lockstep = opts->force_adam_iters >= 0 || opts->force_lbfgs_iters >= 0;
+  if (h->cluster_fit != 0 && h->tiles <= dia::kMaxClusterTiles && !dia::eval_is_aux(p) && h->cfg.bg_degree == 0 &&
+      (!lockstep || (long long)n_epochs * h->tiles <= (long long)h->sms * 2)) {
+    const void* kf = cluster_kernel_for(h->cfg.m);
+    const size_t smem = cluster_smem_for(h->cfg.m);
+    if (h->cluster_fit < 0) {
+      int o = 0;
+      cudaError_t ce = cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (ce == cudaSuccess) ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kf, dia::kThreads, smem);
+      h->cluster_fit = (ce == cudaSuccess && o >= 1) ? 1 : 0;
+      if (ce != cudaSuccess) cudaGetLastError();
+    }
+    if (h->cluster_fit == 1) {
+      dia::fit_init_kernel<<<n_epochs, 256, 0, h->stream>>>(h->fit.b, d_theta, h->np, n_epochs);
+      dia::StepArgs sa;
+      sa.b = h->fit.b;  sa.partials = h->d_partials;  sa.n_blocks = h->tiles;  sa.np = h->np;  sa.hist_cap = h->fit.hist_cap;
+      sa.o = *opts;  sa.theta_out = d_theta;  sa.result = d_result;  sa.cond = 0;  sa.m = h->cfg.m;  sa.lamN = lambda_n(h);
+      sa.use_graph = 0;
+      p.epoch_per_cta = 0;  p.small_rpt = 0;
+      cudaLaunchConfig_t lc = {};
+      lc.gridDim = dim3((unsigned)(n_epochs * h->tiles));  lc.blockDim = dim3(dia::kThreads);
+      lc.dynamicSmemBytes = smem;  lc.stream = h->stream;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = (unsigned)h->tiles;  at[0].val.clusterDim.y = 1;  at[0].val.clusterDim.z = 1;
+      lc.attrs = at;  lc.numAttrs = 1;
+      void* args[] = {(void*)&p, (void*)&tm, (void*)&sa};
+      cudaError_t ce = cudaLaunchKernelExC(&lc, kf, args);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "cluster fit launch");
+      return DIA_OK;
+    }
+  }
   std::string err;
   const int unroll = 4;        // (eval ; step) pairs per WHILE iteration: 8 % faster on 128^2 images than 1
   rc = dia::fit_run(&h->fit, h, p, tm, *opts, n_epochs, d_theta, d_result, dia::eval_grid_p(h, p),

@@ -3,6 +3,7 @@
 // five instantiations of the fused kernel for its m and its own copy of the constant block, and exports two
 // accessors that dia_api.cu uses to launch the kernels and to address the constant symbol.
 #include "dia_eval.cuh"
+#include "dia_fit_cluster.cuh"
 
 #ifndef DIA_INST_M
 #error "compile with -DDIA_INST_M=<odd kernel size>"
@@ -15,7 +16,7 @@ namespace dia {
 
 // variant: 0 = plain objective, 1 = generic (mask / flat / variance map), 2 = difference image,
 //          3 = plain objective with the kernel pixels in the constant bank, 4 = kernel-kernel block of the Hessian,
-//          5 = generic with the kernel pixels in the constant bank
+//          5 = generic with the kernel pixels in the constant bank, 6 = whole fit of a small image in one cluster
 const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
   switch (variant) {
     case 0: return (const void*)eval_kernel<DIA_INST_M, false, false, false>;
@@ -24,9 +25,13 @@ const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
     case 3: return (const void*)eval_kernel<DIA_INST_M, false, false, true>;
     case 4: return (const void*)hess_block_kernel<DIA_INST_M>;
     case 5: return (const void*)eval_kernel<DIA_INST_M, true, false, true>;
+    case 6: return (const void*)fit_cluster_kernel<DIA_INST_M>;
   }
   return nullptr;
 }
+
+// dynamic shared memory of fit_cluster_kernel
+size_t DIA_CAT(cluster_smem_m, DIA_INST_M)() { return ClusterGeo<DIA_INST_M>::SMEM; }
 
 // host shadow of this unit's constant block (what cudaMemcpyToSymbol / graph memcpy nodes take)
 const void* DIA_CAT(const_symbol_m, DIA_INST_M)() { return (const void*)&c_blk; }

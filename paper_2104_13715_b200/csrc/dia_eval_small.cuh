@@ -107,12 +107,6 @@ struct SmallGeo {
   static constexpr int MAXREG = M == 1 ? 80 : (M == 3 ? 128 : 255);
 };
 
-__device__ __forceinline__ float lg2_approx(float x) {      // v is a variance: never subnormal, so no rescaling step
-  float y;
-  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
 // Per-pixel terms of the plain objective (D1; the formulas of pixel_terms<false, .> in
 // dia_eval.cuh) with the loss a template parameter and ln v from the MUFU unit (lg2.approx, absolute error 2^-22 in
 // log2 v: 1e-7 on a term of size 2-6).  hg = inv_gain / 2.

@@ -88,7 +88,19 @@ struct StepArgs {
   cudaGraphConditionalHandle cond;
   int m;                     // kernel size
   double lamN;               // lambda * N_data of Eq. 20, 0 = no penalty
+  int use_graph;             // 1: the last epoch to stop clears the WHILE condition `cond` of the fit graph
 };
+
+// Shared-memory scratch of one optimiser transition (fit_step_body): the step kernel declares it statically, the
+// cluster kernel (dia_fit_cluster.cuh) carves it out of its dynamic shared memory.
+struct StepScratch {
+  double (*sh_rows)[kFitThreads / 32];   // [2][8]   block reductions
+  double* s_alpha;                       // [kMaxHistory]
+  double* gsum;                          // [kFitThreads * PER]
+  double* xs;                            // [kFitThreads * PER]  (penalty only)
+};
+template <int PER>
+constexpr size_t step_scratch_bytes() { return 8 * (2 * (kFitThreads / 32) + kMaxHistory + 2 * kFitThreads * PER); }
 
 // ---------------------------------------------------------------- block-wide FP64 reductions
 // One barrier per reduction: two scratch rows are used alternately (`par` toggles on every call, and every
@@ -134,6 +146,7 @@ __device__ __forceinline__ double laplacian_row(const double* __restrict__ x, in
   return nadj * x[k] - s;
 }
 
+#ifndef DIA_INST_M      // the stand-alone kernels and the host side belong to the API translation unit only
 // Eq. 20: adds lamN |L theta|^2 to loss[e] and 2 lamN L (L theta) to grad[e][0..m*m) for the
 // stand-alone evaluation path (one CTA per epoch, launched after reduce_partials_kernel).
 __global__ void __launch_bounds__(kFitThreads) penalty_kernel(const float* __restrict__ theta, int m, int np, double lamN,
@@ -171,14 +184,13 @@ __global__ void fit_init_kernel(FitBuffers b, const float* __restrict__ theta_in
   }
 }
 
-// One optimiser transition for epoch blockIdx.x, run after every evaluation.
+#endif  // DIA_INST_M
+
+// One optimiser transition for epoch e, run by one CTA of kFitThreads threads after every evaluation of that epoch.
 template <int PER>
-__global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a) {
-  const int e = blockIdx.x;
-  if (a.b.done[e]) return;
-  __shared__ double sh_rows[2][kFitThreads / 32];
-  BlockRed sh{sh_rows, 0};
-  __shared__ double s_alpha[kMaxHistory];
+__device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, const StepScratch& sc) {
+  BlockRed sh{sc.sh_rows, 0};
+  double* const s_alpha = sc.s_alpha;
   const int np = a.np, nk = a.m * a.m, tid = threadIdx.x;   // nk kernel pixels, np - nk background coefficients
   const dia_fit_opts& o = a.o;
   FitState st = a.b.st[e];                       // every thread holds a private copy; thread 0 writes back
@@ -194,7 +206,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
   const int hist = o.lbfgs_history;
 
   // ---- second-level reduction of the evaluation's block partials: one warp per output, fixed order
-  __shared__ double gsum[kFitThreads * PER];
+  double* const gsum = sc.gsum;
   double gn[PER];
   double Ln = 0.0;
   {
@@ -206,7 +218,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
       for (int b = lane; b < a.n_blocks; b += 32) {
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-          if (k + j < np + 1) s4[j] += src[(size_t)(k + j) * a.n_blocks + b];
+          if (k + j < np + 1) s4[j] += __ldcg(src + (size_t)(k + j) * a.n_blocks + b);   // written by other SMs: L2
       }
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -224,7 +236,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
     __syncthreads();
   }
   if (a.lamN > 0.0) {                            // Eq. 20 penalty at the evaluation point (uniform branch)
-    __shared__ double xs[kFitThreads * PER];
+    double* const xs = sc.xs;
     double* const us = gsum;                     // gsum is dead: gn / Ln hold its content (keeps static shared memory < 48 KB)
     for (int k = tid; k < nk; k += kFitThreads) xs[k] = (double)th32[k];
     __syncthreads();
@@ -426,10 +438,23 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
       a.result[e] = r;
       a.b.done[e] = 1;
       __threadfence();
-      if (atomicSub(a.b.remaining, 1) == 1) cudaGraphSetConditional(a.cond, 0);
+      if (atomicSub(a.b.remaining, 1) == 1 && a.use_graph) cudaGraphSetConditional(a.cond, 0);
     }
   }
   if (tid == 0) a.b.st[e] = st;
+}
+
+#ifndef DIA_INST_M
+template <int PER>
+__global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a) {
+  const int e = blockIdx.x;
+  if (a.b.done[e]) return;
+  __shared__ double sh_rows[2][kFitThreads / 32];
+  __shared__ double s_alpha[kMaxHistory];
+  __shared__ double gsum[kFitThreads * PER];
+  __shared__ double xs[kFitThreads * PER];
+  const StepScratch sc{sh_rows, s_alpha, gsum, xs};
+  fit_step_body<PER>(a, e, sc);
 }
 
 // ---------------------------------------------------------------- host side
@@ -513,7 +538,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
     StepArgs sa;
     sa.b = w->b; sa.partials = p.partials; sa.n_blocks = part_cols; sa.np = w->np; sa.hist_cap = w->hist_cap;
     sa.o = o; sa.theta_out = d_theta; sa.result = d_result; sa.cond = cond;
-    sa.m = m; sa.lamN = lamN;
+    sa.m = m; sa.lamN = lamN; sa.use_graph = 1;
     void* step_args[] = {(void*)&sa};
     cudaKernelNodeParams ks = {};
     ks.func = w->np <= kFitThreads * kPerThreadSmall ? (void*)fit_step_kernel<kPerThreadSmall>
@@ -553,5 +578,7 @@ inline int fit_run(FitWorkspace* w, const dia_handle* h, const EvalParams& p, co
   DIA_CU(cudaGraphLaunch(slot->exec, stream));
   return DIA_OK;
 }
+
+#endif  // DIA_INST_M
 
 }  // namespace dia

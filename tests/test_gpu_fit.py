@@ -191,16 +191,22 @@ def test_fit_many_small_pairs(dia):
 
 
 def test_fit_with_laplacian_regularisation(dia):
-    """Eq. 20 inside dia_fit.  The penalty lifts the flat directions of K, so even the free-running
-    fit under the paper's stop rule is now well determined; lock-step first (strict), then free-running."""
-    w = make_workload(0)
+    """Eq. 20 inside dia_fit: lock-step against the oracle (strict), then free-running under the paper's
+    stop rule.  The penalty lifts the flat directions of K; it does not touch the scale-background valley (a constant
+    kernel offset against B0: L 1 = 0), so the free-running part uses the background-subtracted reference of the
+    paper's practice, where B0 is well determined too -- then the stopped iterate itself meets the strict
+    criterion (with the sky left in the reference dB0 hovers around 1e-4: tests/test_gpu_fit_protocol.py)."""
     lam = 10.0
+    w = make_workload(0)
     cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
     h = dia.Handle(_dev(w.R), w.m, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
     og, oo = _both_opts(dia, force_adam_iters=30, force_lbfgs_iters=10)
     tho, ro = oracle.fit(cfg, w.R, w.I, w.theta0, oo)
     thg, rg = h.fit(_dev(w.I), _dev(w.theta0), og)
     _assert_fit_close(tho, ro, thg.cpu().numpy(), rg, "lambda lockstep")
+    h.close()
+    w = make_workload(0, sky_subtract=True)
+    h = dia.Handle(_dev(w.R), w.m, sigma0=w.sigma0, gain=w.gain, lambda_reg=lam)
     og, oo = _both_opts(dia)
     tho, ro = oracle.fit(cfg, w.R, w.I, w.theta0, oo)
     thg, rg = h.fit(_dev(w.I), _dev(w.theta0), og)
@@ -338,3 +344,29 @@ def test_fit_lockstep_large_kernels(dia, m, lam):
     h.close()
     assert [r.n_evals for r in rg] == [r.n_evals for r in ro]
     _assert_fit_close(tho, ro, thg.cpu().numpy(), rg, f"lockstep m={m} lambda={lam}")
+
+
+@pytest.mark.parametrize("c,n,m,E", [(0, None, None, 1), (0, 100, 5, 3), (4, 142, 19, 5), (1, 190, 9, 2)])
+def test_fit_cluster_kernel_matches_graph_loop(dia, monkeypatch, c, n, m, E):
+    """Small image pairs with the plain objective are fitted inside one kernel, one thread-block cluster per epoch
+    (csrc/dia_fit_cluster.cuh: tiles resident in shared memory, cluster barriers instead of launches).  Same device
+    functions, same orders: for image pairs whose tiles sit on different CTAs in the graph loop the fitted parameters,
+    iteration counts and losses must be bit-identical to it (test hook DIA_DISABLE_CLUSTER=1), free-running and in
+    lock-step; (190^2: 3 x 3 = 9 tiles exceed the portable cluster size and take the graph loop on both sides)."""
+    w = make_workload(c, n=n, m=m, n_epochs=E)
+    outs = []
+    for disable in ("0", "1"):
+        monkeypatch.setenv("DIA_DISABLE_CLUSTER", disable)
+        h = dia.Handle(_dev(w.R), w.m, max_epochs=E, sigma0=w.sigma0, gain=w.gain)
+        res = []
+        for og in (dia.FitOpts.default(max_adam_iters=2500, max_lbfgs_iters=60),
+                   dia.FitOpts.default(force_adam_iters=25, force_lbfgs_iters=7, lbfgs_backtrack=1)):
+            th, r = h.fit(_dev(w.I), _dev(w.theta0), og)
+            res.append((th.cpu().numpy(), [(x.n_adam, x.n_lbfgs, x.n_evals, x.status, x.loss, x.grad_inf_norm,
+                                            x.photometric_scale) for x in r]))
+        h.close()
+        outs.append(res)
+    for (tha, ra), (thb, rb) in zip(*outs):
+        assert ra == rb
+        assert np.array_equal(tha, thb)
+    assert outs[0][0][1][0][2] > 30          # the free-running fit did iterate
