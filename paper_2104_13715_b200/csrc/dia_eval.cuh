@@ -688,6 +688,35 @@ __device__ __forceinline__ void grad_chunk(GradAcc<M>& A, const float* __restric
   }
 }
 
+// FP64 fold of the thread-private FP32 gradient strips over the S pixel sub-sets: put(o, sum) for every kernel pixel
+// o = a M + b, fixed order.  Called by all threads of the CTA (between barriers).  Small kernels have many sub-sets
+// (S = 256 / M: 36 at m = 7, 85 at m = 3), so there four lanes share an output: quarter sums, then (q0 + q1) + (q2 + q3).
+template <int M, typename F>
+__device__ __forceinline__ void fold_strips(const float* __restrict__ accS, int tid, F&& put) {
+  using G = Geo<M>;
+  if (M * M * 4 <= kThreads) {
+    const int o = tid >> 2, part = tid & 3;
+    const bool live = o < M * M;
+    const int a = live ? o / M : 0, b = live ? o - a * M : 0;
+    constexpr int CH = (G::S + 3) / 4;
+    const int s1 = min((part + 1) * CH, G::S);
+    double s = 0.0;
+#pragma unroll 1
+    for (int ss = part * CH; ss < s1; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
+    s += __shfl_xor_sync(0xffffffffu, s, 1);
+    s += __shfl_xor_sync(0xffffffffu, s, 2);
+    if (live && part == 0) put(o, s);
+  } else {
+    for (int o = tid; o < M * M; o += kThreads) {
+      const int a = o / M, b = o - a * M;
+      double s = 0.0;
+#pragma unroll 1
+      for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
+      put(o, s);
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // the fused kernel
 // ------------------------------------------------------------------------------------------------
@@ -768,13 +797,7 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) eval_kernel(const Eval
   // fold the FP32 strips of all pixel sub-sets into this CTA's FP64 partials, fixed order
   auto flush = [&]() {
     __syncthreads();
-    for (int o = tid; o < M * M; o += kThreads) {
-      const int a = o / M, b = o - a * M;
-      double s = 0.0;
-#pragma unroll 1
-      for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + a) * G::KP + b];
-      out[(size_t)o * ncols] = flushed ? out[(size_t)o * ncols] + s : s;
-    }
+    fold_strips<M>(accS, tid, [&](int o, double s) { out[(size_t)o * ncols] = flushed ? out[(size_t)o * ncols] + s : s; });
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);

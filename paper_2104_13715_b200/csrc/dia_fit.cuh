@@ -98,6 +98,12 @@ struct StepScratch {
   double* s_alpha;                       // [kMaxHistory]
   double* gsum;                          // [kFitThreads * PER]
   double* xs;                            // [kFitThreads * PER]  (penalty only)
+  // cluster loop only (null in the graph loop): the partial column of every CTA of the epoch in that CTA's shared
+  // memory (distributed shared memory) instead of the global partials; a shared-memory copy of the next evaluation
+  // point and of the done flag, which the caller hands to the other CTAs of the cluster
+  const double* const* peer_cols;        // [n_blocks] -> double [np + 1]
+  float* th_local;                       // [np]
+  int* done_local;                       // [1]
 };
 template <int PER>
 constexpr size_t step_scratch_bytes() { return 8 * (2 * (kFitThreads / 32) + kMaxHistory + 2 * kFitThreads * PER); }
@@ -218,7 +224,7 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
       for (int b = lane; b < a.n_blocks; b += 32) {
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-          if (k + j < np + 1) s4[j] += __ldcg(src + (size_t)(k + j) * a.n_blocks + b);   // written by other SMs: L2
+          if (k + j < np + 1) s4[j] += sc.peer_cols ? sc.peer_cols[b][k + j] : src[(size_t)(k + j) * a.n_blocks + b];
       }
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -280,6 +286,7 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
             const double th = theta[k] - lr * mh / (sqrt(vh) + o.adam_eps);
             theta[k] = th;
             th32[k] = (float)th;
+            if (sc.th_local) sc.th_local[k] = (float)th;
           }
         }
         st.n_adam += 1; st.Lprev = Ln; st.t = t; st.L = Ln;
@@ -303,7 +310,10 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
 #pragma unroll
       for (int q = 0; q < PER; ++q) {
         const int k = tid + q * kFitThreads;
-        if (k < np) th32[k] = (float)(theta[k] + st.alpha * dvec[k]);
+        if (k < np) {
+          th32[k] = (float)(theta[k] + st.alpha * dvec[k]);
+          if (sc.th_local) sc.th_local[k] = th32[k];
+        }
       }
     } else if (bad) {
       st.status = DIA_FIT_NONFINITE; finished = true;
@@ -411,7 +421,10 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
 #pragma unroll
       for (int q = 0; q < PER; ++q) {
         const int k = tid + q * kFitThreads;
-        if (k < np) { dvec[k] = q4[q]; th32[k] = (float)(theta[k] + alpha * q4[q]); }
+        if (k < np) {
+          dvec[k] = q4[q]; th32[k] = (float)(theta[k] + alpha * q4[q]);
+          if (sc.th_local) sc.th_local[k] = th32[k];
+        }
       }
     }
   }
@@ -437,6 +450,7 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
       r.n_adam = st.n_adam; r.n_lbfgs = st.n_lbfgs; r.n_evals = st.n_evals; r.status = st.status;
       a.result[e] = r;
       a.b.done[e] = 1;
+      if (sc.done_local) *sc.done_local = 1;
       __threadfence();
       if (atomicSub(a.b.remaining, 1) == 1 && a.use_graph) cudaGraphSetConditional(a.cond, 0);
     }
@@ -453,7 +467,7 @@ __global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a)
   __shared__ double s_alpha[kMaxHistory];
   __shared__ double gsum[kFitThreads * PER];
   __shared__ double xs[kFitThreads * PER];
-  const StepScratch sc{sh_rows, s_alpha, gsum, xs};
+  const StepScratch sc{sh_rows, s_alpha, gsum, xs, nullptr, nullptr, nullptr};
   fit_step_body<PER>(a, e, sc);
 }
 

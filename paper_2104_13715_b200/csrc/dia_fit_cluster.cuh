@@ -4,15 +4,20 @@
 // arithmetic, and the graph loop of dia_fit.cuh spends ~13 us per iteration on two kernel launches, tile staging and
 // reduction latency.  Here a cluster of T = tiles CTAs (T <= 8) owns one epoch for the whole fit:
 //   once       every CTA stages ITS tile of R (+ halo) and of I into shared memory (TMA or cp.async) and keeps them;
-//   iteration  K and B0 from theta32 -> forward stencil, residual, noise model, loss, weights -> gradient correlation
-//              (the device functions of eval_kernel, same arithmetic, same orders) -> this CTA's FP64 partial column
-//              -> cluster barrier -> rank 0 runs the optimiser transition (fit_step_body: second-level reduction, Adam
-//              or L-BFGS step, stop tests) -> cluster barrier -> next iteration, until the epoch's done flag is set.
-// No host round trip, no launch, no re-staging per iteration.  Epochs are independent clusters, so a batch of hundreds
+//   iteration  K and B0 from this CTA's shared-memory copy of theta -> forward stencil, residual, noise model, loss,
+//              weights -> gradient correlation (the device functions of eval_kernel, same arithmetic, same orders) ->
+//              this CTA's FP64 partial column, in ITS shared memory -> cluster barrier -> rank 0 runs the optimiser
+//              transition (fit_step_body: second-level reduction reading the columns of all CTAs through distributed
+//              shared memory, Adam or L-BFGS step, stop tests) and stores the next evaluation point and the done
+//              flag into every CTA's shared memory -> cluster barrier -> next iteration, until done.
+// No host round trip, no launch, no re-staging and no global-memory hand-over per iteration (the optimiser state --
+// FP64 theta, moments, L-BFGS history -- stays in global memory and is touched by rank 0 only).  Epochs are independent clusters, so a batch of hundreds
 // of stamps is one launch; clusters that finish make room for the next.  Plain objective only (no mask / flat /
 // variance map / background polynomial): dia_fit falls back to the graph loop otherwise.  For an image whose tiles
 // all sit on different CTAs in the graph loop (single image pairs) the results are bit-identical to it (tested).
 #pragma once
+#include <cooperative_groups.h>
+
 #include "dia_fit.cuh"
 
 namespace dia {
@@ -33,11 +38,22 @@ template <int M>
 struct ClusterGeo {
   using G = Geo<M>;
   static constexpr int PER = (M * M + 1 <= kFitThreads * kPerThreadSmall) ? kPerThreadSmall : kPerThreadLarge;
-  static constexpr size_t SCRATCH = step_scratch_bytes<PER>();
-  // the optimiser's scratch takes the second R buffer when there is one and it is large enough, else it is appended
-  static constexpr bool IN_RBUF = G::NRBUF == 2 && (size_t)G::R_STRIDE >= SCRATCH;
+  static constexpr int NP = M * M + 1;
+  // the optimiser's scratch, then the exchange area: this CTA's partial column [np + 1] doubles, theta [np] floats, the
+  // table of peer columns, the done flag
+  static constexpr size_t SCRATCH = (step_scratch_bytes<PER>() + 15) / 16 * 16;
+  static constexpr size_t X_PCOL = SCRATCH;
+  static constexpr size_t X_TH = X_PCOL + 8 * (NP + 1);
+  static constexpr size_t X_PEERS = (X_TH + 4 * NP + 15) / 16 * 16;
+  static constexpr size_t X_DONE = X_PEERS + 8 * 16;
+  static constexpr size_t EXTRA = X_DONE + 16;
+  // both take the second R buffer when there is one and it is large enough (m = 19: two CTAs per SM as in eval_kernel),
+  // else they are appended
+  static constexpr bool IN_RBUF = G::NRBUF == 2 && (size_t)G::R_STRIDE >= EXTRA;
   static constexpr size_t OFF_SCRATCH = IN_RBUF ? (size_t)G::R_STRIDE : ((G::SMEM + 15) / 16 * 16);
-  static constexpr size_t SMEM = IN_RBUF ? G::SMEM : OFF_SCRATCH + SCRATCH + 16;
+  static constexpr size_t OFF_PCOL = OFF_SCRATCH + X_PCOL, OFF_TH = OFF_SCRATCH + X_TH, OFF_PEERS = OFF_SCRATCH + X_PEERS,
+                          OFF_DONE = OFF_SCRATCH + X_DONE;
+  static constexpr size_t SMEM = IN_RBUF ? G::SMEM : OFF_SCRATCH + EXTRA + 128;
 };
 
 template <int M>
@@ -56,26 +72,37 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
   const unsigned bar0 = smem_u32(sm + G::OFF_BAR);
   double* const red64 = reinterpret_cast<double*>(sm + G::OFF_BAR + 64);
   double* const scr = reinterpret_cast<double*>(sm + CG::OFF_SCRATCH);
+  double* const pcol = reinterpret_cast<double*>(sm + CG::OFF_PCOL);          // this CTA's partial column
+  float* const thl = reinterpret_cast<float*>(sm + CG::OFF_TH);              // theta of the next evaluation
+  const double** const peers = reinterpret_cast<const double**>(sm + CG::OFF_PEERS);
+  int* const done_l = reinterpret_cast<int*>(sm + CG::OFF_DONE);
   StepScratch sc;
   sc.sh_rows = reinterpret_cast<double (*)[kFitThreads / 32]>(scr);
   sc.s_alpha = scr + 2 * (kFitThreads / 32);
   sc.gsum = sc.s_alpha + kMaxHistory;
   sc.xs = sc.gsum + kFitThreads * CG::PER;
+  sc.peer_cols = peers;  sc.th_local = thl;  sc.done_local = done_l;
 
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int n_tiles = p.tiles_x * p.tiles_y;               // == cluster size
-  const int rank = (int)cluster_ctarank();
+  const int rank = (int)cluster.block_rank();
   const int e = (int)blockIdx.x / n_tiles, tile = rank;
   const int vr = p.n_rows - M + 1, vc = p.n_cols - M + 1;
   const size_t npix = (size_t)p.n_rows * p.n_cols;
   const int tile_y = tile / p.tiles_x, tile_x = tile - tile_y * p.tiles_x;
+  const int np = p.np;                                     // == M * M + 1 (no background polynomial here)
 
   if (tid == 0) {
     const unsigned cnt = p.use_tma ? 1u : (unsigned)kThreads;
 #pragma unroll
     for (int b = 0; b < 3; ++b) mbar_init(bar0 + 8u * b, cnt);
     fence_mbar_init();
+    *done_l = 0;
   }
+  if (rank == 0 && tid < n_tiles) peers[tid] = cluster.map_shared_rank(pcol, tid);
+  for (int k = tid; k < np; k += kThreads) thl[k] = p.theta[(size_t)e * np + k];     // fit_init_kernel's theta32
   __syncthreads();
   stage_R<M>(p, tm, e, tile, smem_u32(Rs), bar0);          // once: the tiles stay resident for the whole fit
   stage_I<M>(p, tm, e, tile, smem_u32(Is), bar0 + 16u);
@@ -87,21 +114,19 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
   const int g_a = tid % M, g_s = tid / M;
   const bool g_active = g_s < G::S;
   float4* const myacc = reinterpret_cast<float4*>(accS + tid * G::KP);
-  const int ncols = n_tiles;
-  double* const out = p.partials + ((size_t)e * p.part_rows) * ncols + rank;
-  const float* __restrict__ th = p.theta + (size_t)e * p.np;
   const bool edge = (tile_y * kTH + kTH > vr) || (tile_x * kTW + kTW > vc);
   const int rows_here = min(kTH, vr - tile_y * kTH);
   const int n_items = rows_here * (kTW / kP);
   if (tid < kMaxBg) Bs[tid] = 0.f;
+  cluster.sync();                                          // every CTA of the cluster has started (its shared memory exists)
 
   while (true) {
-    if (__ldcg(a.b.done + e)) break;                       // set by rank 0 before the barrier that ended the last pass
+    if (*done_l) break;                                    // stored by rank 0 before the barrier that ended the last pass
     for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
       const int ka = idx / G::KP, kb = idx - ka * G::KP;
-      Ks[idx] = (kb < M) ? __ldcg(th + ka * M + kb) : 0.f;
+      Ks[idx] = (kb < M) ? thl[ka * M + kb] : 0.f;
     }
-    const float B0 = __ldcg(th + M * M);
+    const float B0 = thl[M * M];
 #pragma unroll
     for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
@@ -130,13 +155,7 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
       grad_acc_store<M>(A, myacc);
     }
     __syncthreads();
-    for (int o = tid; o < M * M; o += kThreads) {          // FP64 fold of the strips, the order of eval_kernel's flush
-      const int oa = o / M, ob = o - oa * M;
-      double s = 0.0;
-#pragma unroll 1
-      for (int ss = 0; ss < G::S; ++ss) s += (double)accS[(ss * M + oa) * G::KP + ob];
-      out[(size_t)o * ncols] = s;
-    }
+    fold_strips<M>(accS, tid, [&](int o, double s) { pcol[o] = s; });      // the order of eval_kernel's flush
     {
       const double l = warp_sum_f64(loss64), g0 = warp_sum_f64(gb064);
       if (lane == 0) { red64[warp] = l; red64[8 + warp] = g0; }
@@ -145,14 +164,20 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
     if (tid == 0) {
       double ls = 0.0, gs = 0.0;
       for (int w = 0; w < kThreads / 32; ++w) { ls += red64[w]; gs += red64[8 + w]; }
-      out[(size_t)(M * M) * ncols] = gs;
-      out[(size_t)p.np * ncols] = ls;
+      pcol[M * M] = gs;
+      pcol[np] = ls;
     }
-    __threadfence();
-    cluster_sync_all();                                    // every partial column of this epoch is in global memory
-    if (rank == 0) fit_step_body<CG::PER>(a, e, sc);
-    __threadfence();
-    cluster_sync_all();                                    // theta32 / done of the next pass are visible
+    cluster.sync();                                        // every partial column of this epoch is complete
+    if (rank == 0) {
+      fit_step_body<CG::PER>(a, e, sc);                    // leaves the next theta in thl, the done flag in done_l
+      __syncthreads();
+      for (int r = 1; r < n_tiles; ++r) {                  // hand both to the other CTAs of the cluster
+        float* rth = cluster.map_shared_rank(thl, r);
+        for (int k = tid; k < np; k += kThreads) rth[k] = thl[k];
+        if (tid == 0) *cluster.map_shared_rank(done_l, r) = *done_l;
+      }
+    }
+    cluster.sync();                                        // theta / done of the next pass are in place; pcol is free
   }
 }
 
