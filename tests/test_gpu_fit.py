@@ -346,7 +346,7 @@ def test_fit_lockstep_large_kernels(dia, m, lam):
     _assert_fit_close(tho, ro, thg.cpu().numpy(), rg, f"lockstep m={m} lambda={lam}")
 
 
-@pytest.mark.parametrize("c,n,m,E", [(0, None, None, 1), (0, 100, 5, 3), (4, 142, 19, 5), (1, 190, 9, 2)])
+@pytest.mark.parametrize("c,n,m,E", [(0, None, None, 1), (0, 100, 5, 3), (4, 142, 19, 5), (1, 190, 9, 2), (2, 120, 9, 2)])
 def test_fit_cluster_kernel_matches_graph_loop(dia, monkeypatch, c, n, m, E):
     """Small image pairs with the plain objective are fitted inside one kernel, one thread-block cluster per epoch
     (csrc/dia_fit_cluster.cuh: tiles resident in shared memory, cluster barriers instead of launches).  Same device
@@ -357,7 +357,8 @@ def test_fit_cluster_kernel_matches_graph_loop(dia, monkeypatch, c, n, m, E):
     outs = []
     for disable in ("0", "1"):
         monkeypatch.setenv("DIA_DISABLE_CLUSTER", disable)
-        h = dia.Handle(_dev(w.R), w.m, max_epochs=E, sigma0=w.sigma0, gain=w.gain)
+        h = dia.Handle(_dev(w.R), w.m, max_epochs=E, sigma0=w.sigma0, gain=w.gain,
+                       loss=dia.LOSS_HUBER if w.loss == "huber" else dia.LOSS_GAUSSIAN)      # (config 2: the robust objective)
         res = []
         for og in (dia.FitOpts.default(max_adam_iters=2500, max_lbfgs_iters=60),
                    dia.FitOpts.default(force_adam_iters=25, force_lbfgs_iters=7, lbfgs_backtrack=1)):
