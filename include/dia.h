@@ -167,6 +167,33 @@ int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, double* d_si
 int dia_difference_image(dia_handle* h, int n_epochs, const float* d_I, const unsigned char* d_mask,
                          const float* d_var, const float* d_theta, float* d_D, double* d_metrics);
 
+/* dia_eval_loss_grad for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same operation (see dia_eval_loss_grad above), the same kernels
+ * (eval_kernel + reduce_partials_kernel [+ penalty_kernel]), no handle.  The per-CTA FP64 block partials -- the only
+ * scratch memory of that path, which dia_create allocates with cudaMalloc -- live in a file-scope __device__ array of
+ * DIA_STATIC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits.
+ *   cfg      as for dia_create (cfg->max_epochs is ignored: the batch is n_epochs; cfg->stream is the stream);
+ *   d_R      [n_rows][n_cols] DEVICE ([n_epochs][..][..] when cfg->n_refs == n_epochs); the other arguments exactly
+ *            as for dia_eval_loss_grad.  Inputs and outputs are the caller's; nothing is kept after the call.
+ * The call allocates nothing: no cudaMalloc / cudaFree / allocating library routine, on any path.  The first call on a
+ * device looks the array's address up (cudaGetSymbolAddress) and the first call per (device, m) sets the kernels'
+ * shared-memory attribute; later calls only encode two TMA descriptors on the host and enqueue the kernels.
+ * Asynchronous on cfg->stream.  Results are bit-identical to dia_eval_loss_grad on a handle created with
+ * max_epochs == n_epochs whenever that handle runs the shared-memory variant of the generic kernel (always, apart from
+ * m <= 3 plain objectives and launches long enough for the constant-bank variant, whose sums agree to rounding).
+ * Limits and errors: UNSUPPORTED with a message naming both numbers when the partials
+ *   8 * n_epochs * (m*m + n_bg + 1) * min(tiles, resident CTAs)  bytes   (tiles = 64 x 64 tiles of the valid region)
+ * exceed DIA_STATIC_SCRATCH_BYTES (e.g. one 4096^2 pair up to m = 27, or four at m = 19, fit; sixteen do not);
+ * INVALID_ARG / UNSUPPORTED / CUDA as for dia_create and dia_eval_loss_grad (text: dia_last_error(NULL)).
+ * ALL CALLS ON A DEVICE SHARE THE ARRAY: two calls whose kernels can overlap on the GPU (different streams without an
+ * ordering between them, or two host threads) race on it and both results are garbage; calls on one stream are ordered
+ * and safe.  The array keeps the last call's partial sums; the kernel overwrites every element the reduction reads
+ * before it reads it, so nothing has to be cleared between calls (tests/test_zz_no_alloc.py runs two in a row). */
+#define DIA_STATIC_SCRATCH_BYTES (4u << 20)
+int dia_eval_loss_grad_static(const dia_config* cfg, const float* d_R, int n_epochs,
+                              const float* d_I, const unsigned char* d_mask, const float* d_var,
+                              const float* d_theta, double* d_loss, double* d_grad);
+
 /* Frees the handle's workspace (synchronises the handle's stream first). */
 int dia_destroy(dia_handle* h);
 

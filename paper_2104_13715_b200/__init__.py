@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     dia_hessian,
     dia_covariance,
     dia_eval_loss_grad,
+    dia_eval_loss_grad_static,
+    STATIC_SCRATCH_BYTES,
     dia_fit,
     dia_measure_fp32_peak,
     dia_measure_fp32_pattern,

@@ -20,7 +20,9 @@ NOISE_MODEL, NOISE_FIXED = 0, 1
 FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "nonfinite"}
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
-                    "dia_measure_fp32_peak", "dia_measure_fp32_pattern", "dia_difference_image", "dia_hessian", "dia_covariance")
+                    "dia_measure_fp32_peak", "dia_measure_fp32_pattern", "dia_difference_image", "dia_hessian", "dia_covariance",
+                    "dia_eval_loss_grad_static")
+STATIC_SCRATCH_BYTES = 4 << 20          # DIA_STATIC_SCRATCH_BYTES of include/dia.h
 
 
 class DiaError(RuntimeError):
@@ -88,6 +90,7 @@ def load_library(build_if_missing: bool = True):
     lib.dia_create.argtypes = [C.POINTER(_Config), C.c_void_p, C.POINTER(C.c_void_p)]
     lib.dia_eval_loss_grad.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.dia_eval_loss_grad_static.argtypes = [C.POINTER(_Config), C.c_void_p, C.c_int] + [C.c_void_p] * 6
     lib.dia_fit.argtypes = [C.c_void_p, C.POINTER(FitOpts), C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                             C.c_void_p, C.c_void_p]
     lib.dia_destroy.argtypes = [C.c_void_p]
@@ -143,6 +146,24 @@ def dia_eval_loss_grad(handle: int, n_epochs: int, d_I, d_mask, d_var, d_theta, 
                                   _dptr(d_theta, torch.float32, "d_theta"),
                                   _dptr(d_loss, torch.float64, "d_loss"), _dptr(d_grad, torch.float64, "d_grad")),
            handle)
+
+
+def dia_eval_loss_grad_static(n_rows: int, n_cols: int, m: int, d_R, n_epochs: int, d_I, d_mask, d_var, d_theta,
+                              d_loss, d_grad, *, loss: int = LOSS_GAUSSIAN, huber_c: float = 1.345,
+                              noise: int = NOISE_MODEL, sigma0: float = 0.0, gain: float = 1.0, d_flat=None,
+                              stream: Optional[torch.cuda.Stream] = None, n_refs: int = 1, lambda_reg: float = 0.0,
+                              bg_degree: int = 0) -> None:
+    """dia_eval_loss_grad without a handle and without any device allocation: the block partials go to the
+    library's static device array (at most STATIC_SCRATCH_BYTES; include/dia.h).  All arguments are the caller's
+    tensors; calls that can overlap on the GPU race on the array."""
+    lib = load_library()
+    cfg = _Config(n_rows, n_cols, m, n_epochs, loss, huber_c, noise, sigma0, gain,
+                  None if d_flat is None else _dptr(d_flat, torch.float32, "d_flat").value,
+                  None if stream is None else stream.cuda_stream, n_refs, lambda_reg, bg_degree)
+    _check(lib.dia_eval_loss_grad_static(C.byref(cfg), _dptr(d_R, torch.float32, "d_R"), n_epochs,
+                                         _dptr(d_I, torch.float32, "d_I"), _dptr(d_mask, torch.uint8, "d_mask"),
+                                         _dptr(d_var, torch.float32, "d_var"), _dptr(d_theta, torch.float32, "d_theta"),
+                                         _dptr(d_loss, torch.float64, "d_loss"), _dptr(d_grad, torch.float64, "d_grad")))
 
 
 def dia_fit(handle: int, opts: FitOpts, n_epochs: int, d_I, d_mask, d_var, d_theta, d_result) -> None:

@@ -723,3 +723,125 @@ extern "C" int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_
   }
   return DIA_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// dia_eval_loss_grad_static: the evaluation for callers that cannot allocate (include/dia.h).
+// The block partials live in a file-scope device array.  In host code `g_static_partials` is only the host-side
+// shadow of the symbol, not a device address: the address is looked up once per device with cudaGetSymbolAddress,
+// with that device current, and passed to the kernels in EvalParams::partials like any other workspace.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_static_partials[DIA_STATIC_SCRATCH_BYTES / sizeof(double)];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+  double* partials = nullptr;                               // device address of g_static_partials on this device
+  int sms = 0;
+  signed char occ[DIA_MAX_KERNEL_SIZE + 1] = {};            // resident CTAs per SM of eval_kernel<m> (0: not set up yet)
+};
+std::mutex g_static_mutex;
+StaticDevice g_static_dev[kStaticMaxDevices];
+}  // namespace
+
+// once per device (address, SM count) and once per (device, m) (shared-memory attribute, occupancy); no allocation
+static int static_setup(int dev, int m, size_t smem, StaticDevice* out) {
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticDevice& d = g_static_dev[dev];
+  if (!d.partials) {
+    double* ptr = nullptr;
+    cudaError_t ce = cudaGetSymbolAddress((void**)&ptr, g_static_partials);
+    if (ce != cudaSuccess || !ptr) return cuda_fail(nullptr, ce, "cudaGetSymbolAddress(static scratch)");
+    int sms = 0;
+    ce = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaDeviceGetAttribute");
+    d.sms = sms;
+    d.partials = ptr;
+  }
+  if (d.occ[m] == 0) {
+    int occ = 0;
+    for (int aux = 0; aux < 2; ++aux) {                     // plain and generic (mask / flat / variance map) variants
+      const void* k = kernel_for(m, aux == 1);
+      cudaError_t ce = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaFuncSetAttribute(smem)");
+      int o = 0;
+      ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, dia::kThreads, smem);
+      if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "occupancy query");
+      if (o < 1) return fail(nullptr, DIA_ERR_UNSUPPORTED, "the evaluation kernel of this kernel size does not fit on an SM of this device");
+      occ = (aux == 0 || o < occ) ? o : occ;
+    }
+    d.occ[m] = (signed char)(occ > 127 ? 127 : occ);
+  }
+  *out = d;
+  return DIA_OK;
+}
+
+extern "C" int dia_eval_loss_grad_static(const dia_config* cfg, const float* d_R, int n_epochs, const float* d_I,
+                                         const unsigned char* d_mask, const float* d_var, const float* d_theta,
+                                         double* d_loss, double* d_grad) {
+  if (!cfg || !d_R || !d_I || !d_theta || !d_loss || !d_grad) return fail(nullptr, DIA_ERR_INVALID_ARG, "null argument");
+  if (cfg->m < 1 || cfg->m % 2 == 0) return fail(nullptr, DIA_ERR_INVALID_ARG, "m must be odd and >= 1");
+  if (cfg->m > DIA_MAX_KERNEL_SIZE) return fail(nullptr, DIA_ERR_UNSUPPORTED, "m exceeds DIA_MAX_KERNEL_SIZE");
+  if (cfg->n_rows < cfg->m || cfg->n_cols < cfg->m) return fail(nullptr, DIA_ERR_INVALID_ARG, "image smaller than kernel");
+  if (n_epochs < 1) return fail(nullptr, DIA_ERR_INVALID_ARG, "n_epochs must be >= 1");
+  if (!(cfg->lambda_reg >= 0.f)) return fail(nullptr, DIA_ERR_INVALID_ARG, "lambda_reg must be >= 0");
+  if (cfg->bg_degree < 0) return fail(nullptr, DIA_ERR_INVALID_ARG, "bg_degree must be >= 0");
+  if (cfg->bg_degree > DIA_MAX_BG_DEGREE) return fail(nullptr, DIA_ERR_UNSUPPORTED, "bg_degree exceeds DIA_MAX_BG_DEGREE");
+  if (cfg->n_refs > 1 && cfg->n_refs != n_epochs) return fail(nullptr, DIA_ERR_INVALID_ARG, "n_refs must be 0, 1 or n_epochs");
+  if (cfg->loss != DIA_LOSS_GAUSSIAN && cfg->loss != DIA_LOSS_HUBER) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad loss");
+  if (cfg->noise != DIA_NOISE_MODEL && cfg->noise != DIA_NOISE_FIXED) return fail(nullptr, DIA_ERR_INVALID_ARG, "bad noise mode");
+  if (cfg->loss == DIA_LOSS_HUBER && !(cfg->huber_c > 0.f)) return fail(nullptr, DIA_ERR_INVALID_ARG, "huber_c must be > 0");
+  if (cfg->noise == DIA_NOISE_MODEL && !(cfg->gain > 0.f && cfg->sigma0 >= 0.f))
+    return fail(nullptr, DIA_ERR_INVALID_ARG, "need gain > 0 and sigma0 >= 0");
+  if (cfg->noise == DIA_NOISE_FIXED && !d_var) return fail(nullptr, DIA_ERR_INVALID_ARG, "DIA_NOISE_FIXED needs d_var");
+  if (cfg->noise == DIA_NOISE_MODEL && d_var) return fail(nullptr, DIA_ERR_INVALID_ARG, "d_var must be NULL in DIA_NOISE_MODEL");
+
+  int dev = 0;
+  cudaError_t ce = cudaGetDevice(&dev);
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDevice (no CUDA device: there is no CPU fallback)");
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, DIA_ERR_UNSUPPORTED, "device ordinal beyond the static set-up table");
+  StaticDevice sd;
+  int rc = static_setup(dev, cfg->m, smem_for(cfg->m), &sd);
+  if (rc != DIA_OK) return rc;
+
+  // a handle on the stack, laid out as dia_create would for max_epochs == n_epochs; generic kernel only (no
+  // eval_small_kernel, no constant bank), its workspace pointer aimed at the static array
+  dia_handle hs;
+  hs.cfg = *cfg;  hs.cfg.max_epochs = n_epochs;
+  hs.d_R = d_R;  hs.stream = (cudaStream_t)cfg->stream;  hs.sms = sd.sms;
+  hs.n_refs = cfg->n_refs > 1 ? cfg->n_refs : 1;
+  hs.np = cfg->m * cfg->m + (cfg->bg_degree + 1) * (cfg->bg_degree + 2) / 2;
+  hs.smem = smem_for(cfg->m);
+  hs.d_const_stage = nullptr;  hs.small_grid = 0;  hs.grid_limit = 0;  hs.cluster_fit = 0;
+  hs.flush_tiles = dia::kFlushTiles;
+  hs.tiles = ((cfg->n_cols - cfg->m + 1 + dia::kTW - 1) / dia::kTW) * ((cfg->n_rows - cfg->m + 1 + dia::kTH - 1) / dia::kTH);
+  const long long items = (long long)hs.tiles * n_epochs, resident = (long long)sd.sms * sd.occ[cfg->m];
+  hs.grid = (int)(items < resident ? items : resident);
+  hs.use_tma = 0;
+  if (cfg->n_cols % 4 == 0 && aligned16(d_R)) {             // descriptor encoding is host arithmetic, no allocation
+    int rpitch = 0, rh = 0;
+    geometry_for(cfg->m, &rpitch, &rh);
+    hs.use_tma = make_tensor_map(&hs.tmR, d_R, cfg->n_cols, cfg->n_rows, hs.n_refs, rpitch, rh) ? 1 : 0;
+  }
+  hs.d_partials = sd.partials;
+  std::memset(&hs.fit, 0, sizeof(hs.fit));                  // never touched on this path
+
+  const int np1 = hs.np + 1;
+  const unsigned long long need = 8ull * (unsigned long long)n_epochs * np1 * (unsigned long long)dia::eval_part_cols(&hs, n_epochs);
+  if (need > DIA_STATIC_SCRATCH_BYTES)
+    return fail(nullptr, DIA_ERR_UNSUPPORTED, "dia_eval_loss_grad_static: this batch needs " + std::to_string(need) +
+                " bytes of block partials, the static scratch holds DIA_STATIC_SCRATCH_BYTES = " +
+                std::to_string((unsigned long long)DIA_STATIC_SCRATCH_BYTES) + " (use a handle, or fewer epochs per call)");
+
+  dia::EvalParams p;
+  dia::TensorMaps tm;
+  fill_params(&hs, n_epochs, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, -1);
+  ce = dia::launch_eval(&hs, p, tm);
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "eval launch");
+  dia::reduce_partials_kernel<<<dim3((np1 + 7) / 8, n_epochs), 256, 0, hs.stream>>>(
+      hs.d_partials, dia::eval_part_cols_p(&hs, p), np1, nullptr, d_loss, d_grad);
+  if (cfg->lambda_reg > 0.f)
+    dia::penalty_kernel<<<n_epochs, dia::kFitThreads, 0, hs.stream>>>(d_theta, cfg->m, hs.np, lambda_n(&hs), d_loss, d_grad);
+  ce = cudaGetLastError();
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "reduce launch");
+  return DIA_OK;
+}
