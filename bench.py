@@ -534,13 +534,15 @@ def run_gpu(args):
         if rank == 0:
             rows = M * M + 1
             ci = cov_info.cpu().tolist()
-            # work model of dia_hessian: per launch of 32 kernel-pixel rows (kHessRows) one forward pass and 32 gradient
-            # passes (m^2 FMA per valid pixel each); the B0 row is one ordinary evaluation (2 m^2)
-            n_launch = -(-(M * M) // 32)
-            fma_h = (n_launch + M * M + 2 * (rows - M * M)) * 0.5 * useful_fma()
-            line["fits"]["hessian"] = {"ms": ms_h, "rows": rows, "launches": n_launch + 1,
-                                       "tflops": 2.0 * fma_h / (ms_h * 1e-3) / 1e12,
-                                       "work_model": "1 forward + 32 gradient passes per 32-row launch"}
+            # dia_hessian is one tensor-core contraction X' diag(h) X over the valid pixels (hess_tc_kernel):
+            # "useful" counts the dense np x np x pixels product once (2 flops per multiply-add); the kernel computes the
+            # upper block triangle of the 128-padded matrix in four split-float16 terms
+            n_valid = (N - M + 1) ** 2
+            line["fits"]["hessian"] = {"ms": ms_h, "rows": rows, "launches": 3,
+                                       "useful_tflops": 2.0 * rows * rows * n_valid / (ms_h * 1e-3) / 1e12,
+                                       "path": "tcgen05 kind::f16, float16 hi/lo split (4 terms), FP32 in TMEM per tile row, "
+                                               "FP64 per tile",
+                                       "work_model": "2 np^2 flops per valid pixel"}
             line["fits"]["covariance"] = {"ms": ms_c, "np": rows, "launches": rows + 3, "valid": ci[0],
                                           "sigma_P": ci[2], "sigma_B0": float(sig_hat[M * M])}
 

@@ -15,7 +15,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libdia_b200.so")
 KERNEL_SIZES = list(range(1, 48, 2))
-HEADERS = ["dia_eval.cuh", "dia_eval_small.cuh", "dia_fit.cuh", "dia_hess.cuh", "dia_cov.cuh", "dia_probe.cuh"]
+HEADERS = ["dia_eval.cuh", "dia_eval_small.cuh", "dia_fit.cuh", "dia_fit_cluster.cuh", "dia_hess.cuh", "dia_hess_tc.cuh", "dia_cov.cuh",
+           "dia_probe.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 
@@ -52,8 +53,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for m in KERNEL_SIZES:
         jobs.append((os.path.join(CSRC, "dia_eval_inst.cu"), os.path.join(OBJ, f"dia_eval_m{m}.o"),
                      [f"-DDIA_INST_M={m}"], verbose))
-    # the per-kernel-size units include dia_eval.cuh only; objects newer than their sources are kept
-    inst_deps = [os.path.join(CSRC, f) for f in ("dia_eval.cuh", "dia_eval_inst.cu")] + [os.path.join(HERE, "build.py")]
+    # the per-kernel-size units include the kernel headers only; objects newer than their sources are kept
+    inst_deps = [os.path.join(CSRC, f) for f in ("dia_eval.cuh", "dia_fit.cuh", "dia_fit_cluster.cuh", "dia_hess_tc.cuh", "dia_eval_inst.cu")] + \
+                [os.path.join(HERE, "build.py")]
     todo = [j for j in jobs if force or _stale(j[1], _deps() if j[1].endswith("dia_api.o") else inst_deps)]
     workers = max(1, min(len(todo), os.cpu_count() or 1))
     with concurrent.futures.ThreadPoolExecutor(max_workers=workers) as pool:

@@ -17,6 +17,7 @@
 #include "dia_fit.cuh"
 #include "dia_fit_cluster.cuh"
 #include "dia_hess.cuh"
+#include "dia_hess_tc.cuh"
 #include "dia_cov.cuh"
 #include "dia_probe.cuh"
 
@@ -119,7 +120,8 @@ static void geometry_for(int m, int* rpitch, int* rh) {
 // The kernel instantiations live in one translation unit per m (dia_eval_inst.cu); each exports its kernels and
 // the host shadow of its own constant block.
 namespace dia {
-#define X(MM) const void* eval_kernel_ptr_m##MM(int variant); const void* const_symbol_m##MM(); size_t cluster_smem_m##MM();
+#define X(MM) const void* eval_kernel_ptr_m##MM(int variant); const void* const_symbol_m##MM(); size_t cluster_smem_m##MM(); \
+  size_t hess_tc_smem_m##MM();
 DIA_FOR_EACH_M(X)
 #undef X
 }  // namespace dia
@@ -150,6 +152,22 @@ static const void* cluster_kernel_for(int m) {
 #undef X
   }
   return nullptr;
+}
+static const void* hess_tc_kernel_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::eval_kernel_ptr_m##MM(7);
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return nullptr;
+}
+static size_t hess_tc_smem_for(int m) {
+  switch (m) {
+#define X(MM) case MM: return dia::hess_tc_smem_m##MM();
+    DIA_FOR_EACH_M(X)
+#undef X
+  }
+  return 0;
 }
 static size_t cluster_smem_for(int m) {
   switch (m) {
@@ -546,9 +564,36 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
   // gradient pass per row; it delivers the kernel-kernel block, the remaining entries of these rows
   // come from the background rows below by symmetry.
   const int nk = h->cfg.m * h->cfg.m;
+  // m >= 5: all of H is one split-float16 tensor-core contraction (hess_tc_kernel); test hook
+  // DIA_HESS_TC=0 keeps the CUDA-core row passes below
+  const char* tc_env = std::getenv("DIA_HESS_TC");
+  const void* ktc = (h->cfg.m >= 5 && !(tc_env && tc_env[0] == '0')) ? hess_tc_kernel_for(h->cfg.m) : nullptr;
+  dia::HessTcTypes tct;
+  if (ktc && dia::hess_tc_make_types(np, &tct) == 0) ktc = nullptr;
+  if (ktc) {
+    int per_type = h->sms / tct.n_types;
+    if (h->grid_limit > 0 && h->grid_limit / tct.n_types < per_type) per_type = h->grid_limit / tct.n_types;   // test hook: many tiles per CTA
+    tct.ctas_per_type = per_type < 1 ? 1 : (per_type > h->tiles ? h->tiles : per_type);
+    const int tgrid = tct.n_types * tct.ctas_per_type;
+    if (!w.tc_partials || w.tc_grid < tgrid) {
+      cudaFree(w.tc_partials);  w.tc_partials = nullptr;  w.tc_grid = 0;
+      cudaError_t ce = cudaFuncSetAttribute(ktc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hess_tc_smem_for(h->cfg.m));
+      if (ce == cudaSuccess) ce = cudaMalloc(&w.tc_partials, sizeof(double) * (size_t)tgrid * dia::kTcRows * dia::kTcGroup);
+      if (ce != cudaSuccess) { cudaGetLastError(); return fail(h, DIA_ERR_ALLOC, std::string("hessian tensor-core workspace: ") + cudaGetErrorString(ce)); }
+      w.tc_grid = tgrid;
+    }
+    dia::EvalParams p;
+    dia::TensorMaps tm;
+    fill_params(h, 1, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, 0);
+    void* args[] = {(void*)&p, (void*)&w.tc_partials, (void*)&tct};
+    cudaError_t ce = cudaLaunchKernel(ktc, dim3(tgrid), dim3(dia::kThreads), args, hess_tc_smem_for(h->cfg.m), h->stream);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "hessian tensor-core launch");
+    dia::hess_tc_reduce_kernel<<<dim3((dia::kTcRows * dia::kTcGroup + 255) / 256, tct.n_types), 256, 0, h->stream>>>(
+        w.tc_partials, tct, np, d_H);
+  }
   const void* kblock = hess_kernel_for(h->cfg.m);
   const int bgrid = h->grid < h->tiles ? h->grid : h->tiles;
-  for (int q0 = 0; q0 < nk; q0 += dia::kHessRows) {
+  for (int q0 = 0; q0 < (ktc ? 0 : nk); q0 += dia::kHessRows) {
     const int n = nk - q0 < dia::kHessRows ? nk - q0 : dia::kHessRows;
     dia::EvalParams p;
     dia::TensorMaps tm;
@@ -562,12 +607,12 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
         w.partials, bgrid, np1, nullptr, w.loss + q0, d_H + (size_t)q0 * np);
   }
   // Background rows (B0 and the polynomial terms): the fused kernel with the weight h X_q in place of w (D3)
-  for (int q0 = nk; q0 < np; q0 += h->cfg.max_epochs) {
+  for (int q0 = nk; q0 < (ktc ? 0 : np); q0 += h->cfg.max_epochs) {
     const int n = np - q0 < h->cfg.max_epochs ? np - q0 : h->cfg.max_epochs;
     rc = eval_into(h, n, d_I, d_mask, d_var, d_theta, w.loss + q0, d_H + (size_t)q0 * np, q0);
     if (rc != DIA_OK) return rc;
   }
-  dia::hess_fill_columns_kernel<<<(nk * (np - nk) + 255) / 256, 256, 0, h->stream>>>(d_H, np, nk);
+  if (!ktc) dia::hess_fill_columns_kernel<<<(nk * (np - nk) + 255) / 256, 256, 0, h->stream>>>(d_H, np, nk);
   // Eq. 20: the penalty lambda N |L theta|^2 adds 2 lambda N L'L; its gradient is linear in theta, so the
   // gradient at the unit vector e_q is row q
   if (h->cfg.lambda_reg > 0.f)

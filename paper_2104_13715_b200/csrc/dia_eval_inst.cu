@@ -4,6 +4,7 @@
 // accessors that dia_api.cu uses to launch the kernels and to address the constant symbol.
 #include "dia_eval.cuh"
 #include "dia_fit_cluster.cuh"
+#include "dia_hess_tc.cuh"
 
 #ifndef DIA_INST_M
 #error "compile with -DDIA_INST_M=<odd kernel size>"
@@ -16,7 +17,8 @@ namespace dia {
 
 // variant: 0 = plain objective, 1 = generic (mask / flat / variance map), 2 = difference image,
 //          3 = plain objective with the kernel pixels in the constant bank, 4 = kernel-kernel block of the Hessian,
-//          5 = generic with the kernel pixels in the constant bank, 6 = whole fit of a small image in one cluster
+//          5 = generic with the kernel pixels in the constant bank, 6 = whole fit of a small image in one cluster,
+//          7 = kernel-kernel block of the Hessian on the tensor cores (null when its shared memory does not fit)
 const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
   switch (variant) {
     case 0: return (const void*)eval_kernel<DIA_INST_M, false, false, false>;
@@ -26,12 +28,14 @@ const void* DIA_CAT(eval_kernel_ptr_m, DIA_INST_M)(int variant) {
     case 4: return (const void*)hess_block_kernel<DIA_INST_M>;
     case 5: return (const void*)eval_kernel<DIA_INST_M, true, false, true>;
     case 6: return (const void*)fit_cluster_kernel<DIA_INST_M>;
+    case 7: return TcGeo<DIA_INST_M>::FITS ? (const void*)hess_tc_kernel<DIA_INST_M> : nullptr;
   }
   return nullptr;
 }
 
-// dynamic shared memory of fit_cluster_kernel
+// dynamic shared memory of fit_cluster_kernel and of hess_tc_kernel
 size_t DIA_CAT(cluster_smem_m, DIA_INST_M)() { return ClusterGeo<DIA_INST_M>::SMEM; }
+size_t DIA_CAT(hess_tc_smem_m, DIA_INST_M)() { return TcGeo<DIA_INST_M>::SMEM; }
 
 // host shadow of this unit's constant block (what cudaMemcpyToSymbol / graph memcpy nodes take)
 const void* DIA_CAT(const_symbol_m, DIA_INST_M)() { return (const void*)&c_blk; }

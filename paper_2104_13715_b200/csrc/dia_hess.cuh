@@ -13,10 +13,12 @@ struct HessWorkspace {
   double* partials = nullptr;  // [kHessRows][np+1][CTAs] block partials of hess_block_kernel (its own: the row count
                                // per launch does not depend on the handle's max_epochs)
   double* chol = nullptr;      // [np][np] Cholesky factor of dia_covariance (L below, L' above the diagonal)
+  double* tc_partials = nullptr;   // [CTAs][256][128] FP64 blocks of hess_tc_kernel (dia_hess_tc.cuh), allocated on first use
+  int tc_grid = 0;             // CTAs those blocks were sized for
 };
 
 inline void hess_workspace_destroy(HessWorkspace* w) {
-  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->partials); cudaFree(w->chol);
+  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->partials); cudaFree(w->chol); cudaFree(w->tc_partials);
   *w = HessWorkspace();
 }
 

@@ -132,13 +132,15 @@ def test_hessian_argument_errors(dia):
     h.close()
 
 
+@pytest.mark.parametrize("tc", ["1", "0"])
 @pytest.mark.parametrize("grid_limit", [1, 5])
-def test_hessian_many_tiles_per_cta(dia, monkeypatch, grid_limit):
-    """Test hook DIA_GRID_LIMIT: one or five CTAs walk through all 36 tiles of a 400^2 image, so every CTA of
-    hess_block_kernel accumulates its FP64 partial column over many tiles (the launch shape of a 4096^2 image: 4096
-    tiles on 296 CTAs) and restages its single R / I buffer between them; 81 kernel-pixel rows in launches of 32 leave a
-    ragged last one."""
+def test_hessian_many_tiles_per_cta(dia, monkeypatch, grid_limit, tc):
+    """Test hook DIA_GRID_LIMIT: one or five CTAs walk through all 36 tiles of a 400^2 image, so every CTA
+    accumulates its FP64 partials over many tiles (the launch shape of a 4096^2 image: 4096 tiles on 147 or 296 CTAs) and
+    restages its single R / I buffer between them; both paths: hess_tc_kernel (one type at m = 9) and, with
+    DIA_HESS_TC=0, hess_block_kernel, whose 81 kernel-pixel rows in launches of 32 leave a ragged last one."""
     monkeypatch.setenv("DIA_GRID_LIMIT", str(grid_limit))
+    monkeypatch.setenv("DIA_HESS_TC", tc)
     w = make_workload(4, n=400, m=9, n_epochs=1)
     cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
     h = dia.Handle(_dev(w.R), w.m, max_epochs=23, sigma0=w.sigma0, gain=w.gain)
@@ -147,7 +149,50 @@ def test_hessian_many_tiles_per_cta(dia, monkeypatch, grid_limit):
     Ho = oracle.hessian(cfg, w.R, w.I[0], th)
     Hg = h.hessian(_dev(w.I[0]), _dev(th)).cpu().numpy()
     e = _e_H(Hg, Ho)
-    print(f"hessian grid={grid_limit}: e_H={e:.2e}")
+    print(f"hessian grid={grid_limit} tensor cores={tc}: e_H={e:.2e}")
     assert e <= TOL_H
     assert np.array_equal(Hg, h.hessian(_dev(w.I[0]), _dev(th)).cpu().numpy())
     h.close()
+
+
+@pytest.mark.parametrize("c,n,m,outliers,sigma", [(4, 300, 19, 0, True), (1, 256, 15, 0, True), (2, 300, 13, 30, False),
+                                                  (4, 200, 27, 0, False), (0, None, None, 0, True)])
+def test_hessian_tensor_core_path_against_cuda_core_path_and_oracle(dia, monkeypatch, c, n, m, outliers, sigma):
+    """hess_tc_kernel (the default for m >= 5: split-float16 tcgen05 contraction, dia_hess_tc.cuh) against the FP32
+    CUDA-core row passes (DIA_HESS_TC=0) and the oracle: three block types at m = 19, two at m = 13 / 15, a
+    ten-type table with single off-diagonal blocks at m = 27, one 128-row block at m = 7.  `outliers` plants pixels
+    30 000 counts BELOW the model, whose h = d^2 l / dM^2 is negative (D3): their tile rows take the second, negated
+    pass of the kernel.  The uncertainties of Eq. 17 are asserted where the Hessian tests assert them (`sigma`); the
+    729-parameter kernel on a 200^2 image (cond(H) = 2e10, 42 pixels per parameter: the float32 Hessian of EITHER path is
+    at the edge of positive definiteness) is compared entry by entry only."""
+    w = make_workload(c, n=n, m=m, n_epochs=1)
+    I = w.I[0].copy()
+    if outliers:
+        rng = np.random.default_rng(3)
+        hh = (w.m - 1) // 2
+        ys, xs = rng.integers(hh, w.n - hh, outliers), rng.integers(hh, w.n - hh, outliers)
+        I[ys, xs] -= 30000.0
+    huber = w.loss == "huber" and not outliers          # the planted pixels test the quadratic loss's negative h
+    cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain, loss=oracle.LOSS_HUBER if huber else oracle.LOSS_GAUSSIAN)
+    th = w.theta_true[0].astype(np.float32)
+    Ho = oracle.hessian(cfg, w.R, I, th)
+    H = {}
+    for tc in ("1", "0"):
+        monkeypatch.setenv("DIA_HESS_TC", tc)
+        h = dia.Handle(_dev(w.R), w.m, max_epochs=4, sigma0=w.sigma0, gain=w.gain, loss=dia.LOSS_HUBER if huber else dia.LOSS_GAUSSIAN)
+        H[tc] = h.hessian(_dev(I), _dev(th)).cpu().numpy()
+        assert np.array_equal(H[tc], h.hessian(_dev(I), _dev(th)).cpu().numpy())
+        h.close()
+    e_tc, e_cc, e_x = _e_H(H["1"], Ho), _e_H(H["0"], Ho), _e_H(H["1"], H["0"])
+    nk = w.m * w.m
+    print(f"hessian c{c} n={w.n} m={w.m} outliers={outliers}: e_H tensor cores {e_tc:.2e}, CUDA cores {e_cc:.2e}, one against the "
+          f"other {e_x:.2e}; negative-h pixels matter: {bool(outliers)}")
+    assert not np.array_equal(H["1"], H["0"])          # the hook really switches the path
+    assert e_tc <= TOL_H and e_cc <= TOL_H and e_x <= TOL_H
+    if sigma:
+        sPo, sBo = _sigmas(Ho, nk)
+        for tc in ("1", "0"):
+            sPg, sBg = _sigmas(H[tc], nk)
+            print(f"   tensor cores={tc}: sigma_P {sPg:.6e} ({sPo:.6e}: {abs(sPg / sPo - 1):.1e})  sigma_B0 {sBg:.5e} ({sBo:.5e}: "
+                  f"{abs(sBg / sBo - 1):.1e})  cond(H) {np.linalg.cond(Ho):.1e}")
+            assert abs(sPg - sPo) <= TOL_SIGMA * sPo and abs(sBg - sBo) <= TOL_SIGMA * sBo
