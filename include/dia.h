@@ -218,6 +218,14 @@ int dia_get_info(const dia_handle* h, int* grid_blocks, int* threads_per_block,
 int dia_measure_fp32_peak(void* stream, double* fma_per_second);
 int dia_measure_fp32_pattern(void* stream, int pattern, double* fma_per_second);
 
+/* Tensor-core probe (measurement only; csrc/dia_tc_probe.cuh): D [128][N] = sum_k A[r][k] B[n][k] on ONE CTA with
+ * tcgen05.mma, the operands built in shared memory from the float32 DEVICE arrays d_A [128][K] and d_B [N][K] exactly as
+ * dia_hessian's tensor-core kernel builds its own (same layout, descriptors and hi / lo split), one accumulation chain
+ * over all of K in TMEM.  mode: 0 = float16 operands, 1 = float16 hi + lo split (four terms), 2 = tf32 operands,
+ * 3 = tf32 big + small split (three terms).  K a positive multiple of 64, N a multiple of 32 up to 256; d_D [128][N]
+ * float32 DEVICE.  Asynchronous on `stream`.  Shows how the tensor core rounds when it accumulates. */
+int dia_tc_probe_gemm(void* stream, const float* d_A, const float* d_B, float* d_D, int K, int N, int mode);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     dia_fit,
     dia_measure_fp32_peak,
     dia_measure_fp32_pattern,
+    dia_tc_probe_gemm,
     load_library,
     LOSS_GAUSSIAN,
     LOSS_HUBER,

@@ -21,7 +21,7 @@ FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "no
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
                     "dia_measure_fp32_peak", "dia_measure_fp32_pattern", "dia_difference_image", "dia_hessian", "dia_covariance",
-                    "dia_eval_loss_grad_static")
+                    "dia_eval_loss_grad_static", "dia_tc_probe_gemm")
 STATIC_SCRATCH_BYTES = 4 << 20          # DIA_STATIC_SCRATCH_BYTES of include/dia.h
 
 
@@ -100,6 +100,7 @@ def load_library(build_if_missing: bool = True):
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
     lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     lib.dia_measure_fp32_pattern.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+    lib.dia_tc_probe_gemm.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]
     _LIB = lib
     return lib
 
@@ -164,6 +165,19 @@ def dia_eval_loss_grad_static(n_rows: int, n_cols: int, m: int, d_R, n_epochs: i
                                          _dptr(d_I, torch.float32, "d_I"), _dptr(d_mask, torch.uint8, "d_mask"),
                                          _dptr(d_var, torch.float32, "d_var"), _dptr(d_theta, torch.float32, "d_theta"),
                                          _dptr(d_loss, torch.float64, "d_loss"), _dptr(d_grad, torch.float64, "d_grad")))
+
+
+def dia_tc_probe_gemm(d_A: torch.Tensor, d_B: torch.Tensor, mode: int) -> torch.Tensor:
+    """Tensor-core probe (measurement only): D [128][N] = A [128][K] @ B [N][K]' on one CTA, operands and accumulation as
+    in dia_hessian's tensor-core kernel; mode 0 float16, 1 float16 hi + lo split, 2 tf32, 3 tf32 split."""
+    lib = load_library()
+    K, N = int(d_A.shape[1]), int(d_B.shape[0])
+    if tuple(d_A.shape) != (128, K) or tuple(d_B.shape) != (N, K):
+        raise DiaError("d_A must be [128][K] and d_B [N][K]")
+    d_D = torch.empty((128, N), dtype=torch.float32, device=d_A.device)
+    _check(lib.dia_tc_probe_gemm(None, _dptr(d_A, torch.float32, "d_A"), _dptr(d_B, torch.float32, "d_B"),
+                                 _dptr(d_D, torch.float32, "d_D"), K, N, mode))
+    return d_D
 
 
 def dia_fit(handle: int, opts: FitOpts, n_epochs: int, d_I, d_mask, d_var, d_theta, d_result) -> None:

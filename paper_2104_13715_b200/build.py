@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libdia_b200.so")
 KERNEL_SIZES = list(range(1, 48, 2))
-HEADERS = ["dia_eval.cuh", "dia_eval_small.cuh", "dia_fit.cuh", "dia_fit_cluster.cuh", "dia_hess.cuh", "dia_hess_tc.cuh", "dia_cov.cuh",
+HEADERS = ["dia_eval.cuh", "dia_eval_small.cuh", "dia_fit.cuh", "dia_fit_cluster.cuh", "dia_hess.cuh", "dia_hess_tc.cuh", "dia_tc_probe.cuh", "dia_cov.cuh",
            "dia_probe.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

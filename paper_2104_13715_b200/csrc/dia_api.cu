@@ -20,6 +20,7 @@
 #include "dia_hess_tc.cuh"
 #include "dia_cov.cuh"
 #include "dia_probe.cuh"
+#include "dia_tc_probe.cuh"
 
 struct dia_handle {
   dia_config cfg;
@@ -748,6 +749,15 @@ extern "C" int dia_measure_fp32_pattern(void* stream, int pattern, double* fma_p
   const double v = dia::measure_fp32_pattern((cudaStream_t)stream, pattern, 5);
   if (v <= 0.0) { cudaGetLastError(); return fail(nullptr, DIA_ERR_CUDA, "FP32 probe failed (no CUDA device?)"); }
   *fma_per_second = v;
+  return DIA_OK;
+}
+
+extern "C" int dia_tc_probe_gemm(void* stream, const float* d_A, const float* d_B, float* d_D, int K, int N, int mode) {
+  if (!d_A || !d_B || !d_D) return fail(nullptr, DIA_ERR_INVALID_ARG, "null argument");
+  if (K < dia::kTcProbeKC || K % dia::kTcProbeKC != 0 || N < 32 || N > 256 || N % 32 != 0 || mode < 0 || mode > 3)
+    return fail(nullptr, DIA_ERR_INVALID_ARG, "dia_tc_probe_gemm: K must be a positive multiple of 64, N a multiple of 32 up to 256, mode 0..3");
+  const cudaError_t ce = dia::tc_probe_launch((cudaStream_t)stream, d_A, d_B, d_D, K, N, mode);
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "tensor-core probe launch");
   return DIA_OK;
 }
 

@@ -6,13 +6,13 @@
 //   * h = s_+^2 - s_-^2 with s_+- = sqrt(max(+-h, 0)), so that H = B_+' B_+ - B_-' B_- with B = diag(s) X: ONE operand
 //     matrix serves both sides of the product (rows of negative h -- Huber's linear branch, gross outliers -- take a
 //     second pass with the A operand negated; it runs only for tile rows that have such a pixel);
-//   * every float32 element of B is split into two float16 numbers, hi with 9 significant bits and lo = x - hi with 11
-//     (|x - hi - lo| <= 2^-21 |x|; a bfloat16 pair's 2^-17 was measured to leave e_H at 1 - 2e-6 on small images), and
+//   * every float32 element of B is split into two float16 numbers, hi with 8 significant bits and lo = x - hi with 11
+//     (|x - hi - lo| <= 2^-20 |x|; a bfloat16 pair's 2^-17 was measured to leave e_H at 1 - 2e-6 on small images), and
 //     the product is the four tcgen05.mma terms lo lo + lo hi + hi lo + hi hi, accumulated in float32 in TMEM.  The
-//     widths follow from the accumulator's arithmetic (next item): hi hi products are 18 bits wide and stay exact
-//     under a 64-pixel sum, the small terms go first while the accumulator is small; with 11-bit hi parts (three terms)
-//     the hi hi products lose 2e-7 of the sum -- little, but the SAME relative amount from every entry of this block
-//     and none from the background rows, which costs sigma_B0 2.5e-5 at cond(H) = 2e9 (measured).  float16 has a narrow
+//     widths follow from the accumulator's arithmetic (next item): hi hi products are 16 bits wide and stay exact
+//     under a 64-pixel sum, the small terms go first while the accumulator is small.  Measured mean bias of the sums
+//     against hi width: 11 bits (three terms) -2.1e-7, 10 bits -1.3e-7, 9 bits -7.5e-8, 8 bits -5.0e-8, 7 bits -4.4e-8
+//     (narrower hi parts raise the random error of small images instead; profiles/r02_tc_hessian.md).  float16 has a narrow
 //     exponent range, so B is scaled per tile by a power of two c with max s * max |R| * c < 2^15 (no overflow; elements
 //     below 2^-39 of the largest lose precision, which no sum can see) and the tile's sums are multiplied by c^-2
 //     when they are folded to FP64;
@@ -124,7 +124,11 @@ __device__ __forceinline__ void tc_build_row(unsigned char* __restrict__ op_hi, 
       float p0 = r[8 * kg + 2 * t] * sv[2 * t], p1 = r[8 * kg + 2 * t + 1] * sv[2 * t + 1];
       if (SCALED) { p0 *= f;  p1 *= f; }
       __half2 h = __floats2half2_rn(p0, p1);                                         // .x (low half) = p0
-      const unsigned hb = (*reinterpret_cast<const unsigned*>(&h) + 0x00020002u) & 0xFFFCFFFCu;    // 11 -> 9 significant bits
+#ifndef DIA_TC_HI_DROP
+#define DIA_TC_HI_DROP 3
+#endif
+      constexpr unsigned kHalf = (1u << (DIA_TC_HI_DROP - 1)) * 0x00010001u, kMask = ~(((1u << DIA_TC_HI_DROP) - 1u) * 0x00010001u);
+      const unsigned hb = (*reinterpret_cast<const unsigned*>(&h) + kHalf) & kMask;                // 11 -> 8 significant bits, round to nearest
       h = *reinterpret_cast<const __half2*>(&hb);
       const __half2 l = __floats2half2_rn(p0 - __low2float(h), p1 - __high2float(h));
       hi[t] = *reinterpret_cast<const unsigned*>(&h);
@@ -134,6 +138,13 @@ __device__ __forceinline__ void tc_build_row(unsigned char* __restrict__ op_hi, 
     *reinterpret_cast<uint4*>(op_lo + kg * lbo) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
   }
 }
+
+#ifdef DIA_TC_PROFILE
+__device__ long long g_tc_prof[16];
+#define TC_T(k) do { if (blockIdx.x == 0 && threadIdx.x == 32) { const long long t_ = clock64(); g_tc_prof[k] += t_ - tc_t0; tc_t0 = t_; } } while (0)
+#else
+#define TC_T(k) do { } while (0)
+#endif
 
 template <int M>
 __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p, double* __restrict__ partials,
@@ -215,6 +226,9 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
   bool first_tile = true;
   double* const outp = partials + (size_t)blockIdx.x * (kTcRows * kTcGroup);
 
+#ifdef DIA_TC_PROFILE
+  long long tc_t0 = clock64();
+#endif
   for (int t = cidx; t < n_tiles; t += ty.ctas_per_type) {
     const int tile_y = t / p.tiles_x, tile_x = t - tile_y * p.tiles_x;
     stage_tile_cp_async<G::RH, G::RPITCH>(p.R, p.n_rows, p.n_cols, p.cp8, tile_y * kTH, tile_x * kTW, smem_u32(Rs));
@@ -292,6 +306,30 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
     __syncthreads();
 
     const int rows_here = min(kTH, vr - tile_y * kTH);
+    TC_T(0);
+#ifndef DIA_TC_FOLD_ROWS
+#define DIA_TC_FOLD_ROWS 64
+#endif
+    int rows_in_acc = 0;
+    // fold the float32 row sums into this CTA's FP64 block [column][row]
+    auto fold = [&]() {
+      double* o = outp + (size_t)((warp >> 2) * ncol) * kTcGroup + (warp & 3) * 32 + lane;
+      if (n_groups == 2) {
+#pragma unroll
+        for (int c = 0; c < kTcGroup; ++c) {
+          o[(size_t)c * kTcGroup] = first_tile ? inv_c2 * (double)acc[c] : o[(size_t)c * kTcGroup] + inv_c2 * (double)acc[c];
+          acc[c] = 0.f;
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < kTcGroup / 2; ++c) {
+          o[(size_t)c * kTcGroup] = first_tile ? inv_c2 * (double)acc[c] : o[(size_t)c * kTcGroup] + inv_c2 * (double)acc[c];
+          acc[c] = 0.f;
+        }
+      }
+      first_tile = false;
+      rows_in_acc = 0;
+    };
     bool pend = false;                       // a finished row is waiting for its flush
     unsigned pend_bar = 0, pend_par = 0, pend_tb = 0;
     auto flush_pending = [&]() {
@@ -306,6 +344,7 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
         for (int cc = 0; cc < 2; ++cc) tc_flush32(ta + 32u * cc, acc + 32 * cc);
       }
       pend = false;
+      if (++rows_in_acc == DIA_TC_FOLD_ROWS) fold();
     };
 #pragma unroll 1
     for (int i = 0; i < rows_here; ++i) {
@@ -314,6 +353,7 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
       for (int pass = 0; pass < n_pass; ++pass) {
         const unsigned sb = gst & 1u;
         if (gst >= 2) mbar_wait(bar0 + 8u * sb, ((gst >> 1) - 1u) & 1u);      // the MMAs of stage gst - 2 have read this buffer
+        TC_T(1);
         unsigned char* const op_hi = ops + sb * T::OP_BUF;
         if (my_bg)
           tc_build_row<true>(op_hi + my_off, op_hi + T::OP_TILE + my_off, T::LBO, etapow + bg_m * kTW, (pass ? Is : Hs) + i * kIPitch,
@@ -321,9 +361,11 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
         else if (my_valid)
           tc_build_row<false>(op_hi + my_off, op_hi + T::OP_TILE + my_off, T::LBO, Rs + (i + my_a) * G::RPITCH + my_b,
                               (pass ? Is : Hs) + i * kIPitch);
+        TC_T(2);
         fence_proxy_async();
         tc_fence_before();
         __syncthreads();
+        TC_T(3);
         if (tid == 0) {
           tc_fence_after();
           const unsigned base = smem_u32(op_hi);
@@ -340,7 +382,9 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
           }
           tc_commit(bar0 + 8u * sb);
         }
+        TC_T(4);
         if (pend) flush_pending();           // the previous row, while this stage's MMAs run
+        TC_T(5);
         if (pass == n_pass - 1) {
           pend = true;  pend_bar = bar0 + 8u * sb;  pend_par = (gst >> 1) & 1u;  pend_tb = grow & 1u;
           ++grow;
@@ -349,24 +393,9 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
       }
     }
     if (pend) flush_pending();
-    // fold the tile's float32 sums into this CTA's FP64 block [column][row]
-    {
-      double* o = outp + (size_t)((warp >> 2) * ncol) * kTcGroup + (warp & 3) * 32 + lane;
-      if (n_groups == 2) {
-#pragma unroll
-        for (int c = 0; c < kTcGroup; ++c) {
-          o[(size_t)c * kTcGroup] = first_tile ? inv_c2 * (double)acc[c] : o[(size_t)c * kTcGroup] + inv_c2 * (double)acc[c];
-          acc[c] = 0.f;
-        }
-      } else {
-#pragma unroll
-        for (int c = 0; c < kTcGroup / 2; ++c) {
-          o[(size_t)c * kTcGroup] = first_tile ? inv_c2 * (double)acc[c] : o[(size_t)c * kTcGroup] + inv_c2 * (double)acc[c];
-          acc[c] = 0.f;
-        }
-      }
-    }
-    first_tile = false;
+    TC_T(6);
+    if (rows_in_acc > 0) fold();
+    TC_T(7);
     tc_fence_before();
     __syncthreads();                         // tiles and flags free for the next tile
   }
