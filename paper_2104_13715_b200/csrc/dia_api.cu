@@ -11,6 +11,7 @@
 #include <new>
 #include <mutex>
 #include <string>
+#include <vector>
 
 #include "dia_eval.cuh"
 #include "dia_eval_small.cuh"
@@ -583,14 +584,24 @@ extern "C" int dia_hessian(dia_handle* h, const float* d_I, const unsigned char*
       if (ce != cudaSuccess) { cudaGetLastError(); return fail(h, DIA_ERR_ALLOC, std::string("hessian tensor-core workspace: ") + cudaGetErrorString(ce)); }
       w.tc_grid = tgrid;
     }
+    if (!w.tc_perm) {                        // slot -> parameter table (depends on m and the background degree only)
+      const int slots = (np + dia::kTcGroup - 1) / dia::kTcGroup * dia::kTcGroup;
+      int rpitch = 0, rh = 0;
+      geometry_for(h->cfg.m, &rpitch, &rh);
+      std::vector<short> perm((size_t)slots);
+      dia::hess_tc_make_perm(h->cfg.m, np, rpitch, perm.data());
+      cudaError_t ce = cudaMalloc(&w.tc_perm, sizeof(short) * (size_t)slots);
+      if (ce == cudaSuccess) ce = cudaMemcpy(w.tc_perm, perm.data(), sizeof(short) * (size_t)slots, cudaMemcpyHostToDevice);
+      if (ce != cudaSuccess) { cudaGetLastError(); cudaFree(w.tc_perm); w.tc_perm = nullptr; return fail(h, DIA_ERR_ALLOC, "hessian slot table"); }
+    }
     dia::EvalParams p;
     dia::TensorMaps tm;
     fill_params(h, 1, d_I, d_mask, d_var, d_theta, nullptr, &p, &tm, 0);
-    void* args[] = {(void*)&p, (void*)&w.tc_partials, (void*)&tct};
+    void* args[] = {(void*)&p, (void*)&w.tc_partials, (void*)&w.tc_perm, (void*)&tct};
     cudaError_t ce = cudaLaunchKernel(ktc, dim3(tgrid), dim3(dia::kThreads), args, hess_tc_smem_for(h->cfg.m), h->stream);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "hessian tensor-core launch");
     dia::hess_tc_reduce_kernel<<<dim3((dia::kTcRows * dia::kTcGroup + 255) / 256, tct.n_types), 256, 0, h->stream>>>(
-        w.tc_partials, tct, np, d_H);
+        w.tc_partials, w.tc_perm, tct, np, d_H);
   }
   const void* kblock = hess_kernel_for(h->cfg.m);
   const int bgrid = h->grid < h->tiles ? h->grid : h->tiles;

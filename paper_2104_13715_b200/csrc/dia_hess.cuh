@@ -15,10 +15,11 @@ struct HessWorkspace {
   double* chol = nullptr;      // [np][np] Cholesky factor of dia_covariance (L below, L' above the diagonal)
   double* tc_partials = nullptr;   // [CTAs][256][128] FP64 blocks of hess_tc_kernel (dia_hess_tc.cuh), allocated on first use
   int tc_grid = 0;             // CTAs those blocks were sized for
+  short* tc_perm = nullptr;    // [128 G] parameter of every operand slot of hess_tc_kernel (hess_tc_make_perm)
 };
 
 inline void hess_workspace_destroy(HessWorkspace* w) {
-  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->partials); cudaFree(w->chol); cudaFree(w->tc_partials);
+  cudaFree(w->loss); cudaFree(w->ident); cudaFree(w->partials); cudaFree(w->chol); cudaFree(w->tc_partials); cudaFree(w->tc_perm);
   *w = HessWorkspace();
 }
 

@@ -24,7 +24,10 @@
 //     deterministic.
 // The background rows (X = eta^m xi^n of Eq. 18-19, X = 1 for B0) are rows m^2 .. np - 1 of the same operand matrix, so
 // the whole of H comes from this one contraction and every entry carries the same (tiny) accumulator bias.
-// The 128-row groups of parameters g = 0 .. ceil(np / 128) - 1 give blocks (gi, gj) of H; by symmetry only
+// Operand row (slot) t of group g holds parameter perm[128 g + t] (hess_tc_make_perm): the slots are dealt so that the
+// 32 rows of a warp read 32 different shared-memory banks of the staged R tile when they build their operand rows
+// (in parameter order lanes 0 / 1 and 30 / 31 of most warps collide: 39 % of the wavefronts, ncu).
+// The 128-slot groups g = 0 .. ceil(np / 128) - 1 give blocks (gi, gj) of H; by symmetry only
 // gi <= gj are computed.  A CTA has one TYPE for its whole life (HessTcTypes): an operand tile of two row groups
 // [g0 | g1], an A operand (one of the two: 128 rows of D in TMEM lanes) and a B operand of one or two groups
 // (N = 128 or 256 columns of D), i.e. a diagonal block paired with an off-diagonal block that shares its rows, or a
@@ -148,6 +151,7 @@ __device__ long long g_tc_prof[16];
 
 template <int M>
 __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p, double* __restrict__ partials,
+                                                              const short* __restrict__ perm,
                                                               const __grid_constant__ HessTcTypes ty) {
   using G = Geo<M>;
   using T = TcGeo<M>;
@@ -178,8 +182,8 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
   const int g0 = ty.g0[type], g1 = ty.g1[type];
   const int a_sel = ty.a_sel[type], b_start = ty.b_start[type], n_groups = ty.n_groups[type];
   const int my_g = (tid >> 7) ? g1 : g0;
-  const int my_q = my_g * kTcGroup + (tid & (kTcGroup - 1));
-  const bool my_valid = my_g != 255 && my_q < p.np;
+  const int my_q = my_g != 255 ? (int)perm[my_g * kTcGroup + (tid & (kTcGroup - 1))] : -1;
+  const bool my_valid = my_q >= 0;
   const bool my_bg = my_valid && my_q >= M * M;                 // a background row: X = eta^bg_m xi^bg_n
   const int my_a = (my_valid && !my_bg) ? my_q / M : 0, my_b = (my_valid && !my_bg) ? my_q - (my_q / M) * M : 0;
   int bg_m = 0, bg_n = 0;
@@ -407,8 +411,8 @@ __global__ void __launch_bounds__(kThreads, 1) hess_tc_kernel(const EvalParams p
 #ifndef DIA_INST_M
 // Sums the FP64 blocks of the CTAs of each type in CTA order and writes the entries of H (both
 // triangles for an off-diagonal block; a diagonal block delivers both of its triangles itself).
-__global__ void hess_tc_reduce_kernel(const double* __restrict__ partials, const __grid_constant__ HessTcTypes ty, int np,
-                                      double* __restrict__ H) {
+__global__ void hess_tc_reduce_kernel(const double* __restrict__ partials, const short* __restrict__ perm,
+                                      const __grid_constant__ HessTcTypes ty, int np, double* __restrict__ H) {
   const int type = blockIdx.y;
   const int n_cols = kTcGroup * ty.n_groups[type];
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -416,13 +420,39 @@ __global__ void hess_tc_reduce_kernel(const double* __restrict__ partials, const
   const int n = idx / kTcGroup, r = idx - n * kTcGroup;
   const int gA = ty.a_sel[type] ? ty.g1[type] : ty.g0[type];
   const int gB = (ty.b_start[type] + n / kTcGroup) ? ty.g1[type] : ty.g0[type];
-  const int pr = gA * kTcGroup + r, qc = gB * kTcGroup + (n % kTcGroup);
-  if (pr >= np || qc >= np) return;
+  const int pr = perm[gA * kTcGroup + r], qc = perm[gB * kTcGroup + (n % kTcGroup)];
+  if (pr < 0 || qc < 0) return;
   double s = 0.0;
   for (int c = 0; c < ty.ctas_per_type; ++c)
     s += partials[(size_t)(c * ty.n_types + type) * (kTcRows * kTcGroup) + idx];
   H[(size_t)pr * np + qc] = s;
   if (gA != gB) H[(size_t)qc * np + pr] = s;
+}
+
+// perm[slot] for the 128 G slots (G = ceil(np / 128)), -1 for an empty slot: kernel pixel (a, b) reads the staged R tile
+// at a * r_pitch + b + const, so its bank class is (a * r_pitch + b) mod 32; each row goes to the first warp (32 slots)
+// that has no row of its class yet, background rows (no R reads) and leftovers fill the gaps.
+inline void hess_tc_make_perm(int m, int np, int r_pitch, short* perm) {
+  const int G = (np + kTcGroup - 1) / kTcGroup, n_warps = 4 * G;
+  for (int s = 0; s < G * kTcGroup; ++s) perm[s] = -1;
+  unsigned used[64 * 4] = {};                  // per warp: bank classes taken (G <= 64)
+  int fill[64 * 4] = {};
+  short late[kTcGroup * 64];
+  int n_late = 0;
+  for (int q = 0; q < np; ++q) {
+    int w = -1;
+    if (q < m * m) {
+      const unsigned bit = 1u << (((q / m) * r_pitch + q % m) & 31);
+      for (int c = 0; c < n_warps && w < 0; ++c)
+        if (fill[c] < 32 && !(used[c] & bit)) { w = c;  used[c] |= bit; }
+    }
+    if (w < 0) { late[n_late++] = (short)q;  continue; }
+    perm[32 * w + fill[w]++] = (short)q;
+  }
+  for (int k = 0, w = 0; k < n_late; ++k) {
+    while (fill[w] >= 32) ++w;
+    perm[32 * w + fill[w]++] = late[k];
+  }
 }
 
 // The types for np parameters: every diagonal block (i, i) paired with an off-diagonal block of its row or column
