@@ -543,7 +543,7 @@ def run_gpu(args):
                                        "path": "tcgen05 kind::f16, float16 hi/lo split (4 terms), FP32 in TMEM per tile row, "
                                                "FP64 per tile",
                                        "work_model": "2 np^2 flops per valid pixel"}
-            line["fits"]["covariance"] = {"ms": ms_c, "np": rows, "launches": rows + 3, "valid": ci[0],
+            line["fits"]["covariance"] = {"ms": ms_c, "np": rows, "launches": 2 * (-(-rows // 32)) + 3, "valid": ci[0],
                                           "sigma_P": ci[2], "sigma_B0": float(sig_hat[M * M])}
 
     # ---- small kernels on the same resident batch: the HBM side of the roofline

@@ -642,7 +642,7 @@ extern "C" int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, d
   const int np = h->np;
   dia::HessWorkspace& w = h->hess;
   if (!w.chol) {
-    cudaError_t ce = cudaMalloc(&w.chol, sizeof(double) * (size_t)np * np);
+    cudaError_t ce = cudaMalloc(&w.chol, sizeof(double) * ((size_t)np * np + dia::kCholPanel * dia::kCholPanel));   // + the panel's diagonal block
     if (ce == cudaSuccess)
       ce = cudaFuncSetAttribute(dia::cov_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)(sizeof(double) * dia::kSolveWarps * np));
@@ -653,10 +653,13 @@ extern "C" int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, d
     }
   }
   dia::cov_init_kernel<<<1, 1, 0, h->stream>>>(d_info);
-  for (int j = 0; j < np; ++j) {
-    const int rows = np - 1 - j;
-    const int grid = rows > 0 ? (rows + dia::kCholWarps - 1) / dia::kCholWarps : 1;
-    dia::chol_column_kernel<<<grid, dia::kCholWarps * 32, sizeof(double) * j, h->stream>>>(d_H, w.chol, np, j, d_info);
+  for (int j0 = 0; j0 < np; j0 += dia::kCholPanel) {          // blocked left-looking Cholesky: two launches per panel
+    const int nb = np - j0 < dia::kCholPanel ? np - j0 : dia::kCholPanel;
+    dia::chol_panel_update_kernel<<<(np - j0 + dia::kCholWarps - 1) / dia::kCholWarps, dia::kCholWarps * 32, 0, h->stream>>>(
+        d_H, w.chol, w.chol + (size_t)np * np, np, j0, nb);
+    const int below = np - j0 - nb;
+    dia::chol_panel_factor_kernel<<<below > 0 ? (below + dia::kCholWarps - 1) / dia::kCholWarps : 1, dia::kCholWarps * 32, 0,
+                                    h->stream>>>(w.chol, w.chol + (size_t)np * np, np, j0, nb, d_info);
   }
   dia::cov_solve_kernel<<<(np + 1 + dia::kSolveWarps - 1) / dia::kSolveWarps, dia::kSolveWarps * 32,
                           sizeof(double) * dia::kSolveWarps * np, h->stream>>>(w.chol, np, h->cfg.m * h->cfg.m, d_cov,

@@ -1,10 +1,15 @@
 // Kernels of dia_covariance (include/dia.h): covariance estimate Sigma = H^-1 of Eq. 16-17 with
 // the validity test of PAPER.md:193, all in FP64 on the device.
 //
-// H = L L' by a left-looking Cholesky factorisation, one launch per column (column j needs columns 0..j-1 complete;
-// inside a launch one warp owns one row i > j and forms the dot product of rows i and j of L).  A symmetric matrix is
-// positive definite -- every eigenvalue positive, hence a positive determinant: the two tests the paper lists --
-// exactly when every pivot d_j = H_jj - sum_k L_jk^2 is positive, so the pivots are the test (R20).
+// H = L L' by a blocked left-looking Cholesky factorisation, two launches per panel of kCholPanel = 32 columns (12
+// panels at np = 362, 70 at np = 2219; the unblocked form took one launch per column):
+//   chol_panel_update_kernel  one warp per row i >= j0: P[i][c] = H[i][j0+c] - sum_{k<j0} L[i][k] L[j0+c][k] for the 32
+//                             columns of the panel (the panel's rows of L staged through shared memory in chunks of k);
+//   chol_panel_factor_kernel  every CTA factorises the 32 x 32 diagonal block of P in shared memory (redundantly: it is
+//                             32 short steps), then one warp per row below solves l_i L_dd' = P_i.
+// A symmetric matrix is positive definite -- every eigenvalue positive, hence a positive determinant: the two tests
+// the paper lists -- exactly when every pivot d_j = H_jj - sum_k L_jk^2 is positive, so the pivots are the test
+// (R20).
 // L is stored in the lower triangle of the workspace W and L' in its upper triangle, so that both triangular solves
 // read rows.  Then one warp per right-hand side: y = L^-1 e_k (forward), sigma_k = |y| (Sigma_kk = e_k' L^-T L^-1 e_k),
 // x = L^-T y (backward) = row k of Sigma; one more warp solves for u (1 on the kernel pixels, Eq. 3) and gives
@@ -16,7 +21,7 @@
 
 namespace dia {
 
-constexpr int kCholWarps = 8;    // rows per CTA in chol_column_kernel
+constexpr int kCholWarps = 8;    // rows per CTA in the Cholesky kernels
 constexpr int kSolveWarps = 2;   // right-hand sides per CTA in cov_solve_kernel
 constexpr int kCovInfo = 5;      // valid, ln det H, sigma_P, smallest pivot, first non-positive pivot (-1: none)
 
@@ -24,37 +29,115 @@ __global__ void cov_init_kernel(double* __restrict__ info) {
   info[0] = 1.0;  info[1] = 0.0;  info[2] = 0.0;  info[3] = INFINITY;  info[4] = -1.0;
 }
 
-// column j of L.  grid: ceil((np - 1 - j) / kCholWarps) CTAs (at least one), kCholWarps warps; smem: j doubles
+constexpr int kCholPanel = 32;   // columns per panel
+constexpr int kCholChunk = 128;  // k values of the panel's rows staged per pass of the update kernel
+
+// P[i][c] for rows i >= j0 and the nb columns of the panel: the rows below the diagonal block are written over
+// W[i][j0+c], the block itself (c <= i - j0) goes to `diag` [kCholPanel][kCholPanel] -- every CTA of the factor
+// kernel reads it while CTA 0 writes the factorised block into W.
+// grid: ceil((np - j0) / kCholWarps) CTAs of kCholWarps warps; smem: kCholPanel x kCholChunk doubles.
 __global__ void __launch_bounds__(kCholWarps * 32)
-chol_column_kernel(const double* __restrict__ H, double* __restrict__ W, int np, int j, double* __restrict__ info) {
-  extern __shared__ double rowj[];
+chol_panel_update_kernel(const double* __restrict__ H, double* __restrict__ W, double* __restrict__ diag, int np, int j0,
+                         int nb) {
+  __shared__ double S[kCholPanel][kCholChunk + 1];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const double* Wj = W + (size_t)j * np;
-  for (int k = threadIdx.x; k < j; k += blockDim.x) rowj[k] = Wj[k];
-  __syncthreads();
-  double s = 0.0;
-  for (int k = lane; k < j; k += 32) s = fma(rowj[k], rowj[k], s);
-  const double d = H[(size_t)j * np + j] - warp_sum_f64(s);   // the same value in every warp of every CTA
-  const double ljj = sqrt(d);                                  // NaN from here on if d < 0: info[0] says so
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    W[(size_t)j * np + j] = ljj;
-    if (!(d > 0.0) || !isfinite(d)) {
-      if (info[4] < 0.0) info[4] = (double)j;
-      info[0] = 0.0;
+  const int i = j0 + blockIdx.x * kCholWarps + warp;
+  const bool live = i < np;
+  const double* Wi = W + (size_t)(live ? i : j0) * np;
+  double t[kCholPanel];
+#pragma unroll
+  for (int c = 0; c < kCholPanel; ++c) t[c] = 0.0;
+  for (int k0 = 0; k0 < j0; k0 += kCholChunk) {
+    const int kn = min(kCholChunk, j0 - k0);
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < kCholPanel * kCholChunk; idx += blockDim.x) {
+      const int c = idx / kCholChunk, k = idx - c * kCholChunk;
+      S[c][k] = (c < nb && k < kn) ? W[(size_t)(j0 + c) * np + k0 + k] : 0.0;
     }
-    info[1] += log(d);
-    if (d < info[3]) info[3] = d;                              // NaN pivots after a failure leave it alone
+    __syncthreads();
+    for (int k = lane; k < kn; k += 32) {
+      const double a = Wi[k0 + k];
+#pragma unroll
+      for (int c = 0; c < kCholPanel; ++c) t[c] = fma(a, S[c][k], t[c]);
+    }
   }
-  const int i = j + 1 + blockIdx.x * kCholWarps + warp;
+#pragma unroll
+  for (int c = 0; c < kCholPanel; ++c) t[c] = warp_sum_f64(t[c]);
+  if (!live) return;
+  double mine = 0.0;                                  // lane c keeps column c
+#pragma unroll
+  for (int c = 0; c < kCholPanel; ++c) if (lane == c) mine = t[c];
+  if (lane < nb && j0 + lane <= i) {
+    const double v = H[(size_t)i * np + j0 + lane] - mine;
+    if (i < j0 + nb) diag[(i - j0) * kCholPanel + lane] = v;
+    else W[(size_t)i * np + j0 + lane] = v;
+  }
+}
+
+// Factorises the diagonal block of the panel and solves the rows below it.  grid: max(1, ceil((np - j0 - nb) /
+// kCholWarps)) CTAs of kCholWarps warps.  CTA 0 writes the block itself and the pivots' record.
+__global__ void __launch_bounds__(kCholWarps * 32)
+chol_panel_factor_kernel(double* __restrict__ W, const double* __restrict__ diag, int np, int j0, int nb,
+                         double* __restrict__ info) {
+  __shared__ double D[kCholPanel][kCholPanel + 1];
+  __shared__ double piv[kCholPanel];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int idx = threadIdx.x; idx < kCholPanel * kCholPanel; idx += blockDim.x) {
+    const int r = idx / kCholPanel, c = idx - r * kCholPanel;
+    D[r][c] = (r < nb && c <= r) ? diag[r * kCholPanel + c] : 0.0;
+  }
+  __syncthreads();
+  if (warp == 0) {                                    // lane r owns row r of the block
+    for (int c = 0; c < nb; ++c) {
+      double s = 0.0;
+      for (int k = 0; k < c; ++k) s = fma(D[c][k], D[c][k], s);
+      const double d = D[c][c] - s;                   // the same value in every lane
+      const double lcc = sqrt(d);                     // NaN from here on if d < 0: info[0] says so
+      double v = 0.0;
+      if (lane > c && lane < nb) {
+        double tt = 0.0;
+        for (int k = 0; k < c; ++k) tt = fma(D[lane][k], D[c][k], tt);
+        v = (D[lane][c] - tt) / lcc;
+      }
+      __syncwarp();
+      if (lane == c) { D[c][c] = lcc;  piv[c] = d; }
+      if (lane > c && lane < nb) D[lane][c] = v;
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  if (blockIdx.x == 0) {
+    for (int idx = threadIdx.x; idx < nb * nb; idx += blockDim.x) {
+      const int r = idx / nb, c = idx - r * nb;
+      if (c <= r) {
+        W[(size_t)(j0 + r) * np + j0 + c] = D[r][c];
+        W[(size_t)(j0 + c) * np + j0 + r] = D[r][c];
+      }
+    }
+    if (threadIdx.x == 0) {
+      for (int c = 0; c < nb; ++c) {
+        const double d = piv[c];
+        if (!(d > 0.0) || !isfinite(d)) {
+          if (info[4] < 0.0) info[4] = (double)(j0 + c);
+          info[0] = 0.0;
+        }
+        info[1] += log(d);
+        if (d < info[3]) info[3] = d;                 // NaN pivots after a failure leave it alone
+      }
+    }
+  }
+  const int i = j0 + nb + blockIdx.x * kCholWarps + warp;
   if (i >= np) return;
-  const double* Wi = W + (size_t)i * np;
-  double t = 0.0;
-  for (int k = lane; k < j; k += 32) t = fma(Wi[k], rowj[k], t);
-  t = warp_sum_f64(t);
-  if (lane == 0) {
-    const double l = (H[(size_t)i * np + j] - t) / ljj;
-    W[(size_t)i * np + j] = l;
-    W[(size_t)j * np + i] = l;
+  double* Wi = W + (size_t)i * np + j0;
+  const double pc = lane < nb ? Wi[lane] : 0.0;       // P[i][lane]
+  double l = 0.0;                                     // l[lane] once column lane is done
+  for (int c = 0; c < nb; ++c) {
+    const double t = warp_sum_f64((lane < c) ? l * D[c][lane] : 0.0);
+    if (lane == c) l = (pc - t) / D[c][c];
+  }
+  if (lane < nb) {
+    Wi[lane] = l;
+    W[(size_t)(j0 + lane) * np + i] = l;
   }
 }
 
