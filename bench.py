@@ -12,7 +12,7 @@ weights -> kernel gradient -> block partials), the FP64 second-level reduction, 
 step and its convergence bookkeeping, for all 16 epochs inside one CUDA-graph launch.
   metric / value : loss+gradient evaluations per second (one evaluation = one epoch, 4096^2, m = 19),
                    counted from the n_evals the device reports, inputs resident in HBM
-  e2e            : the same through Handle.fit_host -- pinned host I / theta0 copied in, theta-hat and the
+  e2e            : the same through dia_fit_host (C ABI; Handle.fit_host marshals) -- pinned host I / theta0 copied in, theta-hat and the
                    result structs copied out, inside the timed region
   roofline       : the fused kernel against the FP32 FMA pipe ("alu"); its launch duration is measured with
                    CUDA events around back-to-back dia_eval_loss_grad launches of the same batch

@@ -157,6 +157,23 @@ int dia_hessian(dia_handle* h, const float* d_I, const unsigned char* d_mask, co
  * allocates an np x np workspace (synchronises once); later calls are asynchronous on the handle's stream. */
 int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, double* d_sigma, double* d_info);
 
+/* Host-buffer forms of dia_eval_loss_grad and dia_fit: the same operations for callers whose data live in HOST memory
+ * (page-locked buffers make the copies asynchronous; pageable ones work, slower).  The library owns the device staging
+ * buffers (allocated on first use for cfg->max_epochs epochs, freed by dia_destroy) and a copy stream; both calls
+ * SYNCHRONISE before they return, and the host outputs are complete then.  Plain noise model only (no d_var).
+ *   dia_eval_loss_grad_host: h_I [n_epochs][n_rows][n_cols], h_theta [n_epochs][np] in; h_loss [n_epochs],
+ *     h_grad [n_epochs][np] out.
+ *   dia_fit_host: h_theta holds theta0 on entry and theta-hat on exit, h_result [n_epochs] out, h_mask NULL or
+ *     [n_epochs][n_rows][n_cols].  The batch is cut into `chunks` groups of epochs (0 = default: 4 when there are at
+ *     least 8 epochs, else 1): the copy of group k+1 runs on the copy stream while group k is being fitted, so only the
+ *     first copy is exposed; the groups are fitted by dia_fit one after the other, which gives the same result per
+ *     epoch as one dia_fit over the whole batch.
+ * Errors: as dia_eval_loss_grad / dia_fit, ALLOC for the staging buffers, UNSUPPORTED with DIA_NOISE_FIXED. */
+int dia_eval_loss_grad_host(dia_handle* h, int n_epochs, const float* h_I, const float* h_theta,
+                            double* h_loss, double* h_grad);
+int dia_fit_host(dia_handle* h, const dia_fit_opts* opts, int n_epochs, const float* h_I,
+                 const unsigned char* h_mask, float* h_theta, dia_fit_result* h_result, int chunks);
+
 /* Difference image and fit-quality metrics for n_epochs targets at the given theta (the science product,
  * PAPER.md:20; metrics of Eq. 29-30):
  *   D_ij = I_ij - M_ij on the valid region V (mask or not), 0 outside V;

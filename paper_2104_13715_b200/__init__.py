@@ -18,6 +18,8 @@ from .binding import (  # noqa: F401
     dia_eval_loss_grad_static,
     STATIC_SCRATCH_BYTES,
     dia_fit,
+    dia_fit_host,
+    dia_eval_loss_grad_host,
     dia_measure_fp32_peak,
     dia_measure_fp32_pattern,
     dia_tc_probe_gemm,

@@ -21,7 +21,7 @@ FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "no
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
                     "dia_measure_fp32_peak", "dia_measure_fp32_pattern", "dia_difference_image", "dia_hessian", "dia_covariance",
-                    "dia_eval_loss_grad_static", "dia_tc_probe_gemm")
+                    "dia_eval_loss_grad_static", "dia_tc_probe_gemm", "dia_eval_loss_grad_host", "dia_fit_host")
 STATIC_SCRATCH_BYTES = 4 << 20          # DIA_STATIC_SCRATCH_BYTES of include/dia.h
 
 
@@ -100,6 +100,8 @@ def load_library(build_if_missing: bool = True):
     lib.dia_get_info.argtypes = [C.c_void_p] + [C.POINTER(C.c_int)] * 4
     lib.dia_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     lib.dia_measure_fp32_pattern.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+    lib.dia_eval_loss_grad_host.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 4
+    lib.dia_fit_host.argtypes = [C.c_void_p, C.POINTER(FitOpts), C.c_int] + [C.c_void_p] * 4 + [C.c_int]
     lib.dia_tc_probe_gemm.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]
     _LIB = lib
     return lib
@@ -178,6 +180,26 @@ def dia_tc_probe_gemm(d_A: torch.Tensor, d_B: torch.Tensor, mode: int) -> torch.
     _check(lib.dia_tc_probe_gemm(None, _dptr(d_A, torch.float32, "d_A"), _dptr(d_B, torch.float32, "d_B"),
                                  _dptr(d_D, torch.float32, "d_D"), K, N, mode))
     return d_D
+
+
+def _hptr(t: Optional[torch.Tensor], dtype, what: str):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise DiaError(f"{what} must be a contiguous HOST tensor of dtype {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def dia_eval_loss_grad_host(handle: int, n_epochs: int, h_I, h_theta, h_loss, h_grad) -> None:
+    lib = load_library()
+    _check(lib.dia_eval_loss_grad_host(handle, n_epochs, _hptr(h_I, torch.float32, "h_I"), _hptr(h_theta, torch.float32, "h_theta"),
+                                       _hptr(h_loss, torch.float64, "h_loss"), _hptr(h_grad, torch.float64, "h_grad")), handle)
+
+
+def dia_fit_host(handle: int, opts: FitOpts, n_epochs: int, h_I, h_mask, h_theta, h_result, chunks: int = 0) -> None:
+    lib = load_library()
+    _check(lib.dia_fit_host(handle, C.byref(opts), n_epochs, _hptr(h_I, torch.float32, "h_I"), _hptr(h_mask, torch.uint8, "h_mask"),
+                            _hptr(h_theta, torch.float32, "h_theta"), _hptr(h_result, torch.uint8, "h_result"), chunks), handle)
 
 
 def dia_fit(handle: int, opts: FitOpts, n_epochs: int, d_I, d_mask, d_var, d_theta, d_result) -> None:
@@ -321,19 +343,13 @@ class Handle:
                for i in range(E)]
         return theta, out
 
-    # ---- host-buffer entry points: the same C-ABI calls with the host<->device copies around them
-    def _staging(self, E: int, dev, want_mask: bool):
-        key = (E, want_mask)
-        if getattr(self, "_stage_key", None) != key:
-            self._stage_key = key
-            self._dI = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.float32, device=dev)
-            self._dth = torch.empty((E, self.np), dtype=torch.float32, device=dev)
-            self._dmask = torch.empty((E, self.n_rows, self.n_cols), dtype=torch.uint8, device=dev) if want_mask else None
-            self._dres = torch.zeros(E * C.sizeof(FitResult), dtype=torch.uint8, device=dev)
+    # ---- host-buffer entry points: dia_fit_host / dia_eval_loss_grad_host of the C ABI (staging buffers, copy
+    # stream and the chunked copy / fit overlap live in the library); only the pinned OUTPUT buffers are kept here
+    def _host_out(self, E: int):
+        if getattr(self, "_host_E", None) != E:
+            self._host_E = E
             self._hres = torch.empty(E * C.sizeof(FitResult), dtype=torch.uint8).pin_memory()
             self._hth = torch.empty((E, self.np), dtype=torch.float32).pin_memory()
-            self._dloss = torch.empty(E, dtype=torch.float64, device=dev)
-            self._dgrad = torch.empty((E, self.np), dtype=torch.float64, device=dev)
             self._hloss = torch.empty(E, dtype=torch.float64).pin_memory()
             self._hgrad = torch.empty((E, self.np), dtype=torch.float64).pin_memory()
 
@@ -352,67 +368,31 @@ class Handle:
 
     def fit_host(self, I_host: torch.Tensor, theta0_host: torch.Tensor, opts: Optional[FitOpts] = None,
                  mask_host: Optional[torch.Tensor] = None, chunks: Optional[int] = None):
-        """dia_fit with HOST inputs and outputs (pinned tensors make the copies asynchronous): copies I, theta0
-        (and the mask) to the device, fits, copies theta-hat and the result structs back and synchronises.
-        The batch is cut into `chunks` groups of epochs (default 4 when there are at least 8 epochs): the copy of
-        group k+1 runs on a second stream while group k is being fitted, so only the first copy is exposed.
+        """dia_fit_host: dia_fit with HOST inputs and outputs (pinned tensors make the copies asynchronous).  The
+        library copies I, theta0 (and the mask) to its staging buffers in `chunks` groups of epochs (default 4 when
+        there are at least 8 epochs) on a second stream while the previous group is being fitted, copies theta-hat and
+        the result structs back and synchronises.
         Returns (theta_hat [E][np] float32 host tensor, list[FitResult], bytes host->device, bytes device->host);
-        theta_hat is a copy (the pinned staging buffers are reused by the next call)."""
+        theta_hat is a copy (the pinned output buffers are reused by the next call)."""
         E = 1 if I_host.dim() == 2 else I_host.shape[0]
-        dev = self.R.device
-        self._staging(E, dev, mask_host is not None)
+        self._host_out(E)
         opts = opts or FitOpts.default()
-        if chunks is None:
-            chunks = 4 if E >= 8 else 1
-        chunks = max(1, min(chunks, E))
-        bounds = [(k * E) // chunks for k in range(chunks + 1)]
-        hI = I_host.reshape(self._dI.shape)
-        hth = theta0_host.reshape(E, self.np)
-        hmask = None if mask_host is None else mask_host.reshape(self._dmask.shape)
+        self._hth.copy_(theta0_host.reshape(E, self.np))            # in: theta0, out: theta-hat
+        dia_fit_host(self._h, opts, E, I_host, mask_host, self._hth, self._hres, 0 if chunks is None else chunks)
         nres = C.sizeof(FitResult)
-        if getattr(self, "_copy_stream", None) is None:
-            self._copy_stream = torch.cuda.Stream(device=dev)
-        with self._stream_ctx():
-            fit_stream = torch.cuda.current_stream()
-            self._copy_stream.wait_stream(fit_stream)            # staging buffers are free again
-            ready = []
-            with torch.cuda.stream(self._copy_stream):
-                for k in range(chunks):
-                    a, b = bounds[k], bounds[k + 1]
-                    self._dI[a:b].copy_(hI[a:b], non_blocking=True)
-                    self._dth[a:b].copy_(hth[a:b], non_blocking=True)
-                    if hmask is not None:
-                        self._dmask[a:b].copy_(hmask[a:b], non_blocking=True)
-                    ev = torch.cuda.Event()
-                    ev.record()
-                    ready.append(ev)
-            for k in range(chunks):
-                a, b = bounds[k], bounds[k + 1]
-                fit_stream.wait_event(ready[k])
-                dia_fit(self._h, opts, b - a, self._dI[a:b], None if hmask is None else self._dmask[a:b], None,
-                        self._dth[a:b], self._dres[a * nres:b * nres])
-            self._hth.copy_(self._dth, non_blocking=True)
-            self._hres.copy_(self._dres, non_blocking=True)
-            fit_stream.synchronize()
         raw = self._hres.numpy().tobytes()
         res = [FitResult.from_buffer_copy(raw[i * nres:(i + 1) * nres]) for i in range(E)]
-        h2d = self._dI.numel() * 4 + self._dth.numel() * 4 + (self._dmask.numel() if mask_host is not None else 0)
+        h2d = I_host.numel() * 4 + self._hth.numel() * 4 + (mask_host.numel() if mask_host is not None else 0)
         d2h = self._hth.numel() * 4 + self._hres.numel()
         return self._hth.clone(), res, h2d, d2h
 
     def eval_loss_grad_host(self, I_host: torch.Tensor, theta_host: torch.Tensor):
-        """dia_eval_loss_grad with HOST inputs and outputs; returns (loss, grad, bytes h2d, bytes d2h); loss and grad
-        are copies (the pinned staging buffers are reused by the next call)."""
+        """dia_eval_loss_grad_host: dia_eval_loss_grad with HOST inputs and outputs; returns (loss, grad, bytes h2d,
+        bytes d2h); loss and grad are copies (the pinned output buffers are reused by the next call)."""
         E = 1 if I_host.dim() == 2 else I_host.shape[0]
-        self._staging(E, self.R.device, False)
-        with self._stream_ctx():
-            self._dI.copy_(I_host.reshape(self._dI.shape), non_blocking=True)
-            self._dth.copy_(theta_host.reshape(E, self.np), non_blocking=True)
-            dia_eval_loss_grad(self._h, E, self._dI, None, None, self._dth, self._dloss, self._dgrad)
-            self._hloss.copy_(self._dloss, non_blocking=True)
-            self._hgrad.copy_(self._dgrad, non_blocking=True)
-            torch.cuda.current_stream().synchronize()
-        return (self._hloss.clone(), self._hgrad.clone(), self._dI.numel() * 4 + self._dth.numel() * 4,
+        self._host_out(E)
+        dia_eval_loss_grad_host(self._h, E, I_host, theta_host, self._hloss, self._hgrad)
+        return (self._hloss.clone(), self._hgrad.clone(), I_host.numel() * 4 + theta_host.numel() * 4,
                 self._hloss.numel() * 8 + self._hgrad.numel() * 8)
 
     def close(self):

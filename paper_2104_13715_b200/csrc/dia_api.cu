@@ -41,6 +41,13 @@ struct dia_handle {
   double* d_partials;      // [max_epochs][np+1][min(tiles, grid)]
   dia::FitWorkspace fit;   // device optimiser state + cached graph
   dia::HessWorkspace hess; // dia_hessian scratch, allocated on first use
+  struct HostPath {        // device staging of the host-buffer entry points (dia_*_host), allocated on first use
+    float* dI = nullptr;  float* dth = nullptr;  unsigned char* dmask = nullptr;  dia_fit_result* dres = nullptr;
+    double* dloss = nullptr;  double* dgrad = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ready[16] = {};          // chunk k has arrived
+    cudaEvent_t free_ev = nullptr;       // the staging buffers are free again
+  } host;
   std::string err;
 };
 
@@ -490,6 +497,15 @@ extern "C" int dia_create(const dia_config* cfg, const float* d_R, dia_handle** 
   return DIA_OK;
 }
 
+static void host_path_destroy(dia_handle* h) {
+  dia_handle::HostPath& hp = h->host;
+  cudaFree(hp.dI); cudaFree(hp.dth); cudaFree(hp.dmask); cudaFree(hp.dres); cudaFree(hp.dloss); cudaFree(hp.dgrad);
+  for (cudaEvent_t& e : hp.ready) if (e) cudaEventDestroy(e);
+  if (hp.free_ev) cudaEventDestroy(hp.free_ev);
+  if (hp.copy_stream) cudaStreamDestroy(hp.copy_stream);
+  hp = dia_handle::HostPath();
+}
+
 extern "C" int dia_destroy(dia_handle* h) {
   if (!h) return DIA_ERR_INVALID_ARG;
   cudaStreamSynchronize(h->stream);
@@ -500,6 +516,7 @@ extern "C" int dia_destroy(dia_handle* h) {
     cudaFree(h->d_const_stage);
     const_slot_release(h->cfg.m);
   }
+  host_path_destroy(h);
   delete h;
   return DIA_OK;
 }
@@ -763,6 +780,98 @@ extern "C" int dia_measure_fp32_pattern(void* stream, int pattern, double* fma_p
   const double v = dia::measure_fp32_pattern((cudaStream_t)stream, pattern, 5);
   if (v <= 0.0) { cudaGetLastError(); return fail(nullptr, DIA_ERR_CUDA, "FP32 probe failed (no CUDA device?)"); }
   *fma_per_second = v;
+  return DIA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-buffer entry points (include/dia.h): copies on a second stream, the device calls above in between
+// ---------------------------------------------------------------------------------------------
+static int host_path_prepare(dia_handle* h, bool want_mask) {
+  dia_handle::HostPath& hp = h->host;
+  const size_t E = (size_t)h->cfg.max_epochs, npix = (size_t)h->cfg.n_rows * h->cfg.n_cols, np = (size_t)h->np;
+  cudaError_t ce = cudaSuccess;
+  if (!hp.dI) {
+    ce = cudaMalloc(&hp.dI, sizeof(float) * E * npix);
+    if (ce == cudaSuccess) ce = cudaMalloc(&hp.dth, sizeof(float) * E * np);
+    if (ce == cudaSuccess) ce = cudaMalloc(&hp.dres, sizeof(dia_fit_result) * E);
+    if (ce == cudaSuccess) ce = cudaMalloc(&hp.dloss, sizeof(double) * E);
+    if (ce == cudaSuccess) ce = cudaMalloc(&hp.dgrad, sizeof(double) * E * np);
+    if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&hp.copy_stream, cudaStreamNonBlocking);
+    for (cudaEvent_t& e : hp.ready) if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&hp.free_ev, cudaEventDisableTiming);
+  }
+  if (ce == cudaSuccess && want_mask && !hp.dmask) ce = cudaMalloc(&hp.dmask, E * npix);
+  if (ce != cudaSuccess) {
+    cudaGetLastError();
+    host_path_destroy(h);
+    return fail(h, DIA_ERR_ALLOC, std::string("host-path staging buffers: ") + cudaGetErrorString(ce));
+  }
+  return DIA_OK;
+}
+
+extern "C" int dia_eval_loss_grad_host(dia_handle* h, int n_epochs, const float* h_I, const float* h_theta, double* h_loss,
+                                       double* h_grad) {
+  if (!h) return DIA_ERR_INVALID_ARG;
+  if (n_epochs < 1 || n_epochs > h->cfg.max_epochs) return fail(h, DIA_ERR_INVALID_ARG, "n_epochs out of range");
+  if (!h_I || !h_theta || !h_loss || !h_grad) return fail(h, DIA_ERR_INVALID_ARG, "null host buffer");
+  if (h->cfg.noise == DIA_NOISE_FIXED) return fail(h, DIA_ERR_UNSUPPORTED, "the host-buffer calls take no variance map");
+  int rc = host_path_prepare(h, false);
+  if (rc != DIA_OK) return rc;
+  dia_handle::HostPath& hp = h->host;
+  const size_t npix = (size_t)h->cfg.n_rows * h->cfg.n_cols, np = (size_t)h->np, E = (size_t)n_epochs;
+  cudaError_t ce = cudaMemcpyAsync(hp.dI, h_I, sizeof(float) * E * npix, cudaMemcpyHostToDevice, h->stream);
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(hp.dth, h_theta, sizeof(float) * E * np, cudaMemcpyHostToDevice, h->stream);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "host to device copy");
+  rc = dia_eval_loss_grad(h, n_epochs, hp.dI, nullptr, nullptr, hp.dth, hp.dloss, hp.dgrad);
+  if (rc != DIA_OK) return rc;
+  ce = cudaMemcpyAsync(h_loss, hp.dloss, sizeof(double) * E, cudaMemcpyDeviceToHost, h->stream);
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(h_grad, hp.dgrad, sizeof(double) * E * np, cudaMemcpyDeviceToHost, h->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "device to host copy");
+  return DIA_OK;
+}
+
+extern "C" int dia_fit_host(dia_handle* h, const dia_fit_opts* opts, int n_epochs, const float* h_I,
+                            const unsigned char* h_mask, float* h_theta, dia_fit_result* h_result, int chunks) {
+  if (!h) return DIA_ERR_INVALID_ARG;
+  if (n_epochs < 1 || n_epochs > h->cfg.max_epochs) return fail(h, DIA_ERR_INVALID_ARG, "n_epochs out of range");
+  if (!opts || !h_I || !h_theta || !h_result) return fail(h, DIA_ERR_INVALID_ARG, "null opts or host buffer");
+  if (h->cfg.noise == DIA_NOISE_FIXED) return fail(h, DIA_ERR_UNSUPPORTED, "the host-buffer calls take no variance map");
+  int rc = host_path_prepare(h, h_mask != nullptr);
+  if (rc != DIA_OK) return rc;
+  dia_handle::HostPath& hp = h->host;
+  const size_t npix = (size_t)h->cfg.n_rows * h->cfg.n_cols, np = (size_t)h->np;
+  const int max_chunks = (int)(sizeof(hp.ready) / sizeof(hp.ready[0]));
+  if (chunks <= 0) chunks = n_epochs >= 8 ? 4 : 1;
+  if (chunks > n_epochs) chunks = n_epochs;
+  if (chunks > max_chunks) chunks = max_chunks;
+  // the copy stream starts when everything enqueued on the handle's stream so far (a previous user of the staging
+  // buffers) is done
+  cudaError_t ce = cudaEventRecord(hp.free_ev, h->stream);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(hp.copy_stream, hp.free_ev, 0);
+  for (int k = 0; k < chunks && ce == cudaSuccess; ++k) {
+    const size_t a = (size_t)k * n_epochs / chunks, b = (size_t)(k + 1) * n_epochs / chunks;
+    ce = cudaMemcpyAsync(hp.dI + a * npix, h_I + a * npix, sizeof(float) * (b - a) * npix, cudaMemcpyHostToDevice, hp.copy_stream);
+    if (ce == cudaSuccess)
+      ce = cudaMemcpyAsync(hp.dth + a * np, h_theta + a * np, sizeof(float) * (b - a) * np, cudaMemcpyHostToDevice, hp.copy_stream);
+    if (ce == cudaSuccess && h_mask)
+      ce = cudaMemcpyAsync(hp.dmask + a * npix, h_mask + a * npix, (b - a) * npix, cudaMemcpyHostToDevice, hp.copy_stream);
+    if (ce == cudaSuccess) ce = cudaEventRecord(hp.ready[k], hp.copy_stream);
+  }
+  if (ce != cudaSuccess) { cudaStreamSynchronize(hp.copy_stream); return cuda_fail(h, ce, "host to device copy"); }
+  for (int k = 0; k < chunks; ++k) {
+    const size_t a = (size_t)k * n_epochs / chunks, b = (size_t)(k + 1) * n_epochs / chunks;
+    ce = cudaStreamWaitEvent(h->stream, hp.ready[k], 0);
+    if (ce != cudaSuccess) { cudaStreamSynchronize(hp.copy_stream); return cuda_fail(h, ce, "stream wait"); }
+    rc = dia_fit(h, opts, (int)(b - a), hp.dI + a * npix, h_mask ? hp.dmask + a * npix : nullptr, nullptr, hp.dth + a * np,
+                 hp.dres + a);
+    if (rc != DIA_OK) { cudaStreamSynchronize(hp.copy_stream); cudaStreamSynchronize(h->stream); return rc; }
+  }
+  ce = cudaMemcpyAsync(h_theta, hp.dth, sizeof(float) * (size_t)n_epochs * np, cudaMemcpyDeviceToHost, h->stream);
+  if (ce == cudaSuccess)
+    ce = cudaMemcpyAsync(h_result, hp.dres, sizeof(dia_fit_result) * (size_t)n_epochs, cudaMemcpyDeviceToHost, h->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "device to host copy");
   return DIA_OK;
 }
 

@@ -274,8 +274,9 @@ def test_fit_constant_bank_graph_matches_shared_memory_graph(dia, monkeypatch):
 
 
 def test_fit_host_chunked_pipeline_matches_device_fit(dia):
-    """Handle.fit_host cuts the batch into groups whose host->device copies overlap the fit of the previous
-    group; the fitted parameters must equal those of one device-resident dia_fit over the whole batch."""
+    """dia_fit_host (C ABI; Handle.fit_host marshals) cuts the batch into groups whose host->device copies overlap the
+    fit of the previous group; the fitted parameters must equal those of one device-resident dia_fit over the whole
+    batch.  dia_eval_loss_grad_host likewise against dia_eval_loss_grad, with pageable host memory too."""
     w = make_workload(4, n=200, n_epochs=9, m=7)
     og = dia.FitOpts.default(force_adam_iters=40, force_lbfgs_iters=10)
     h = dia.Handle(_dev(w.R), w.m, max_epochs=9, sigma0=w.sigma0, gain=w.gain)
@@ -286,6 +287,16 @@ def test_fit_host_chunked_pipeline_matches_device_fit(dia):
         assert torch.equal(thh, thd.cpu())
         assert [r.n_evals for r in rh] == [r.n_evals for r in rd] and [r.loss for r in rh] == [r.loss for r in rd]
         assert h2d == w.I.nbytes + w.theta0.nbytes
+    Ld, gd = h.eval_loss_grad(_dev(w.I), _dev(w.theta0))
+    for hI2, hth2 in ((hI, hth), (torch.from_numpy(w.I.copy()), torch.from_numpy(w.theta0.copy()))):     # pinned, pageable
+        Lh, gh, _, d2h = h.eval_loss_grad_host(hI2, hth2)
+        assert torch.equal(Lh, Ld.cpu()) and torch.equal(gh, gd.cpu()) and d2h == 8 * (9 + 9 * 50)
+    Lh, gh, _, _ = h.eval_loss_grad_host(hI[:2], hth[:2])                            # fewer epochs than max_epochs
+    assert torch.equal(Lh, Ld.cpu()[:2]) and torch.equal(gh, gd.cpu()[:2])
+    mask = (np.random.default_rng(1).random(w.I.shape) > 0.01).astype(np.uint8)
+    thm, rm = h.fit(_dev(w.I), _dev(w.theta0), og, mask=_dev(mask))
+    thh, rh, h2d, _ = h.fit_host(hI, hth, og, mask_host=torch.from_numpy(mask).pin_memory())
+    assert torch.equal(thh, thm.cpu()) and h2d == w.I.nbytes + w.theta0.nbytes + mask.nbytes
     h.close()
 
 
