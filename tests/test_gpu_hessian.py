@@ -46,11 +46,12 @@ def _sigmas(H, nk):
 
 
 @pytest.mark.parametrize("c,n,m,E", [(0, None, None, 16), (1, 256, 15, 16), (4, 192, 19, 1), (4, 333, 11, 7),
-                                     (0, 100, 3, 4), (0, 72, 1, 2)])
+                                     (0, 90, 5, 1), (0, 100, 3, 4), (0, 72, 1, 2)])
 def test_hessian_plain_objective(dia, c, n, m, E):
     """Gaussian loss, noise model of Eq. 6, at the fitted theta (the MLE of Eq. 15); max_epochs = 1 walks the
-    single-launch path, 333 the cp.async staging path and a chunk size that does not divide 2 np; m = 3 and m = 1 are
-    handles whose evaluations run eval_small_kernel while the Hessian takes the block kernel and the fused kernel."""
+    single-launch path, 333 the cp.async staging path and a chunk size that does not divide 2 np; m >= 5 takes the
+    tensor-core kernel (m = 5: 26 of its 128 operand rows in use), m = 3 and m = 1 are handles whose evaluations run
+    eval_small_kernel while the Hessian takes the block kernel and the fused kernel."""
     w = make_workload(c, n=n, m=m, n_epochs=1)
     cfg = oracle.RefConfig(w.n, w.n, w.m, sigma0=w.sigma0, gain=w.gain)
     h = dia.Handle(_dev(w.R), w.m, max_epochs=E, sigma0=w.sigma0, gain=w.gain)
