@@ -157,12 +157,13 @@ def test_hessian_many_tiles_per_cta(dia, monkeypatch, grid_limit, tc):
 
 
 @pytest.mark.parametrize("c,n,m,outliers,sigma", [(4, 300, 19, 0, True), (1, 256, 15, 0, True), (2, 300, 13, 30, False),
-                                                  (4, 200, 27, 0, False), (4, 150, 33, 0, False), (0, None, None, 0, True)])
+                                                  (4, 200, 27, 0, False), (4, 150, 33, 0, False), (4, 112, 47, 0, False),
+                                                  (0, None, None, 0, True)])
 def test_hessian_tensor_core_path_against_cuda_core_path_and_oracle(dia, monkeypatch, c, n, m, outliers, sigma):
     """hess_tc_kernel (the default for m >= 5: split-float16 tcgen05 contraction, dia_hess_tc.cuh) against the FP32
     CUDA-core row passes (DIA_HESS_TC=0) and the oracle: three block types at m = 19, two at m = 13 / 15, a
-    a 15-type table with single off-diagonal blocks at m = 27 (6 groups), 36 types at m = 33 (9 groups), one
-    128-row block at m = 7.  `outliers` plants pixels
+    a 15-type table with single off-diagonal blocks at m = 27 (6 groups), 36 types at m = 33 (9 groups), 153 types on 153 CTAs
+    at m = 47 (18 groups: more CTAs than SMs), one 128-row block at m = 7.  `outliers` plants pixels
     30 000 counts BELOW the model, whose h = d^2 l / dM^2 is negative (D3): their tile rows take the second, negated
     pass of the kernel.  The uncertainties of Eq. 17 are asserted where the Hessian tests assert them (`sigma`); the
     729-parameter kernel on a 200^2 image (cond(H) = 2e10, 42 pixels per parameter: the float32 Hessian of EITHER path is
