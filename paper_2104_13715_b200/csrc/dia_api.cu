@@ -660,9 +660,7 @@ extern "C" int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, d
   dia::HessWorkspace& w = h->hess;
   if (!w.chol) {
     cudaError_t ce = cudaMalloc(&w.chol, sizeof(double) * ((size_t)np * np + dia::kCholPanel * dia::kCholPanel));   // + the panel's diagonal block
-    if (ce == cudaSuccess)
-      ce = cudaFuncSetAttribute(dia::cov_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)(sizeof(double) * dia::kSolveWarps * np));
+
     if (ce != cudaSuccess) {
       cudaFree(w.chol);  w.chol = nullptr;
       h->err = std::string("covariance workspace: ") + cudaGetErrorString(ce);
@@ -678,9 +676,18 @@ extern "C" int dia_covariance(dia_handle* h, const double* d_H, double* d_cov, d
     dia::chol_panel_factor_kernel<<<below > 0 ? (below + dia::kCholWarps - 1) / dia::kCholWarps : 1, dia::kCholWarps * 32, 0,
                                     h->stream>>>(w.chol, w.chol + (size_t)np * np, np, j0, nb, d_info);
   }
-  dia::cov_solve_kernel<<<(np + 1 + dia::kSolveWarps - 1) / dia::kSolveWarps, dia::kSolveWarps * 32,
-                          sizeof(double) * dia::kSolveWarps * np, h->stream>>>(w.chol, np, h->cfg.m * h->cfg.m, d_cov,
-                                                                                d_sigma, d_info);
+  {
+    const double* Wc = w.chol;
+    int np_ = np, nk_ = h->cfg.m * h->cfg.m;
+    void* sargs[] = {(void*)&Wc, (void*)&np_, (void*)&nk_, (void*)&d_cov, (void*)&d_sigma, (void*)&d_info};
+    size_t ssmem = 0;
+    const void* ksolve = dia::cov_solve_kernel_for(np, &ssmem);
+    cudaError_t ce = cudaFuncSetAttribute(ksolve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssmem);
+    if (ce == cudaSuccess)
+      ce = cudaLaunchKernel(ksolve, dim3((np + 1 + dia::kSolveWarps - 1) / dia::kSolveWarps), dim3(dia::kSolveWarps * 32), sargs, ssmem,
+                            h->stream);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "covariance solve launch");
+  }
   if (d_cov) dia::hess_symmetrise_kernel<<<(np * np + 255) / 256, 256, 0, h->stream>>>(d_cov, np);
   cudaError_t ce = cudaGetLastError();
   if (ce != cudaSuccess) return cuda_fail(h, ce, "covariance launch");
