@@ -41,3 +41,11 @@ size_t DIA_CAT(hess_tc_smem_m, DIA_INST_M)() { return TcGeo<DIA_INST_M>::SMEM; }
 const void* DIA_CAT(const_symbol_m, DIA_INST_M)() { return (const void*)&c_blk; }
 
 }  // namespace dia
+
+#if defined(DIA_CLUSTER_PROFILE) && DIA_INST_M == 7
+// profiling builds only (-DDIA_CLUSTER_PROFILE): the clock64 phase counters of fit_cluster_kernel<7>, CTA 0
+extern "C" void dia_cluster_prof(long long* out, int reset) {
+  if (reset) { long long z[16] = {}; cudaMemcpyToSymbol(dia::g_cl_prof, z, sizeof(z)); }
+  else cudaMemcpyFromSymbol(out, dia::g_cl_prof, sizeof(long long) * 16);
+}
+#endif

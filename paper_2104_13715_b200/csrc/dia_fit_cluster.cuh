@@ -56,6 +56,13 @@ struct ClusterGeo {
   static constexpr size_t SMEM = IN_RBUF ? G::SMEM : OFF_SCRATCH + EXTRA + 128;
 };
 
+#ifdef DIA_CLUSTER_PROFILE
+__device__ long long g_cl_prof[16];
+#define CL_T(k) do { if (blockIdx.x == 0 && threadIdx.x == 0) { const long long t_ = clock64(); g_cl_prof[k] += t_ - cl_t0; cl_t0 = t_; } } while (0)
+#else
+#define CL_T(k) do { } while (0)
+#endif
+
 template <int M>
 __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(const EvalParams p, const __grid_constant__ TensorMaps tm,
                                                                  const StepArgs a) {
@@ -120,6 +127,9 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
   if (tid < kMaxBg) Bs[tid] = 0.f;
   cluster.sync();                                          // every CTA of the cluster has started (its shared memory exists)
 
+#ifdef DIA_CLUSTER_PROFILE
+  long long cl_t0 = clock64();
+#endif
   while (true) {
     if (*done_l) break;                                    // stored by rank 0 before the barrier that ended the last pass
     for (int idx = tid; idx < G::K_FLOATS; idx += kThreads) {
@@ -130,6 +140,7 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
 #pragma unroll
     for (int q = 0; q < G::KP / 4; ++q) myacc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
+    CL_T(0);
     double loss64, gb064;
     {                                                      // forward, exactly as eval_kernel
       float tot[kP];
@@ -144,6 +155,7 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
       gb064 = (double)wsum;
     }
     __syncthreads();
+    CL_T(1);
     if (g_active) {                                        // gradient
       GradAcc<M> A;
       grad_acc_load<M>(A, myacc);
@@ -155,6 +167,7 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
       grad_acc_store<M>(A, myacc);
     }
     __syncthreads();
+    CL_T(2);
     fold_strips<M>(accS, tid, [&](int o, double s) { pcol[o] = s; });      // the order of eval_kernel's flush
     {
       const double l = warp_sum_f64(loss64), g0 = warp_sum_f64(gb064);
@@ -167,17 +180,22 @@ __global__ void __launch_bounds__(kThreads, Geo<M>::CTAS) fit_cluster_kernel(con
       pcol[M * M] = gs;
       pcol[np] = ls;
     }
+    CL_T(3);
     cluster.sync();                                        // every partial column of this epoch is complete
+    CL_T(4);
     if (rank == 0) {
       fit_step_body<CG::PER>(a, e, sc);                    // leaves the next theta in thl, the done flag in done_l
       __syncthreads();
+      CL_T(5);
       for (int r = 1; r < n_tiles; ++r) {                  // hand both to the other CTAs of the cluster
         float* rth = cluster.map_shared_rank(thl, r);
         for (int k = tid; k < np; k += kThreads) rth[k] = thl[k];
         if (tid == 0) *cluster.map_shared_rank(done_l, r) = *done_l;
       }
     }
+    CL_T(6);
     cluster.sync();                                        // theta / done of the next pass are in place; pcol is free
+    CL_T(7);
   }
 }
 
