@@ -243,6 +243,17 @@ int dia_measure_fp32_pattern(void* stream, int pattern, double* fma_per_second);
  * float32 DEVICE.  Asynchronous on `stream`.  Shows how the tensor core rounds when it accumulates. */
 int dia_tc_probe_gemm(void* stream, const float* d_A, const float* d_B, float* d_D, int K, int N, int mode);
 
+/* The work plan of dia_hessian's tensor-core kernel for kernel size m and background degree d (host arithmetic only, no
+ * device needed; exported for tests): the np = m*m + (d+1)(d+2)/2 parameters fill n_groups = ceil(np / 128) groups of 128
+ * operand slots, perm[slot] is the parameter of a slot (-1: empty; 128 n_groups entries), and every CTA type t is the
+ * five bytes types[5 t ..] = { g0, g1 (255: none), a_sel, b_start, b_groups }: an operand tile [g0 | g1], the A operand
+ * (rows of the result block) group (a_sel ? g1 : g0), the B operand b_groups groups starting at tile position b_start.
+ * Every block (gi <= gj) of H is computed by exactly one type.  Returns INVALID_ARG when the outputs are too small
+ * (max_types, max_slots), UNSUPPORTED when the table does not fit the kernel's limits (dia_hessian then runs the
+ * CUDA-core path). */
+int dia_hess_tc_plan(int m, int bg_degree, int* n_groups, int* n_types, unsigned char* types, int max_types,
+                     short* perm, int max_slots);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     dia_measure_fp32_peak,
     dia_measure_fp32_pattern,
     dia_tc_probe_gemm,
+    dia_hess_tc_plan,
     load_library,
     LOSS_GAUSSIAN,
     LOSS_HUBER,

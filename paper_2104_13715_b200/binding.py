@@ -21,7 +21,7 @@ FIT_STATUS = {0: "converged_grad", 1: "converged_change", 2: "max_iters", 3: "no
 EXPORTED_SYMBOLS = ("dia_default_fit_opts", "dia_create", "dia_eval_loss_grad", "dia_fit",
                     "dia_destroy", "dia_status_string", "dia_last_error", "dia_get_info",
                     "dia_measure_fp32_peak", "dia_measure_fp32_pattern", "dia_difference_image", "dia_hessian", "dia_covariance",
-                    "dia_eval_loss_grad_static", "dia_tc_probe_gemm", "dia_eval_loss_grad_host", "dia_fit_host")
+                    "dia_eval_loss_grad_static", "dia_tc_probe_gemm", "dia_eval_loss_grad_host", "dia_fit_host", "dia_hess_tc_plan")
 STATIC_SCRATCH_BYTES = 4 << 20          # DIA_STATIC_SCRATCH_BYTES of include/dia.h
 
 
@@ -102,6 +102,7 @@ def load_library(build_if_missing: bool = True):
     lib.dia_measure_fp32_pattern.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
     lib.dia_eval_loss_grad_host.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 4
     lib.dia_fit_host.argtypes = [C.c_void_p, C.POINTER(FitOpts), C.c_int] + [C.c_void_p] * 4 + [C.c_int]
+    lib.dia_hess_tc_plan.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_void_p, C.c_int, C.c_void_p, C.c_int]
     lib.dia_tc_probe_gemm.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]
     _LIB = lib
     return lib
@@ -200,6 +201,19 @@ def dia_fit_host(handle: int, opts: FitOpts, n_epochs: int, h_I, h_mask, h_theta
     lib = load_library()
     _check(lib.dia_fit_host(handle, C.byref(opts), n_epochs, _hptr(h_I, torch.float32, "h_I"), _hptr(h_mask, torch.uint8, "h_mask"),
                             _hptr(h_theta, torch.float32, "h_theta"), _hptr(h_result, torch.uint8, "h_result"), chunks), handle)
+
+
+def dia_hess_tc_plan(m: int, bg_degree: int = 0):
+    """Work plan of dia_hessian's tensor-core kernel (host arithmetic, no device): (n_groups, types [n][5] uint8 =
+    g0, g1, a_sel, b_start, b_groups, perm [128 n_groups] int16 = parameter of every operand slot, -1 = empty)."""
+    import numpy as np
+    lib = load_library()
+    G, n = C.c_int(), C.c_int()
+    types = np.zeros((160, 5), dtype=np.uint8)
+    perm = np.zeros(128 * 32, dtype=np.int16)
+    _check(lib.dia_hess_tc_plan(m, bg_degree, C.byref(G), C.byref(n), types.ctypes.data_as(C.c_void_p), 160,
+                                perm.ctypes.data_as(C.c_void_p), perm.size))
+    return G.value, types[:n.value].copy(), perm[:128 * G.value].copy()
 
 
 def dia_fit(handle: int, opts: FitOpts, n_epochs: int, d_I, d_mask, d_var, d_theta, d_result) -> None:

@@ -882,6 +882,28 @@ extern "C" int dia_fit_host(dia_handle* h, const dia_fit_opts* opts, int n_epoch
   return DIA_OK;
 }
 
+extern "C" int dia_hess_tc_plan(int m, int bg_degree, int* n_groups, int* n_types, unsigned char* types, int max_types,
+                                short* perm, int max_slots) {
+  if (m < 1 || m % 2 == 0 || m > DIA_MAX_KERNEL_SIZE || bg_degree < 0 || bg_degree > DIA_MAX_BG_DEGREE || !n_groups || !n_types ||
+      !types || !perm)
+    return fail(nullptr, DIA_ERR_INVALID_ARG, "dia_hess_tc_plan: bad argument");
+  const int np = m * m + (bg_degree + 1) * (bg_degree + 2) / 2;
+  const int G = (np + dia::kTcGroup - 1) / dia::kTcGroup;
+  dia::HessTcTypes t;
+  const int n = dia::hess_tc_make_types(np, &t);
+  if (n == 0) return fail(nullptr, DIA_ERR_UNSUPPORTED, "type table exceeds the kernel's limit");
+  if (n > max_types || G * dia::kTcGroup > max_slots) return fail(nullptr, DIA_ERR_INVALID_ARG, "dia_hess_tc_plan: outputs too small");
+  int rpitch = 0, rh = 0;
+  geometry_for(m, &rpitch, &rh);
+  dia::hess_tc_make_perm(m, np, rpitch, perm);
+  for (int i = 0; i < n; ++i) {
+    types[5 * i] = t.g0[i];  types[5 * i + 1] = t.g1[i];  types[5 * i + 2] = t.a_sel[i];  types[5 * i + 3] = t.b_start[i];
+    types[5 * i + 4] = t.n_groups[i];
+  }
+  *n_groups = G;  *n_types = n;
+  return DIA_OK;
+}
+
 extern "C" int dia_tc_probe_gemm(void* stream, const float* d_A, const float* d_B, float* d_D, int K, int N, int mode) {
   if (!d_A || !d_B || !d_D) return fail(nullptr, DIA_ERR_INVALID_ARG, "null argument");
   if (K < dia::kTcProbeKC || K % dia::kTcProbeKC != 0 || N < 32 || N > 256 || N % 32 != 0 || mode < 0 || mode > 3)

@@ -207,3 +207,43 @@ def test_bench_accounting():
     import bench
     assert bench.useful_fma(4096, 19, 1) == pytest.approx(1.2007e10, rel=1e-4)
     assert bench.useful_fma(128, 7, 1) == pytest.approx(1.459e6, rel=1e-3)
+
+
+@pytest.mark.parametrize("m,d", [(5, 0), (7, 0), (11, 3), (13, 0), (15, 2), (19, 0), (19, 3), (27, 0), (33, 1), (41, 0), (47, 3)])
+def test_tensor_core_hessian_work_plan(m, d):
+    """Host logic of dia_hessian's tensor-core path (dia_hess_tc_plan; no device): the operand slots hold every
+    parameter exactly once, every block (gi <= gj) of H is computed by exactly one CTA type, a type's A operand is one
+    of the (at most two) groups of its operand tile, and the slots are dealt so that the 32 rows a warp builds read 32
+    different shared-memory banks of the staged R tile (kernel pixel (a, b) reads a * pitch + b + const)."""
+    import paper_2104_13715_b200 as dia
+    G, types, perm = dia.dia_hess_tc_plan(m, d)
+    np_ = m * m + (d + 1) * (d + 2) // 2
+    assert G == -(-np_ // 128) and perm.shape == (128 * G,)
+    assert sorted(perm[perm >= 0].tolist()) == list(range(np_))
+    blocks = []
+    for g0, g1, a_sel, b_start, nb in types.tolist():
+        tile = [g0, g1]
+        assert g0 < G and (g1 < G or g1 == 255) and nb in (1, 2) and b_start + nb <= 2 and a_sel in (0, 1)
+        gA = tile[a_sel]
+        assert gA != 255
+        for t in range(b_start, b_start + nb):
+            assert tile[t] != 255
+            blocks.append((min(gA, tile[t]), max(gA, tile[t])))
+    assert sorted(blocks) == [(i, j) for i in range(G) for j in range(i, G)]
+    # bank classes: R tile pitch of the fused kernel = RMIN rounded up to 4 (mod 8), RMIN = 48 + round_up(16 + m - 1, 4)
+    rmin = 48 + -(-(16 + m - 1) // 4) * 4
+    pitch = rmin + ((4 - rmin % 8) + 8) % 8
+    conflicts = 0
+    for w in range(4 * G):
+        rows = [q for q in perm[32 * w:32 * w + 32].tolist() if 0 <= q < m * m]
+        banks = [((q // m) * pitch + q % m) % 32 for q in rows]
+        conflicts += len(banks) - len(set(banks))
+    assert conflicts <= max(2, m * m // 100), conflicts        # the greedy deal leaves at most a few leftovers
+
+
+def test_tensor_core_hessian_work_plan_errors():
+    import paper_2104_13715_b200 as dia
+    with pytest.raises(dia.DiaError):
+        dia.dia_hess_tc_plan(4, 0)
+    with pytest.raises(dia.DiaError):
+        dia.dia_hess_tc_plan(7, 9)
