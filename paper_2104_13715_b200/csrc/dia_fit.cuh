@@ -196,9 +196,12 @@ __global__ void fit_init_kernel(FitBuffers b, const float* __restrict__ theta_in
 // (np <= 32 JW <= 256; lane l owns elements l, l + 32, ...).  The 2 n_pairs steps depend on each other through a dot
 // product each: a lane-strided partial sum and a warp butterfly, with the history rows of the next D steps already in
 // flight in a ring of D register slots, instead of a block-wide sum (two barriers) and rows loaded when needed.
-// Measured (128^2, m = 7, full history of 100 pairs): 88 us per L-BFGS iteration against 102 us -- the step stays at
-// ~0.3 us, which is the latency of its dependent FP64 chain (dot, five shuffle + add levels, scale, update), not
-// memory and not barriers.
+// The warp runs alone (the rest of the block waits at a barrier), so the latency of EVERY instruction of a step adds
+// up: the history slot is stepped instead of computed with a modulo, a row address is one multiply-add, the dot
+// product is split into independent chains (a dependent FP64 operation costs ~40 cycles on this part).
+// Measured (128^2, m = 7, full history of 100 pairs): 65 us per L-BFGS iteration against 102 us for the block-wide
+// form (clock64: 110 000 of its 121 000 step cycles were this loop); a step is now ~0.25 us, its dependent chain
+// (dot, five shuffle + add levels, scale, update) ~0.2 us.
 // Not inlined: its registers must not count against the caller (fit_cluster_kernel runs under a 128-register cap;
 // inlined, a first version cost it 5 KB of spills and 15 % of its Adam rate).
 template <int JW, int D>
@@ -208,66 +211,76 @@ __device__ __noinline__ void two_loop_warp(double* __restrict__ x, int np, const
                                            double* __restrict__ s_alpha) {
   const int lane = threadIdx.x & 31;
   double v[JW], a[D][JW], b[D][JW], r[D];
-  auto load_rows = [&](int i, double* sr, double* yr, double& rh) {      // history pair of step i
-    const int id = (head + i) % hist;
+  bool ok[JW];
 #pragma unroll
-    for (int j = 0; j < JW; ++j) {
-      const int k = lane + 32 * j;
-      sr[j] = (k < np) ? Sm[(size_t)id * np + k] : 0.0;
-      yr[j] = (k < np) ? Ym[(size_t)id * np + k] : 0.0;
-    }
+  for (int j = 0; j < JW; ++j) { ok[j] = lane + 32 * j < np; v[j] = ok[j] ? x[lane + 32 * j] : 0.0; }
+  // one warp runs alone here, so every instruction's latency counts: the history slot of a step is stepped, not
+  // computed with a modulo, and a row's address is one multiply-add
+  auto load_rows = [&](int id, double* sr, double* yr, double& rh) {      // history pair in slot id
+    const double* sp = Sm + (size_t)id * np + lane;
+    const double* yp = Ym + (size_t)id * np + lane;
+#pragma unroll
+    for (int j = 0; j < JW; ++j) { sr[j] = ok[j] ? sp[32 * j] : 0.0; yr[j] = ok[j] ? yp[32 * j] : 0.0; }
     rh = rho[id];
   };
+  auto dot = [](const double* p, const double* q) {     // up to four independent chains: a dependent FP64 FMA costs ~40 cycles
+    double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
 #pragma unroll
-  for (int j = 0; j < JW; ++j) { const int k = lane + 32 * j; v[j] = (k < np) ? x[k] : 0.0; }
+    for (int j = 0; j < JW; j += 4) {
+      c0 = fma(p[j], q[j], c0);
+      if (j + 1 < JW) c1 = fma(p[j + 1], q[j + 1], c1);
+      if (j + 2 < JW) c2 = fma(p[j + 2], q[j + 2], c2);
+      if (j + 3 < JW) c3 = fma(p[j + 3], q[j + 3], c3);
+    }
+    return (c0 + c1) + (c2 + c3);
+  };
+  auto dec = [&](int id) { return id == 0 ? hist - 1 : id - 1; };
+  auto inc = [&](int id) { return id + 1 == hist ? 0 : id + 1; };
+  const int id_last = n_pairs > 0 ? (head + n_pairs - 1) % hist : 0;
+  int idp = id_last;                                                      // slot of the next row to request
 #pragma unroll
   for (int u = 0; u < D; ++u) {
     r[u] = 0.0;
 #pragma unroll
     for (int j = 0; j < JW; ++j) { a[u][j] = 0.0; b[u][j] = 0.0; }
-    if (n_pairs - 1 - u >= 0) load_rows(n_pairs - 1 - u, a[u], b[u], r[u]);
+    if (u < n_pairs) { load_rows(idp, a[u], b[u], r[u]); idp = dec(idp); }
   }
   for (int base = n_pairs - 1; base >= 0; base -= D) {
 #pragma unroll
     for (int u = 0; u < D; ++u) {
       const int i = base - u;                          // slot u holds step i
       if (i >= 0) {
-        double part = 0.0;
-#pragma unroll
-        for (int j = 0; j < JW; ++j) part += a[u][j] * v[j];
-        const double al = r[u] * warp_sum_f64(part);
+        const double al = r[u] * warp_sum_f64(dot(a[u], v));
         if (lane == 0) s_alpha[i] = al;
 #pragma unroll
         for (int j = 0; j < JW; ++j) v[j] -= al * b[u][j];
-        if (i - D >= 0) load_rows(i - D, a[u], b[u], r[u]);
+        if (i - D >= 0) { load_rows(idp, a[u], b[u], r[u]); idp = dec(idp); }
       }
     }
   }
   double gamma = 1.0;
-  if (n_pairs > 0) { const int id = (head + n_pairs - 1) % hist; gamma = (1.0 / rho[id]) / yy[id]; }
+  if (n_pairs > 0) gamma = (1.0 / rho[id_last]) / yy[id_last];
 #pragma unroll
   for (int j = 0; j < JW; ++j) v[j] *= gamma;
   __syncwarp();
+  idp = head;
 #pragma unroll
   for (int u = 0; u < D; ++u)
-    if (u < n_pairs) load_rows(u, a[u], b[u], r[u]);
+    if (u < n_pairs) { load_rows(idp, a[u], b[u], r[u]); idp = inc(idp); }
   for (int base = 0; base < n_pairs; base += D) {
 #pragma unroll
     for (int u = 0; u < D; ++u) {
       const int i = base + u;
       if (i < n_pairs) {
-        double part = 0.0;
-#pragma unroll
-        for (int j = 0; j < JW; ++j) part += b[u][j] * v[j];
-        const double c = s_alpha[i] - r[u] * warp_sum_f64(part);
+        const double c = s_alpha[i] - r[u] * warp_sum_f64(dot(b[u], v));
 #pragma unroll
         for (int j = 0; j < JW; ++j) v[j] += c * a[u][j];
-        if (i + D < n_pairs) load_rows(i + D, a[u], b[u], r[u]);
+        if (i + D < n_pairs) { load_rows(idp, a[u], b[u], r[u]); idp = inc(idp); }
       }
     }
   }
 #pragma unroll
-  for (int j = 0; j < JW; ++j) { const int k = lane + 32 * j; if (k < np) x[k] = v[j]; }
+  for (int j = 0; j < JW; ++j) if (ok[j]) x[lane + 32 * j] = v[j];
 }
 
 // One optimiser transition for epoch e, run by one CTA of kFitThreads threads after every evaluation of that epoch.
