@@ -309,6 +309,19 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
   {
     const double* src = a.partials + (size_t)e * (np + 1) * a.n_blocks;
     const int lane = tid & 31, wid = tid >> 5;
+    if (a.n_blocks <= 8) {
+      // few columns (a small image; always in the cluster loop): one thread per output adds its <= 8 values in the
+      // association order of the warp butterfly below -- ((v0+v4)+(v2+v6)) + ((v1+v5)+(v3+v7)), absent columns 0 -- so
+      // the bits are those of the general path, without its four butterflies per warp in the chain (3800 -> ~800
+      // cycles of a 20 000-cycle Adam iteration at 128^2)
+      for (int k = tid; k < np + 1; k += kFitThreads) {
+        double v[8];
+#pragma unroll
+        for (int b = 0; b < 8; ++b)
+          v[b] = b < a.n_blocks ? (sc.peer_cols ? sc.peer_cols[b][k] : src[(size_t)k * a.n_blocks + b]) : 0.0;
+        gsum[k] = ((v[0] + v[4]) + (v[2] + v[6])) + ((v[1] + v[5]) + (v[3] + v[7]));
+      }
+    } else
     // four rows per warp at a time, so that enough loads are in flight to hide the L2 latency
     for (int k = wid * 4; k < np + 1; k += (kFitThreads / 32) * 4) {
       double s4[4] = {0.0, 0.0, 0.0, 0.0};
