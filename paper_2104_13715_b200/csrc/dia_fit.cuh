@@ -283,6 +283,74 @@ __device__ __noinline__ void two_loop_warp(double* __restrict__ x, int np, const
   for (int j = 0; j < JW; ++j) if (ok[j]) x[lane + 32 * j] = v[j];
 }
 
+// The same recursion for 256 < np <= 32 JW <= 512 (m = 17 .. 21: the paper's stamp fits): the register ring does not
+// fit beside v there, so a row is reloaded IN PLACE as soon as its last use of the step is over -- the S row right
+// after the dot product, the Y row right after the update (the other way round in the second loop) -- and is in flight
+// during the butterfly and the rest of the step.
+template <int JW>
+__device__ __noinline__ void two_loop_warp_inplace(double* __restrict__ x, int np, const double* __restrict__ Sm,
+                                                   const double* __restrict__ Ym, const double* __restrict__ rho,
+                                                   const double* __restrict__ yy, int head, int n_pairs, int hist,
+                                                   double* __restrict__ s_alpha) {
+  const int lane = threadIdx.x & 31;
+  double v[JW], a[JW], b[JW];
+  bool ok[JW];
+#pragma unroll
+  for (int j = 0; j < JW; ++j) { ok[j] = lane + 32 * j < np; v[j] = ok[j] ? x[lane + 32 * j] : 0.0; a[j] = 0.0; b[j] = 0.0; }
+  auto load = [&](const double* M, int id, double* dst) {
+    const double* p = M + (size_t)id * np + lane;
+#pragma unroll
+    for (int j = 0; j < JW; ++j) dst[j] = ok[j] ? p[32 * j] : 0.0;
+  };
+  auto dot = [](const double* p, const double* q) {
+    double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+#pragma unroll
+    for (int j = 0; j < JW; j += 4) {
+      c0 = fma(p[j], q[j], c0);
+      if (j + 1 < JW) c1 = fma(p[j + 1], q[j + 1], c1);
+      if (j + 2 < JW) c2 = fma(p[j + 2], q[j + 2], c2);
+      if (j + 3 < JW) c3 = fma(p[j + 3], q[j + 3], c3);
+    }
+    return (c0 + c1) + (c2 + c3);
+  };
+  auto dec = [&](int id) { return id == 0 ? hist - 1 : id - 1; };
+  auto inc = [&](int id) { return id + 1 == hist ? 0 : id + 1; };
+  const int id_last = n_pairs > 0 ? (head + n_pairs - 1) % hist : 0;
+  int id = id_last;
+  double r = 0.0;
+  if (n_pairs > 0) { load(Sm, id, a); load(Ym, id, b); r = rho[id]; }
+  for (int i = n_pairs - 1; i >= 0; --i) {
+    const int idn = dec(id);
+    const double part = dot(a, v);
+    if (i > 0) load(Sm, idn, a);                       // S of the next step: in flight during the butterfly
+    const double al = r * warp_sum_f64(part);
+    if (lane == 0) s_alpha[i] = al;
+#pragma unroll
+    for (int j = 0; j < JW; ++j) v[j] -= al * b[j];
+    if (i > 0) { load(Ym, idn, b); r = rho[idn]; }
+    id = idn;
+  }
+  double gamma = 1.0;
+  if (n_pairs > 0) gamma = (1.0 / rho[id_last]) / yy[id_last];
+#pragma unroll
+  for (int j = 0; j < JW; ++j) v[j] *= gamma;
+  __syncwarp();
+  id = head;
+  if (n_pairs > 0) { load(Sm, id, a); load(Ym, id, b); r = rho[id]; }
+  for (int i = 0; i < n_pairs; ++i) {
+    const int idn = inc(id);
+    const double part = dot(b, v);
+    if (i + 1 < n_pairs) load(Ym, idn, b);
+    const double c = s_alpha[i] - r * warp_sum_f64(part);
+#pragma unroll
+    for (int j = 0; j < JW; ++j) v[j] += c * a[j];
+    if (i + 1 < n_pairs) { load(Sm, idn, a); r = rho[idn]; }
+    id = idn;
+  }
+#pragma unroll
+  for (int j = 0; j < JW; ++j) if (ok[j]) x[lane + 32 * j] = v[j];
+}
+
 // One optimiser transition for epoch e, run by one CTA of kFitThreads threads after every evaluation of that epoch.
 template <int PER>
 __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, const StepScratch& sc) {
@@ -483,14 +551,16 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
 #pragma unroll
       for (int q = 0; q < PER; ++q) gq[q] = q4[q];
       // two-loop recursion (N&W Alg. 7.4)
-      if (np <= 256) {                                    // one warp, history rows prefetched (two_loop_warp)
+      if (np <= 512) {                                    // one warp, history rows prefetched (two_loop_warp)
 #pragma unroll
         for (int q = 0; q < PER; ++q) { const int k = tid + q * kFitThreads; if (k < np) sc.xs[k] = q4[q]; }
         __syncthreads();
         if (tid < 32) {
           if (np <= 64) two_loop_warp<2, 6>(sc.xs, np, Sm, Ym, rho, yy, st.head, st.n_pairs, hist, s_alpha);
           else if (np <= 128) two_loop_warp<4, 4>(sc.xs, np, Sm, Ym, rho, yy, st.head, st.n_pairs, hist, s_alpha);
-          else two_loop_warp<8, 2>(sc.xs, np, Sm, Ym, rho, yy, st.head, st.n_pairs, hist, s_alpha);
+          else if (np <= 256) two_loop_warp<8, 2>(sc.xs, np, Sm, Ym, rho, yy, st.head, st.n_pairs, hist, s_alpha);
+          else if (np <= 384) two_loop_warp_inplace<12>(sc.xs, np, Sm, Ym, rho, yy, st.head, st.n_pairs, hist, s_alpha);
+          else two_loop_warp_inplace<16>(sc.xs, np, Sm, Ym, rho, yy, st.head, st.n_pairs, hist, s_alpha);
         }
         __syncthreads();
 #pragma unroll
