@@ -647,8 +647,12 @@ __device__ __forceinline__ void fit_step_body(const StepArgs& a, const int e, co
 }
 
 #ifndef DIA_INST_M
+// Two CTAs per SM in the launch bounds = a cap of 128 registers: the one-warp recursions above would otherwise raise the
+// kernel's allocation to 178 registers per thread for all 256 threads, and the step kernel's place in the graph loop is
+// sensitive to its footprint -- measured per Adam iteration at c2 (1024^2, m = 19: eval 45 us): 54.6 us with the cap,
+// 65.4 us without, 62.1 us for the 88-register kernel before the recursions were added.
 template <int PER>
-__global__ void __launch_bounds__(kFitThreads) fit_step_kernel(const StepArgs a) {
+__global__ void __launch_bounds__(kFitThreads, 2) fit_step_kernel(const StepArgs a) {
   const int e = blockIdx.x;
   if (a.b.done[e]) return;
   __shared__ double sh_rows[2][kFitThreads / 32];
