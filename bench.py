@@ -538,8 +538,18 @@ def run_gpu(args):
             # "useful" counts the dense np x np x pixels product once (2 flops per multiply-add); the kernel computes the
             # upper block triangle of the 128-padded matrix in four split-float16 terms
             n_valid = (N - M + 1) ** 2
+            g_ = -(-rows // 128)
+            executed = 2.0 * 4 * (g_ * (g_ + 1) // 2) * 128 * 128 * n_valid        # four split terms, upper block triangle
+            tensor_peak = float(peaks.get("bf16_tflops") or 2250.0)                 # fp16 = bf16 rate (nominal ratio 1); burst figure
             line["fits"]["hessian"] = {"ms": ms_h, "rows": rows, "launches": 3,
                                        "useful_tflops": 2.0 * rows * rows * n_valid / (ms_h * 1e-3) / 1e12,
+                                       "roofline": {"bound": "tensor", "achieved": executed / (ms_h * 1e-3) / 1e12, "peak": tensor_peak,
+                                                    "unit": "TFLOP/s", "frac": executed / (ms_h * 1e-3) / 1e12 / tensor_peak,
+                                                    "traffic": 139.1e6,
+                                                    "note": "executed float16 MMA work of hess_tc_kernel (4 terms x 6 blocks of 128 x 128 per "
+                                                            "valid pixel) over the whole dia_hessian call, against MEASURED_PEAKS.json's "
+                                                            "cuBLAS bf16 burst figure (else the nominal 2250); traffic: dram bytes of the "
+                                                            "ncu capture in profiles/r02_tc_hessian.md"},
                                        "path": "tcgen05 kind::f16, float16 hi/lo split (4 terms), FP32 in TMEM per tile row, "
                                                "FP64 per tile",
                                        "work_model": "2 np^2 flops per valid pixel"}
