@@ -178,7 +178,8 @@ __device__ __forceinline__ void small_row(const float (&win)[M][SmallGeo<M>::SEG
 // second register set before the current one is used.
 template <int M, bool HUBER, bool FAST>
 __device__ __forceinline__ void small_strip(const EvalParams& p, const float* __restrict__ Rimg, const float* __restrict__ Iimg,
-                                            int y0, int x0, int nrows, int n_in, bool vec, unsigned long long pol_keep,
+                                            int y0, int x0, int nrows, int n_in, bool vec, bool warp_full,
+                                            unsigned long long pol_keep,
                                             unsigned long long pol_stream, const float* __restrict__ K, float B0, float hg,
                                             float (&acc)[SmallGeo<M>::P], double& loss64, double& gb064) {
   using G = SmallGeo<M>;
@@ -225,7 +226,7 @@ __device__ __forceinline__ void small_strip(const EvalParams& p, const float* __
           } else {
             load_seg<SEG>(Rimg, p.n_rows, p.n_cols, y0 + r + M - 1, x0, vec, pol_keep, win[(U + M - 1) % M]);
             load_seg<SEG>(Iimg, p.n_rows, p.n_cols, y0 + r + H, x0, vec, pol_stream, iv);
-            if (n_in >= kSmallPx) small_row<M, U, HUBER, false>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
+            if (warp_full) small_row<M, U, HUBER, false>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
             else small_row<M, U, HUBER, true>(win, iv, K, B0, p, hg, n_in, acc, loss64, gb064);
           }
           Rp += pitch;
@@ -312,7 +313,12 @@ __global__ void __maxnreg__(SmallGeo<M>::MAXREG) eval_small_kernel(const EvalPar
       out = p.partials + ((size_t)e * p.part_rows) * ncols + col;
       __syncthreads();                     // K visible (finish_epoch ended with a barrier after its last reads)
     }
-    const int tile_y = t / tiles_x, tile_x = t - tile_y * tiles_x;
+    // item t -> tile (tile_y, tile_x), the columns rotated by the row: a CTA's items are `grid` apart, and with
+    // gcd(grid, tiles_x) > 1 (296 and 16 at 4096^2) an unrotated map hands the same few tile columns -- for some CTAs
+    // the ragged right-edge column every other item -- to a CTA for its whole life
+    const int tile_y = t / tiles_x;
+    int tile_x = t - tile_y * tiles_x + tile_y % tiles_x;
+    if (tile_x >= tiles_x) tile_x -= tiles_x;
     const int x0 = tile_x * tile_w + kSmallPx * lx;                       // first pixel of the strip (valid coords)
     const int y0 = tile_y * tile_h + (warp * (32 >> lxlog) + ly) * rpt;   // first row of this thread
     const int nrows = min(rpt, vr - y0);                                  // <= 0: nothing to do
@@ -323,11 +329,18 @@ __global__ void __maxnreg__(SmallGeo<M>::MAXREG) eval_small_kernel(const EvalPar
     float acc[P];
 #pragma unroll
     for (int i = 0; i < P; ++i) acc[i] = 0.f;
-    if (n_in > 0 && nrows > 0) {
-      if (vec && n_in >= kSmallPx && x0 + SEG <= p.n_cols)
-        small_strip<M, HUBER, true>(p, Rimg, Iimg, y0, x0, nrows, n_in, vec, pol_keep, pol_stream, K, B0, hg, acc, loss64, gb064);
+    // One path per WARP: a warp whose last lane's strip crosses the edge would otherwise run the fast path for 31
+    // lanes and then the predicated one for the last (measured: the edge tile column cost 2.1 x an inner one, 6.5 % of
+    // all warp instructions ran with one lane, and the CTAs that owned that column held the grid up: SMs 76 % active)
+    const bool live = n_in > 0 && nrows > 0;
+    const bool fast = vec && n_in >= kSmallPx && x0 + SEG <= p.n_cols;
+    const bool warp_fast = __all_sync(0xffffffffu, fast || !live);
+    const bool warp_full = __all_sync(0xffffffffu, n_in >= kSmallPx || !live);
+    if (live) {
+      if (warp_fast)
+        small_strip<M, HUBER, true>(p, Rimg, Iimg, y0, x0, nrows, n_in, vec, warp_full, pol_keep, pol_stream, K, B0, hg, acc, loss64, gb064);
       else
-        small_strip<M, HUBER, false>(p, Rimg, Iimg, y0, x0, nrows, n_in, vec, pol_keep, pol_stream, K, B0, hg, acc, loss64, gb064);
+        small_strip<M, HUBER, false>(p, Rimg, Iimg, y0, x0, nrows, n_in, vec, warp_full, pol_keep, pol_stream, K, B0, hg, acc, loss64, gb064);
     }
     warp_transpose_sum<P>(acc, lane);
     g64 += (double)acc[0];
