@@ -134,6 +134,24 @@ __device__ __forceinline__ void small_pixel_terms(float Mv, float Iv, float sigm
   }
 }
 
+// The Gaussian terms in the form the row loop uses: the FMA pipe, not instruction issue, is what this kernel runs out
+// of (every variant that was tried -- fewer instructions, no memory stalls -- ends at the same ~31 pipe cycles per pixel,
+// profiles/r02_small3.md), so the terms are arranged for the fewest FP32 operations: with t = r / v,
+//   a = 1 - z^2 = fma(-t, r, 1),   w = (b' / 2 * a - r) / v,   l = z^2 / 2 + ln v / 2 = (1 - a) / 2 + ln 2 / 2 * log2 v,
+// and the caller sums a and log2 v over the strip's row and forms the loss once per row: 9 FP32 operations per pixel
+// (v, r, t, a, b, w and three running sums) instead of 11.
+__device__ __forceinline__ void small_gauss_terms(float Mv, float Iv, float sigma0_sq, float inv_gain, float hg, float& a,
+                                                  float& lg, float& wi) {
+  const float v = fmaf(inv_gain, fmaxf(Mv, 0.f), sigma0_sq);
+  const float hbp = Mv > 0.f ? hg : 0.f;
+  const float res = Iv - Mv;
+  const float inv_v = rcp_approx(v);
+  const float t = res * inv_v;
+  a = fmaf(-t, res, 1.0f);
+  lg = lg2_approx(v);
+  wi = fmaf(hbp, a, -res) * inv_v;
+}
+
 // One row of a strip: model, per-pixel terms, gradient sums.  EDGE: the strip crosses the right edge of the valid
 // region, pixels beyond it contribute nothing (selects, not multiplications: zero-filled pixels may give NaN).
 template <int M, int U, bool HUBER, bool EDGE>
@@ -143,7 +161,7 @@ __device__ __forceinline__ void small_row(const float (&win)[M][SmallGeo<M>::SEG
   constexpr int H = SmallGeo<M>::H;
   // window row a lives in win[(U + a) % M].  One FP32 chain per pixel, wings first, the centre pixel last (the
   // largest terms of a peaked kernel come last; with m^2 <= 25 terms the order matters little)
-  float lsum = 0.f, wsum = 0.f;
+  float lsum = 0.f, wsum = 0.f, asum = 0.f;
 #pragma unroll
   for (int q = 0; q < kSmallPx; ++q) {
     float tot = B0;
@@ -157,17 +175,28 @@ __device__ __forceinline__ void small_row(const float (&win)[M][SmallGeo<M>::SEG
       }
     }
     float li, wi;
-    small_pixel_terms<HUBER>(tot, iv[q + H], p.sigma0_sq, p.inv_gain, hg, p.huber_c, li, wi);
-    if (EDGE) {
-      if (q >= n_in) { li = 0.f; wi = 0.f; }
+    if constexpr (HUBER) {
+      small_pixel_terms<true>(tot, iv[q + H], p.sigma0_sq, p.inv_gain, hg, p.huber_c, li, wi);
+      if (EDGE) {
+        if (q >= n_in) { li = 0.f; wi = 0.f; }
+      }
+      lsum += li;
+    } else {
+      float a1;
+      small_gauss_terms(tot, iv[q + H], p.sigma0_sq, p.inv_gain, hg, a1, li, wi);      // li: log2 v
+      if (EDGE) {
+        if (q >= n_in) { a1 = 1.f; li = 0.f; wi = 0.f; }
+      }
+      asum += a1;
+      lsum += li;
     }
-    lsum += li;
     wsum += wi;
 #pragma unroll
     for (int a = 0; a < M; ++a)
 #pragma unroll
       for (int b = 0; b < M; ++b) acc[a * M + b] = fmaf(wi, win[(U + a) % M][q + b], acc[a * M + b]);
   }
+  if constexpr (!HUBER) lsum = fmaf(0.34657359028f, lsum, 0.5f * ((float)kSmallPx - asum));
   loss64 += (double)lsum;
   gb064 += (double)wsum;
 }
