@@ -560,7 +560,7 @@ def run_gpu(args):
     if rank == 0 and not args.no_stamps:
         hbm_peak = float(peaks.get("hbm_gbs") or 6650.0)
         line["small_kernels"] = []
-        for ms_ in (1, 3):
+        for ms_ in (1, 3, 5):
             hs = dia.Handle(dR, ms_, max_epochs=E, sigma0=cfg.sigma0, gain=cfg.gain)
             ths = torch.full((E, ms_ * ms_ + 1), 1.0 / (ms_ * ms_), dtype=torch.float32, device=dev)
             ths[:, -1] = 0.0
@@ -578,9 +578,14 @@ def run_gpu(args):
             ms_s = ev_a.elapsed_time(ev_b)
             hs.close()
             gbs = 4.0 * N * N * (1 + E) / (ms_s / 20 * 1e-3) / 1e9
+            tfl = 4.0 * ms_ * ms_ * (N - ms_ + 1) ** 2 * E / (ms_s / 20 * 1e-3) / 1e12
+            # m = 5 sits between the roofs (100 FLOP per 8 bytes): both fractions are given, the larger one binds
+            fh = gbs / hbm_peak
+            ff = tfl / (SM_COUNT * FP32_LANES_PER_SM * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12)
             line["small_kernels"].append({"m": ms_, "epochs": E, "us_per_epoch": 1e3 * ms_s / 20 / E,
-                                          "evals_per_s": E * 20 / (ms_s * 1e-3), "bound": "hbm",
-                                          "algorithmic_GBps": gbs, "hbm_peak_gbs": hbm_peak, "frac": gbs / hbm_peak,
+                                          "evals_per_s": E * 20 / (ms_s * 1e-3), "bound": "hbm" if fh >= ff else "alu",
+                                          "algorithmic_GBps": gbs, "hbm_peak_gbs": hbm_peak, "frac": max(fh, ff),
+                                          "frac_hbm": fh, "tflops_useful": tfl, "frac_fp32_nominal": ff,
                                           "kernel": f"dia::eval_small_kernel<{ms_}, false>"})
 
     # ---- many small image pairs, one reference each (the paper's stamp workloads)

@@ -197,7 +197,7 @@ int dia_difference_image(dia_handle* h, int n_epochs, const float* d_I, const un
  * shared-memory attribute; later calls only encode two TMA descriptors on the host and enqueue the kernels.
  * Asynchronous on cfg->stream.  Results are bit-identical to dia_eval_loss_grad on a handle created with
  * max_epochs == n_epochs whenever that handle runs the shared-memory variant of the generic kernel (always, apart from
- * m <= 3 plain objectives and launches long enough for the constant-bank variant, whose sums agree to rounding).
+ * m <= 5 plain objectives and launches long enough for the constant-bank variant, whose sums agree to rounding).
  * Limits and errors: UNSUPPORTED with a message naming both numbers when the partials
  *   8 * n_epochs * (m*m + n_bg + 1) * min(tiles, resident CTAs)  bytes   (tiles = 64 x 64 tiles of the valid region)
  * exceed DIA_STATIC_SCRATCH_BYTES (e.g. one 4096^2 pair up to m = 27, or four at m = 19, fit; sixteen do not);

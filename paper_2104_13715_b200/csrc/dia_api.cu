@@ -237,13 +237,14 @@ static const void* small_kernel_for(int m, int loss = DIA_LOSS_GAUSSIAN) {
   switch (m) {
     case 1: return hub ? (const void*)dia::eval_small_kernel<1, true> : (const void*)dia::eval_small_kernel<1, false>;
     case 3: return hub ? (const void*)dia::eval_small_kernel<3, true> : (const void*)dia::eval_small_kernel<3, false>;
-    // m = 5 stays with the generic kernel: this design needs 180-230 registers per thread there (one CTA per SM) and
-    // was measured 12 % slower
+    case 5: return hub ? (const void*)dia::eval_small_kernel<5, true> : (const void*)dia::eval_small_kernel<5, false>;
+    // m = 5: 240 registers, one CTA of eight warps per SM -- 63.3 against the generic kernel's 73.1 us per 4096^2 epoch
+    // since the edge fix (12 % slower than the generic kernel before it)
   }
   return nullptr;
 }
 static size_t small_smem_for(int) { return 0; }   // static shared memory only
-static int small_threads_for(int m) { return m == 1 ? dia::SmallGeo<1>::THREADS : dia::SmallGeo<3>::THREADS; }
+static int small_threads_for(int m) { return m == 1 ? dia::SmallGeo<1>::THREADS : (m == 3 ? dia::SmallGeo<3>::THREADS : dia::SmallGeo<5>::THREADS); }
 // Geometry of an eval_small_kernel launch (dia_eval_small.cuh): lanes side by side until they span the valid width,
 // and the largest number of rows per thread that still leaves three tiles per resident CTA.
 namespace dia { int eval_grid(const dia_handle* h, int n_epochs); int eval_part_cols(const dia_handle* h, int n_epochs); }

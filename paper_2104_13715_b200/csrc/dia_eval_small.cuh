@@ -1,4 +1,4 @@
-// dia_eval_small.cuh -- fused loss + gradient kernel for SMALL kernels (m = 1, 3; written for any odd m <= 5), plain objective only
+// dia_eval_small.cuh -- fused loss + gradient kernel for SMALL kernels (m = 1, 3, 5), plain objective only
 // (Eq. 2, 6, 8 / 12-13; no mask, flat field, variance map, background polynomial).
 //
 // For m <= 5 the evaluation has 4 m^2 <= 100 FLOP per 8 bytes of image: the roofline is HBM bandwidth (m <= 3) or
@@ -102,7 +102,8 @@ struct SmallGeo {
   static constexpr int SEG = round_up(kSmallPx + M - 1, 4);     // 8 (m = 1) or 12 floats per window row
   static constexpr int P = M == 1 ? 1 : (M == 3 ? 16 : 32);     // padded number of kernel-gradient sums
   // m = 1: 3 CTAs of 8 warps at 80 registers; m = 3: 2 CTAs at 128 registers (3 CTAs of 7 warps at 96 registers, or
-  // of 8 warps at 80, spill and were measured 19 % and 13 % slower); m = 5: one CTA
+  // of 8 warps at 80, spill and were measured 19 % and 13 % slower); m = 5: one CTA at ~240 registers (three CTAs of
+  // four warps at 168 spill and were measured 9 % slower)
   static constexpr int THREADS = 256;
   static constexpr int MAXREG = M == 1 ? 80 : (M == 3 ? 128 : 255);
 };

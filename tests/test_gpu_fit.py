@@ -363,8 +363,12 @@ def test_fit_cluster_kernel_matches_graph_loop(dia, monkeypatch, c, n, m, E):
     (csrc/dia_fit_cluster.cuh: tiles resident in shared memory, cluster barriers instead of launches).  Same device
     functions, same orders: for image pairs whose tiles sit on different CTAs in the graph loop the fitted parameters,
     iteration counts and losses must be bit-identical to it (test hook DIA_DISABLE_CLUSTER=1), free-running and in
-    lock-step; (190^2: 3 x 3 = 9 tiles exceed the portable cluster size and take the graph loop on both sides)."""
+    lock-step; (190^2: 3 x 3 = 9 tiles exceed the portable cluster size and take the graph loop on both sides).
+    The graph loop it is compared with is the one over the generic kernel, whose device functions the cluster kernel
+    shares: DIA_DISABLE_SMALL=1 keeps the m = 5 case off eval_small_kernel (other arithmetic order, equal to rounding:
+    tests/test_gpu_small_kernels.py)."""
     w = make_workload(c, n=n, m=m, n_epochs=E)
+    monkeypatch.setenv("DIA_DISABLE_SMALL", "1")
     outs = []
     for disable in ("0", "1"):
         monkeypatch.setenv("DIA_DISABLE_CLUSTER", disable)

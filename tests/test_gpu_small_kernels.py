@@ -1,6 +1,5 @@
-"""GPU-vs-oracle parity of the register-resident kernel for small kernels (m = 1, 3; dia_eval_small.cuh), which
-evaluates the plain objective (no mask / flat / variance map / background polynomial) of handles with m <= 3
-(m = 5 is listed too: it runs the generic kernel on the same shapes).
+"""GPU-vs-oracle parity of the register-resident kernel for small kernels (m = 1, 3, 5; dia_eval_small.cuh), which
+evaluates the plain objective (no mask / flat / variance map / background polynomial) of handles with m <= 5.
 
 Same protocol as tests/test_gpu_parity.py (loss to 1e-5 relative, gradient to 1e-5 of the cancellation-free scale S_p),
 on shapes chosen for this kernel's geometry: 8-pixel strips, lanes side by side up to 256 columns, 2-16 rows per thread,
@@ -74,7 +73,7 @@ def test_small_kernel_parity(dia, nr, nc, m, loss):
     h.close()
 
 
-@pytest.mark.parametrize("m", [1, 3])
+@pytest.mark.parametrize("m", [1, 3, 5])
 def test_small_kernel_is_the_one_that_runs_and_agrees_with_the_generic_kernel(dia, monkeypatch, m):
     """DIA_DISABLE_SMALL=1 forces the generic shared-memory kernel: both must agree with the oracle, and with each other
     far inside the tolerance; a mask (generic kernel on the same handle) of all ones gives the generic result."""
