@@ -97,6 +97,40 @@ def test_small_kernel_is_the_one_that_runs_and_agrees_with_the_generic_kernel(di
     assert (Lm - Lg).abs().max() <= 1e-6 * Lg.abs().max()
 
 
+@pytest.mark.parametrize("m", [1, 3, 5])
+def test_small_kernel_right_edge_positions(dia, monkeypatch, m):
+    """The ragged right edge, lane by lane.  A warp's 32 strips of 8 pixels either all take the unpredicated path or all
+    the predicated one, and the last strip may hold 1 .. 8 valid pixels: widths are chosen so that the edge falls into
+    the first, a middle and the last lane of a warp, in the first and in a later tile column, with 16-byte aligned rows
+    (128-bit loads) and without.  Several tile rows on three CTAs, so that the rotation of the tile columns by the tile
+    row meets every column.  Against the oracle at the parity tolerance, and against the generic kernel on the same data
+    (DIA_DISABLE_SMALL=1) far inside it; both deterministic."""
+    widths = [16, 20, 36, 132, 136, 140, 250, 256, 260, 264, 268, 508, 512, 516, 520, 772, 1028, 333, 262, 515]
+    rows = 150
+    w = make_workload(4, n=1028, m=m, n_epochs=2)
+    th = w.theta_true.astype(np.float32)
+    res = {}
+    for disable in ("0", "1"):
+        monkeypatch.setenv("DIA_DISABLE_SMALL", disable)
+        monkeypatch.setenv("DIA_GRID_LIMIT", "3")
+        for nc in widths:
+            R, I = _crop(w, rows, nc)
+            h = dia.Handle(_dev(R), m, max_epochs=2, sigma0=w.sigma0, gain=w.gain)
+            L, g = h.eval_loss_grad(_dev(I), _dev(th))
+            L2, g2 = h.eval_loss_grad(_dev(I), _dev(th))
+            assert torch.equal(L, L2) and torch.equal(g, g2), f"width {nc}: evaluation is not deterministic"
+            res[(disable, nc)] = (L.cpu().numpy(), g.cpu().numpy())
+            h.close()
+    for nc in widths:
+        (Ls, gs), (Lg, gg) = res[("0", nc)], res[("1", nc)]
+        R, I = _crop(w, rows, nc)
+        cfg = oracle.RefConfig(rows, nc, m, sigma0=w.sigma0, gain=w.gain)
+        Lo, go, So = oracle.eval_loss_grad(cfg, R, I, th, want_scale=True)
+        _compare(torch.from_numpy(Ls), torch.from_numpy(gs), Lo, go, So, "S", f"small m={m} width {nc}")
+        assert np.abs(Ls - Lg).max() <= 1e-6 * np.abs(Lg).max(), f"width {nc}: loss {Ls} vs {Lg}"
+        assert (np.abs(gs - gg) / So).max() <= 5e-6, f"width {nc}: small and generic kernel differ by {(np.abs(gs - gg) / So).max():.3e} of S"
+
+
 @pytest.mark.parametrize("grid_limit", [1, 3])
 def test_small_kernel_many_tiles_per_cta_batched_and_singles(dia, monkeypatch, grid_limit):
     """One or three CTAs walk through every (epoch, tile) item: epoch changes inside a CTA, partial columns shared by
