@@ -1,15 +1,17 @@
 // dia_eval_small.cuh -- fused loss + gradient kernel for SMALL kernels (m = 1, 3, 5), plain objective only
 // (Eq. 2, 6, 8 / 12-13; no mask, flat field, variance map, background polynomial).
 //
-// For m <= 5 the evaluation has 4 m^2 <= 100 FLOP per 8 bytes of image: the roofline is HBM bandwidth (m <= 3) or
-// instruction issue, not the FMA pipe, and the generic kernel's shared-memory tiles (w tile, gradient strips, two
-// barriers per tile) cost more instructions per pixel than the arithmetic itself (87 per pixel at m = 3, ncu reading
-// in profiles/r01_sweeps.md).  Here everything stays in registers:
+// For m <= 5 the evaluation has 4 m^2 <= 100 FLOP per 8 bytes of image: the algorithmic roofline is HBM bandwidth, and
+// the generic kernel's shared-memory tiles (w tile, gradient strips, two barriers per tile) cost more instructions per
+// pixel than the arithmetic itself (87 per pixel at m = 3, ncu reading in profiles/r01_sweeps.md).  What this kernel
+// runs out of in practice is the FMA pipe at the ~50 % that 8 - 16 warps per SM can keep busy (the per-pixel terms'
+// FP32 operations count as much as the stencil's; profiles/r02_small3.md).  Here everything stays in registers:
 //   * a thread owns an 8-pixel row strip and walks down `rpt` rows with a sliding window of the m reference rows it
 //     needs (one new row of 8 + m - 1 reference pixels and 8 target pixels per step, 128-bit loads straight from
 //     global memory, the rows two steps ahead requested by prefetch.global.L1 -- neighbouring threads' halo re-reads
 //     hit L1); lanes of a warp sit side by side (coalesced 1 KB rows);
-//   * M, residual, variance, loss term and w = dL/dM per pixel: the generic kernel's formulas, ln v from lg2.approx;
+//   * M, residual, variance, loss term and w = dL/dM per pixel: the generic kernel's formulas (rearranged for the
+//     Gaussian loss: small_gauss_terms), ln v from lg2.approx;
 //   * the m^2 gradient sums g[a][b] += w_q R[a][q + b] reuse the window registers: no w tile, no second pass;
 //   * per tile the m^2 FP32 sums are reduced across the warp by a transposing butterfly (lane k ends up with sum k)
 //     and added to a lane-held FP64 total; loss and g_B0 go to thread-private FP64 every row.
